@@ -1,0 +1,174 @@
+/*
+ * cs.h -- C ABI of libcs.so: the Count-Sketch heavy-hitter pass of arXiv 1711.00975 on one B200 (sm_100a).
+ *
+ * Problem statement this boundary follows (PAPER.md = the paper's text; DESIGN.md section 3 = readings):
+ *   given N-body particles in a box and a regular G^3 mesh, return the k cells holding the most particles
+ *   with an estimate of each count, and the excursion set = all cells whose estimated
+ *   count is at least a limit, in ONE streaming pass over the particles into a
+ *   Count Sketch plus one replay of the stream against the finished sketch
+ *   (estimate mode, restricted to the cells that occur in the stream).
+ *
+ * Conventions for every call
+ *   - extern "C", returns an int status: CS_OK (0) or a negative CS_ERR_* code.  Nothing throws, aborts or
+ *     prints.  cs_last_error() returns a thread-local, NUL-terminated message for the last failing call.
+ *   - "dev" pointers are CUDA device memory on the current device; "host" pointers are host memory (pinned
+ *     memory makes the host-streamed calls asynchronous, pageable memory is accepted and slower); "any"
+ *     pointers may be either (the library copies with cudaMemcpyDefault).
+ *   - The caller owns every input / output buffer.  The handle owns the counter tables, the candidate buffers,
+ *     the staging ring and all scratch; cs_destroy frees them.
+ *   - All device work is enqueued on the handle's stream (cs_set_stream; default: the legacy default stream).
+ *     cs_update / cs_estimate / cs_sketch_add / cs_reset do not synchronise.  cs_update_host returns after the
+ *     last host->device copy has been issued and waited for (the host buffer may then be reused); cs_scan*,
+ *     cs_topk, cs_excursion, cs_sketch_read, cs_scan_stats synchronise the stream because they hand
+ *     host-visible results or sizes back.
+ *   - Positions are an array of structures: float32 x,y,z per particle, 12 bytes per particle, at least
+ *     4-byte aligned (16-byte aligned input takes the fully vectorised path from its first particle).
+ *   - There is no CPU fallback: every step below runs in CUDA kernels of this library; without a usable
+ *     CUDA device cs_create fails with CS_ERR_CUDA.
+ *
+ * Arithmetic (bit-exact contract; the paper fixes only "2-independent hashes",
+ * PAPER.md:105, and "4-byte integer counters"):
+ *   p = 2^61 - 1.  splitmix64 stream of seed: x_n = mix64(seed + n*0x9E3779B97F4A7C15), n = 1, 2, ...
+ *   Row j of a scale takes x_{4j+1..4j+4} as a_j, b_j, a'_j, b'_j with a = (x mod (p-1)) + 1, b = x mod p;
+ *   sampling key K = x_{4d+1} of scale 0; scale s draws from the stream of seed + s.
+ *   quantise: per axis i = (uint32) min(max(floorf(x * (float)((double)G / L)), 0), G-1)  (one IEEE binary32
+ *   multiply, no FMA; NaN -> 0);  cell id c = ix + G*(iy + G*iz)  (uint64).
+ *   bucket h_j(c) = ((a_j*c + b_j) mod p) mod w;  sign s_j(c) = 1 - 2*(((a'_j*c + b'_j) mod p) & 1).
+ *   Add(c): T[j][h_j(c)] += s_j(c) for every row j (int32, wraparound)
+ *   Estimate(c) = the floor((d-1)/2)-th smallest (0-based) of s_j(c)*T[j][h_j(c)]
+ *   sampling (sample_p < 1): the particle with running index i (0-based, counted over every particle passed
+ *   in, kept or not) is kept iff mix64(K + (i+1)*0x9E3779B97F4A7C15) < floor(sample_p * 2^64).
+ */
+#ifndef CS_H_
+#define CS_H_
+
+#include <stdint.h>
+
+#ifdef __cplusplus
+extern "C" {
+#endif
+
+#define CS_OK          0
+#define CS_ERR_ARG    -1   /* invalid argument (ranges below), null pointer with a non-zero size */
+#define CS_ERR_NOMEM  -2   /* host or device allocation failed */
+#define CS_ERR_CUDA   -3   /* a CUDA runtime call or kernel failed; text in cs_last_error() */
+#define CS_ERR_STATE  -4   /* call out of order (cs_scan / cs_topk / cs_excursion before cs_scan_begin) */
+
+#define CS_MAX_ROWS    32  /* d */
+#define CS_MAX_SCALES  8   /* grids sketched in one pass */
+#define CS_MAX_HASH_ROWS 64 /* n_scales * d: all hash coefficients travel as kernel parameters */
+
+typedef struct cs_sketch cs_sketch;   /* opaque */
+
+/* ---- host-only helpers (no CUDA device needed) --------------------------------------------------------- */
+
+/* Library version string, e.g. "cs-b200 0.1 (sm_100a)". */
+const char* cs_version(void);
+
+/* Message of the last failing call on this thread ("" if none). */
+const char* cs_last_error(void);
+
+/* Hash coefficients of one scale, as the library derives them on the host (R1-R2):
+ * out_4d[4*j + 0..3] = a_j, b_j, a'_j, b'_j for j < d; *K_out (may be NULL) = sampling key x_{4d+1}.
+ * 1 <= d <= CS_MAX_ROWS.  Pure host arithmetic. */
+int cs_derive_coeffs(uint64_t seed, int d, uint64_t* out_4d, uint64_t* K_out);
+
+/* floor(sample_p * 2^64) as the sampler compares against (R13); 0 for p outside (0, 1). */
+uint64_t cs_sample_threshold(double sample_p);
+
+/* ---- life cycle --------------------------------------------------------------------------------------- */
+
+/* cs_create: one sketch of d rows x w int32 counters over a G^3 mesh on a box of side L.
+ * cs_create_multi: n_scales sketches (same d, w; grid G[s], coefficients from seed + s) updated and scanned
+ * together in one pass over the particles with one sampling decision per particle.
+ * Ranges: 1 <= d <= 32, 1 <= w <= 2^31, 1 <= G <= 2^20 (so G^3 <= 2^60 < p), L finite and > 0,
+ * 1 <= n_scales <= 8, n_scales*d <= 64.  Allocates d*w*4 bytes per scale, zeroed.  *out receives the handle. */
+int cs_create(cs_sketch** out, int d, uint64_t w, uint32_t G, double L, uint64_t seed);
+int cs_create_multi(cs_sketch** out, int n_scales, int d, uint64_t w, const uint32_t* G_host, double L,
+                    uint64_t seed);
+int cs_destroy(cs_sketch* s);                       /* NULL is accepted */
+
+/* Zero the tables, the running particle indices and the candidates; leaves scan mode. */
+int cs_reset(cs_sketch* s);
+
+/* Use `cuda_stream` (a cudaStream_t, e.g. torch.cuda.current_stream().cuda_stream) for all later work. */
+int cs_set_stream(cs_sketch* s, void* cuda_stream);
+
+/* Running particle index of the update stream / of the current scan (sampling, R13, R17).
+ * Setting it lets a stream shard (multi-GPU) reproduce the single-stream sampling decisions. */
+int cs_set_update_index(cs_sketch* s, uint64_t index);
+int cs_set_scan_index(cs_sketch* s, uint64_t index);
+int cs_get_update_index(cs_sketch* s, uint64_t* index_out);
+
+/* ---- stream processing: Alg. 1 l.3-5, Add(M, cell) per kept particle ------ */
+
+/* n particles at xyz_dev (device, AoS float32).  sample_p in (0, 1]; 1 keeps everything and computes no
+ * sampling hash.  n = 0 is a no-op.  Asynchronous on the handle's stream. */
+int cs_update(cs_sketch* s, const float* xyz_dev, uint64_t n, double sample_p);
+
+/* Same for particles in HOST memory: copied in batches through a ring of device staging buffers with
+ * cudaMemcpyAsync on a copy stream, overlapped with the update kernel of the previous batch
+ * (PAPER.md:295-298 batch flow, :570 I/O overlapped with compute). */
+int cs_update_host(cs_sketch* s, const float* xyz_host, uint64_t n, double sample_p);
+
+/* ---- queries ------------------------------------------------------------------------------------------ */
+
+/* est_dev[i] = Estimate(cells_dev[i]) against scale `scale`.  m = 0 is a no-op.
+ * Cells >= G^3 are hashed like any other 64-bit id below 2^61 (ids >= 2^61 give CS_ERR_ARG is NOT checked on
+ * the device: the caller passes ids < G^3). */
+int cs_estimate(cs_sketch* s, int scale, const uint64_t* cells_dev, uint64_t m, int32_t* est_dev);
+
+/* Candidate re-scan (estimate mode restricted to the cells that occur in the replayed stream; R10).
+ * cs_scan_begin clears the candidates and the scan index and fixes what may be asked afterwards:
+ *   top-k for any k <= k_max, excursion sets for any threshold >= thr_min
+ *   (k_max = 0: no top-k; thr_min = INT32_MAX: no excursion set).
+ * cs_scan / cs_scan_host replay particles (normally the same stream with the same sample_p, after the last
+ * cs_update): every kept particle's cell is estimated against the CURRENT tables; cells whose estimate can
+ * still matter are collected, deduplicated and kept ordered by (estimate descending, cell id ascending).
+ * The tables must not change between cs_scan_begin and the last cs_topk / cs_excursion. */
+int cs_scan_begin(cs_sketch* s, uint64_t k_max, int32_t thr_min);
+int cs_scan(cs_sketch* s, const float* xyz_dev, uint64_t n, double sample_p);
+int cs_scan_host(cs_sketch* s, const float* xyz_host, uint64_t n, double sample_p);
+
+/* Feed cell ids directly as candidates of `scale` (estimated against the current tables, deduplicated with the
+ * scanned ones).  Used to merge the candidate lists of several stream shards. */
+int cs_scan_cells(cs_sketch* s, int scale, const uint64_t* cells_dev, uint64_t m);
+
+/* Top-k (made deterministic, R9): the first min(k, #candidates)
+ * candidates in (estimate descending, cell id ascending) order.  ids_out / est_out: any pointer, room for k
+ * entries; *n_out (host) = number written.  k <= k_max. */
+int cs_topk(cs_sketch* s, int scale, uint64_t k, uint64_t* ids_out, int32_t* est_out, uint64_t* n_out);
+
+/* Excursion set (R8): every candidate with estimate >= thr, same order.  Writes the
+ * first min(cap, total) entries; *n_total (host) = total.  thr >= thr_min.  Raw estimates, no 1/p rescale. */
+int cs_excursion(cs_sketch* s, int scale, int32_t thr, uint64_t cap, uint64_t* ids_out, int32_t* est_out,
+                 uint64_t* n_total);
+
+/* out4[0] = candidates currently held, out4[1] = current collection threshold tau as (uint64)(int64)tau,
+ * out4[2] = compactions run since cs_scan_begin, out4[3] = scan kernel launches since cs_scan_begin. */
+int cs_scan_stats(cs_sketch* s, int scale, uint64_t* out4_host);
+
+/* ---- table access: save / restore / merge by linearity ----------------------------------- */
+
+int cs_sketch_read(cs_sketch* s, int scale, int32_t* out_d_by_w);       /* any pointer; row-major T[j*w + b] */
+int cs_sketch_add(cs_sketch* s, int scale, const int32_t* in_d_by_w);   /* any pointer; T += in, wraparound  */
+int cs_coeffs(cs_sketch* s, int scale, uint64_t* out_4d_host, uint64_t* K_out_host);
+
+/* Number of kernels this handle has launched since create (bench.py's gpu_launches). */
+int cs_launch_count(cs_sketch* s, uint64_t* n_out);
+
+/* ---- measurement probes (the roofline denominators are measured, not assumed) ------------- */
+
+/* Issues n_ops red.global.add.s32 (mode 0), returning atom.global.add.s32 (mode 1) or 4-byte ld.global
+ * gathers (mode 2) to addresses generated in registers, uniform over a table of table_bytes, from all SMs,
+ * `reps` times, on `cuda_stream`; *ms_out = average device time of one repetition (CUDA events). */
+int cs_probe_l2(int mode, uint64_t table_bytes, uint64_t n_ops, int reps, void* cuda_stream, double* ms_out);
+
+/* Same stream-read shape as cs_update (16-byte loads of n particles) with no hashing or atomics:
+ * the position-stream term of the roofline.  *ms_out = average device time of one pass. */
+int cs_probe_stream(const float* xyz_dev, uint64_t n, int reps, void* cuda_stream, double* ms_out);
+
+#ifdef __cplusplus
+}
+#endif
+#endif /* CS_H_ */

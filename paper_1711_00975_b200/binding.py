@@ -1,0 +1,255 @@
+"""Thin ctypes binding over libcs.so (include/cs.h).  Argument marshalling only: every step of the path runs
+in the library's CUDA kernels.  torch is used for device memory and streams.  There is no CPU fallback: if the
+library is missing or fails to load, importing succeeds but the first use raises.
+"""
+from __future__ import annotations
+
+import ctypes as C
+from pathlib import Path
+
+import torch
+
+_PKG = Path(__file__).resolve().parent
+LIB_PATH = _PKG / "libcs.so"
+
+CS_OK, CS_ERR_ARG, CS_ERR_NOMEM, CS_ERR_CUDA, CS_ERR_STATE = 0, -1, -2, -3, -4
+INT32_MIN, INT32_MAX = -(2 ** 31), 2 ** 31 - 1
+
+u64, i32, u32, dbl, vp, ci = C.c_uint64, C.c_int32, C.c_uint32, C.c_double, C.c_void_p, C.c_int
+
+# name -> (restype, argtypes); every symbol include/cs.h declares
+SIGNATURES = {
+    "cs_version": (C.c_char_p, []),
+    "cs_last_error": (C.c_char_p, []),
+    "cs_derive_coeffs": (ci, [u64, ci, vp, vp]),
+    "cs_sample_threshold": (u64, [dbl]),
+    "cs_create": (ci, [vp, ci, u64, u32, dbl, u64]),
+    "cs_create_multi": (ci, [vp, ci, ci, u64, vp, dbl, u64]),
+    "cs_destroy": (ci, [vp]),
+    "cs_reset": (ci, [vp]),
+    "cs_set_stream": (ci, [vp, vp]),
+    "cs_set_update_index": (ci, [vp, u64]),
+    "cs_set_scan_index": (ci, [vp, u64]),
+    "cs_get_update_index": (ci, [vp, vp]),
+    "cs_update": (ci, [vp, vp, u64, dbl]),
+    "cs_update_host": (ci, [vp, vp, u64, dbl]),
+    "cs_estimate": (ci, [vp, ci, vp, u64, vp]),
+    "cs_scan_begin": (ci, [vp, u64, i32]),
+    "cs_scan": (ci, [vp, vp, u64, dbl]),
+    "cs_scan_host": (ci, [vp, vp, u64, dbl]),
+    "cs_scan_cells": (ci, [vp, ci, vp, u64]),
+    "cs_topk": (ci, [vp, ci, u64, vp, vp, vp]),
+    "cs_excursion": (ci, [vp, ci, i32, u64, vp, vp, vp]),
+    "cs_scan_stats": (ci, [vp, ci, vp]),
+    "cs_sketch_read": (ci, [vp, ci, vp]),
+    "cs_sketch_add": (ci, [vp, ci, vp]),
+    "cs_coeffs": (ci, [vp, ci, vp, vp]),
+    "cs_launch_count": (ci, [vp, vp]),
+    "cs_probe_l2": (ci, [ci, u64, u64, ci, vp, vp]),
+    "cs_probe_stream": (ci, [vp, u64, ci, vp, vp]),
+}
+
+_lib = None
+
+
+class CsError(RuntimeError):
+    def __init__(self, code: int, what: str, msg: str):
+        super().__init__(f"{what} failed with status {code}: {msg}")
+        self.code = code
+
+
+def lib():
+    """Loads libcs.so (built by paper_1711_00975_b200.build).  Raises if it is missing: no fallback."""
+    global _lib
+    if _lib is None:
+        if not LIB_PATH.exists():
+            raise RuntimeError(f"{LIB_PATH} is missing: run `python -m paper_1711_00975_b200.build` "
+                               "(the CUDA library is the only implementation; there is no CPU fallback)")
+        L = C.CDLL(str(LIB_PATH))
+        for name, (res, args) in SIGNATURES.items():
+            f = getattr(L, name)
+            f.restype = res
+            f.argtypes = args
+        _lib = L
+    return _lib
+
+
+def _chk(rc: int, what: str):
+    if rc != 0:
+        raise CsError(rc, what, lib().cs_last_error().decode())
+
+
+def version() -> str:
+    return lib().cs_version().decode()
+
+
+def derive_coeffs(seed: int, d: int):
+    """Host-only: (d x 4 array of a, b, a', b'; sampling key K) as the library derives them."""
+    import numpy as np
+    out = np.empty(4 * d, dtype=np.uint64)
+    K = u64(0)
+    _chk(lib().cs_derive_coeffs(seed, d, out.ctypes.data_as(vp), C.byref(K)), "cs_derive_coeffs")
+    return out.reshape(d, 4), int(K.value)
+
+
+def sample_threshold(p: float) -> int:
+    return int(lib().cs_sample_threshold(p))
+
+
+def _dev_xyz(xyz: torch.Tensor):
+    if not xyz.is_cuda or xyz.dtype != torch.float32 or not xyz.is_contiguous() or xyz.numel() % 3:
+        raise ValueError("positions must be a contiguous CUDA float32 tensor with 3 floats per particle")
+    return xyz.data_ptr(), xyz.numel() // 3
+
+
+def _host_xyz(xyz: torch.Tensor):
+    if xyz.is_cuda or xyz.dtype != torch.float32 or not xyz.is_contiguous() or xyz.numel() % 3:
+        raise ValueError("positions must be a contiguous CPU float32 tensor with 3 floats per particle")
+    return xyz.data_ptr(), xyz.numel() // 3
+
+
+class CountSketch:
+    """cs_sketch handle.  Methods mirror the C calls of include/cs.h one to one."""
+
+    def __init__(self, d: int, w: int, G, L: float, seed: int, stream: torch.cuda.Stream | None = None):
+        Gs = [int(G)] if isinstance(G, int) else [int(g) for g in G]
+        self.d, self.w, self.G, self.L, self.seed = int(d), int(w), Gs, float(L), int(seed)
+        self.n_scales = len(Gs)
+        self._h = vp(None)
+        arr = (u32 * len(Gs))(*Gs)
+        _chk(lib().cs_create_multi(C.byref(self._h), self.n_scales, self.d, self.w, arr, self.L, self.seed),
+             "cs_create_multi")
+        self.device = torch.device("cuda", torch.cuda.current_device())
+        self.set_stream(stream if stream is not None else torch.cuda.current_stream())
+
+    # -- life cycle
+    def close(self):
+        if self._h:
+            lib().cs_destroy(self._h)
+            self._h = vp(None)
+
+    def __del__(self):
+        try:
+            self.close()
+        except Exception:
+            pass
+
+    def reset(self):
+        _chk(lib().cs_reset(self._h), "cs_reset")
+
+    def set_stream(self, stream: torch.cuda.Stream):
+        self._stream = stream
+        _chk(lib().cs_set_stream(self._h, vp(stream.cuda_stream)), "cs_set_stream")
+
+    def set_update_index(self, index: int):
+        _chk(lib().cs_set_update_index(self._h, index), "cs_set_update_index")
+
+    def set_scan_index(self, index: int):
+        _chk(lib().cs_set_scan_index(self._h, index), "cs_set_scan_index")
+
+    def update_index(self) -> int:
+        v = u64(0)
+        _chk(lib().cs_get_update_index(self._h, C.byref(v)), "cs_get_update_index")
+        return int(v.value)
+
+    # -- stream processing
+    def update(self, xyz: torch.Tensor, sample_p: float = 1.0):
+        p, n = _dev_xyz(xyz)
+        _chk(lib().cs_update(self._h, vp(p), n, sample_p), "cs_update")
+
+    def update_host(self, xyz: torch.Tensor, sample_p: float = 1.0):
+        p, n = _host_xyz(xyz)
+        _chk(lib().cs_update_host(self._h, vp(p), n, sample_p), "cs_update_host")
+
+    # -- queries
+    def estimate(self, cells: torch.Tensor, scale: int = 0) -> torch.Tensor:
+        if not cells.is_cuda or cells.dtype not in (torch.int64, torch.uint64) or not cells.is_contiguous():
+            raise ValueError("cells must be a contiguous CUDA int64/uint64 tensor")
+        out = torch.empty(cells.numel(), dtype=torch.int32, device=cells.device)
+        _chk(lib().cs_estimate(self._h, scale, vp(cells.data_ptr()), cells.numel(), vp(out.data_ptr())), "cs_estimate")
+        return out
+
+    def scan_begin(self, k_max: int, thr_min: int = INT32_MAX):
+        _chk(lib().cs_scan_begin(self._h, k_max, thr_min), "cs_scan_begin")
+
+    def scan(self, xyz: torch.Tensor, sample_p: float = 1.0):
+        p, n = _dev_xyz(xyz)
+        _chk(lib().cs_scan(self._h, vp(p), n, sample_p), "cs_scan")
+
+    def scan_host(self, xyz: torch.Tensor, sample_p: float = 1.0):
+        p, n = _host_xyz(xyz)
+        _chk(lib().cs_scan_host(self._h, vp(p), n, sample_p), "cs_scan_host")
+
+    def scan_cells(self, cells: torch.Tensor, scale: int = 0):
+        if not cells.is_cuda or cells.dtype not in (torch.int64, torch.uint64) or not cells.is_contiguous():
+            raise ValueError("cells must be a contiguous CUDA int64/uint64 tensor")
+        _chk(lib().cs_scan_cells(self._h, scale, vp(cells.data_ptr()), cells.numel()), "cs_scan_cells")
+
+    def topk(self, k: int, scale: int = 0, device=None):
+        """(ids int64 tensor holding the uint64 cell ids, est int32 tensor), on `device` (default: the GPU)."""
+        device = self.device if device is None else torch.device(device)
+        ids = torch.empty(max(k, 1), dtype=torch.int64, device=device)
+        est = torch.empty(max(k, 1), dtype=torch.int32, device=device)
+        n = u64(0)
+        _chk(lib().cs_topk(self._h, scale, k, vp(ids.data_ptr()), vp(est.data_ptr()), C.byref(n)), "cs_topk")
+        return ids[: n.value], est[: n.value]
+
+    def excursion(self, thr: int, scale: int = 0, cap: int | None = None, device=None):
+        """(ids, est, total): all candidates with estimate >= thr (the first `cap` of them if cap is given)."""
+        device = self.device if device is None else torch.device(device)
+        n = u64(0)
+        if cap is None:      # size query first, then fetch everything
+            _chk(lib().cs_excursion(self._h, scale, thr, 0, None, None, C.byref(n)), "cs_excursion")
+            cap = int(n.value)
+        ids = torch.empty(max(cap, 1), dtype=torch.int64, device=device)
+        est = torch.empty(max(cap, 1), dtype=torch.int32, device=device)
+        _chk(lib().cs_excursion(self._h, scale, thr, cap, vp(ids.data_ptr()), vp(est.data_ptr()), C.byref(n)),
+             "cs_excursion")
+        m = min(int(n.value), cap)
+        return ids[:m], est[:m], int(n.value)
+
+    def scan_stats(self, scale: int = 0) -> dict:
+        out = (u64 * 4)()
+        _chk(lib().cs_scan_stats(self._h, scale, out), "cs_scan_stats")
+        tau = out[1] - (1 << 64) if out[1] >= (1 << 63) else out[1]
+        return {"candidates": int(out[0]), "tau": int(tau), "compactions": int(out[2]), "scan_launches": int(out[3])}
+
+    # -- table access
+    def sketch(self, scale: int = 0, device=None) -> torch.Tensor:
+        device = self.device if device is None else torch.device(device)
+        out = torch.empty((self.d, self.w), dtype=torch.int32, device=device)
+        _chk(lib().cs_sketch_read(self._h, scale, vp(out.data_ptr())), "cs_sketch_read")
+        return out
+
+    def sketch_add(self, table: torch.Tensor, scale: int = 0):
+        if table.dtype != torch.int32 or not table.is_contiguous() or table.numel() != self.d * self.w:
+            raise ValueError("table must be a contiguous int32 tensor with d*w entries")
+        _chk(lib().cs_sketch_add(self._h, scale, vp(table.data_ptr())), "cs_sketch_add")
+
+    def coeffs(self, scale: int = 0):
+        import numpy as np
+        out = np.empty(4 * self.d, dtype=np.uint64)
+        K = u64(0)
+        _chk(lib().cs_coeffs(self._h, scale, out.ctypes.data_as(vp), C.byref(K)), "cs_coeffs")
+        return out.reshape(self.d, 4), int(K.value)
+
+    def launch_count(self) -> int:
+        v = u64(0)
+        _chk(lib().cs_launch_count(self._h, C.byref(v)), "cs_launch_count")
+        return int(v.value)
+
+
+def probe_l2(mode: int, table_bytes: int, n_ops: int, reps: int = 3, stream: torch.cuda.Stream | None = None) -> float:
+    """Average ms of one repetition of n_ops red (0) / atom (1) / gather (2) operations over a table."""
+    st = stream if stream is not None else torch.cuda.current_stream()
+    ms = dbl(0.0)
+    _chk(lib().cs_probe_l2(mode, table_bytes, n_ops, reps, vp(st.cuda_stream), C.byref(ms)), "cs_probe_l2")
+    return float(ms.value)
+
+
+def probe_stream(xyz: torch.Tensor, reps: int = 3, stream: torch.cuda.Stream | None = None) -> float:
+    p, n = _dev_xyz(xyz)
+    st = stream if stream is not None else torch.cuda.current_stream()
+    ms = dbl(0.0)
+    _chk(lib().cs_probe_stream(vp(p), n, reps, vp(st.cuda_stream), C.byref(ms)), "cs_probe_stream")
+    return float(ms.value)

@@ -1,0 +1,795 @@
+/*
+ * cs_api.cu -- host runtime and C ABI of libcs.so (include/cs.h): handle, hash-coefficient derivation,
+ * launch scheduling of the update / scan passes, candidate-buffer management (chunking, compaction, growth),
+ * double-buffered host streaming.  Every step of the path runs in the CUDA kernels of cs_kernels.cu,
+ * cs_scan.cu and cs_select.cu; there is no CPU fallback and nothing here touches oracle/.
+ */
+#include <cmath>
+#include <cstdarg>
+#include <cstdio>
+#include <cstring>
+#include <new>
+
+#include "cs_internal.h"
+
+using namespace cs;
+
+namespace {
+
+thread_local char g_err[512] = "";
+
+int fail(int code, const char* fmt, ...) {
+    va_list ap;
+    va_start(ap, fmt);
+    vsnprintf(g_err, sizeof(g_err), fmt, ap);
+    va_end(ap);
+    return code;
+}
+
+#define CS_CUDA(call)                                                                              \
+    do {                                                                                           \
+        cudaError_t e_ = (call);                                                                   \
+        if (e_ != cudaSuccess)                                                                     \
+            return fail(e_ == cudaErrorMemoryAllocation ? CS_ERR_NOMEM : CS_ERR_CUDA, "%s: %s",    \
+                        #call, cudaGetErrorString(e_));                                            \
+    } while (0)
+
+/* ---- host arithmetic: splitmix64 stream and coefficient derivation (R1-R2) ------------------- */
+
+uint64_t host_mix64(uint64_t z) {
+    z = (z ^ (z >> 30)) * 0xBF58476D1CE4E5B9ULL;
+    z = (z ^ (z >> 27)) * 0x94D049BB133111EBULL;
+    return z ^ (z >> 31);
+}
+
+uint64_t stream_at(uint64_t seed, uint64_t n) { return host_mix64(seed + n * GAMMA); }
+
+void derive_coeffs(uint64_t seed, int d, uint64_t* out_4d, uint64_t* K_out) {
+    for (int j = 0; j < d; ++j) {
+        const uint64_t n0 = 4 * (uint64_t)j;
+        out_4d[4 * j + 0] = stream_at(seed, n0 + 1) % (P61 - 1) + 1;   /* a  in [1, p-1] */
+        out_4d[4 * j + 1] = stream_at(seed, n0 + 2) % P61;             /* b  in [0, p-1] */
+        out_4d[4 * j + 2] = stream_at(seed, n0 + 3) % (P61 - 1) + 1;   /* a' */
+        out_4d[4 * j + 3] = stream_at(seed, n0 + 4) % P61;             /* b' */
+    }
+    if (K_out) *K_out = stream_at(seed, 4 * (uint64_t)d + 1);
+}
+
+HashCoef split_coef(uint64_t a, uint64_t b) {
+    HashCoef k;
+    k.a0 = (uint32_t)(a & 0x7FFFFFFFu);
+    k.ah = (uint32_t)(a >> 31);
+    /* A = a * 2^32 mod p: a = x*2^29 + y (y < 2^29)  =>  a*2^32 = x*2^61 + y*2^32 == x + y*2^32 */
+    uint64_t A = (a >> 29) + ((a & 0x1FFFFFFFULL) << 32);
+    if (A >= P61) A -= P61;
+    k.A0 = (uint32_t)(A & 0x7FFFFFFFu);
+    k.Ah = (uint32_t)(A >> 31);
+    k.b = b;
+    return k;
+}
+
+uint64_t sample_threshold(double p) {
+    if (!(p > 0.0) || !(p < 1.0)) return 0;
+    return (uint64_t)std::floor(std::ldexp(p, 64));
+}
+
+int bit_length(uint64_t v) {
+    int b = 0;
+    while (v) { ++b; v >>= 1; }
+    return b;
+}
+
+constexpr int STAGE_SLOTS = 3;
+constexpr uint64_t STAGE_PARTICLES = 1ull << 24;      /* 192 MiB per staging slot */
+constexpr uint64_t MAX_CHUNK = 1ull << 26;            /* particles per scan launch */
+constexpr uint32_t MIN_CAP = 1u << 22;                /* candidate entries per scale */
+
+}  // namespace
+
+struct cs_sketch {
+    int d = 0, n_scales = 0, device = 0, sm_count = 148;
+    uint64_t w = 0, seed = 0, K = 0;
+    double L = 0;
+    uint32_t G[CS_MAX_SCALES] = {};
+    int id_bits[CS_MAX_SCALES] = {};
+    uint64_t coef[CS_MAX_SCALES][4 * CS_MAX_ROWS] = {};
+    PassParams P = {};
+    int32_t* T[CS_MAX_SCALES] = {};
+    cudaStream_t stream = nullptr;
+    uint64_t upd_index = 0, scan_index = 0, launches = 0;
+
+    /* candidate collection */
+    bool scanning = false;
+    uint64_t k_max = 0;
+    int32_t thr_min = INT32_MAX;
+    uint32_t cap = 0;
+    SelectBuffers sb[CS_MAX_SCALES] = {};
+    int cur[CS_MAX_SCALES] = {};
+    bool dirty[CS_MAX_SCALES] = {};
+    uint32_t last_compact[CS_MAX_SCALES] = {};
+    uint64_t n_compactions[CS_MAX_SCALES] = {};
+    uint64_t n_scan_launches = 0;
+    double rate = 1.0;
+    bool first_chunk = true;
+    ScanState* st_dev = nullptr;      /* CS_MAX_SCALES entries */
+    ScanState* st_host = nullptr;     /* pinned mirror */
+    uint32_t* word_dev = nullptr;     /* 1 scratch word */
+    uint32_t* word_host = nullptr;    /* pinned */
+    uint64_t* out_ids = nullptr;      /* staging for cs_topk / cs_excursion results */
+    int32_t* out_est = nullptr;
+    uint64_t out_cap = 0;
+
+    /* host streaming */
+    float* stage[STAGE_SLOTS] = {};
+    cudaStream_t copy_stream = nullptr;
+    cudaEvent_t ev_full[STAGE_SLOTS] = {}, ev_free[STAGE_SLOTS] = {};
+};
+
+namespace {
+
+void free_candidates(cs_sketch* s) {
+    for (int i = 0; i < CS_MAX_SCALES; ++i) {
+        for (int h = 0; h < 2; ++h) {
+            if (s->sb[i].id[h]) cudaFree(s->sb[i].id[h]);
+            if (s->sb[i].ek[h]) cudaFree(s->sb[i].ek[h]);
+            s->sb[i].id[h] = nullptr;
+            s->sb[i].ek[h] = nullptr;
+        }
+        if (s->sb[i].scratch) cudaFree(s->sb[i].scratch);
+        s->sb[i].scratch = nullptr;
+    }
+    s->cap = 0;
+}
+
+int alloc_candidates(cs_sketch* s, uint32_t cap) {
+    free_candidates(s);
+    for (int i = 0; i < s->n_scales; ++i) {
+        for (int h = 0; h < 2; ++h) {
+            CS_CUDA(cudaMalloc(&s->sb[i].id[h], (size_t)cap * sizeof(uint64_t)));
+            CS_CUDA(cudaMalloc(&s->sb[i].ek[h], (size_t)cap * sizeof(uint32_t)));
+        }
+        CS_CUDA(cudaMalloc(&s->sb[i].scratch, (size_t)select_scratch_words(cap) * sizeof(uint32_t)));
+        s->cur[i] = 0;
+    }
+    s->cap = cap;
+    return CS_OK;
+}
+
+/* Double the candidate capacity, keeping the entries held (all scales). */
+int grow_candidates(cs_sketch* s) {
+    if (s->cap >= (1u << 30)) return fail(CS_ERR_NOMEM, "candidate list would exceed 2^30 entries per scale");
+    const uint32_t cap = s->cap * 2;
+    CS_CUDA(cudaStreamSynchronize(s->stream));
+    for (int i = 0; i < s->n_scales; ++i) {
+        SelectBuffers nb = {};
+        for (int h = 0; h < 2; ++h) {
+            CS_CUDA(cudaMalloc(&nb.id[h], (size_t)cap * sizeof(uint64_t)));
+            CS_CUDA(cudaMalloc(&nb.ek[h], (size_t)cap * sizeof(uint32_t)));
+        }
+        CS_CUDA(cudaMalloc(&nb.scratch, (size_t)select_scratch_words(cap) * sizeof(uint32_t)));
+        const uint32_t held = s->st_host[i].count < s->cap ? s->st_host[i].count : s->cap;
+        const int c = s->cur[i];
+        CS_CUDA(cudaMemcpyAsync(nb.id[0], s->sb[i].id[c], (size_t)held * 8, cudaMemcpyDeviceToDevice, s->stream));
+        CS_CUDA(cudaMemcpyAsync(nb.ek[0], s->sb[i].ek[c], (size_t)held * 4, cudaMemcpyDeviceToDevice, s->stream));
+        CS_CUDA(cudaStreamSynchronize(s->stream));
+        for (int h = 0; h < 2; ++h) { cudaFree(s->sb[i].id[h]); cudaFree(s->sb[i].ek[h]); }
+        cudaFree(s->sb[i].scratch);
+        s->sb[i] = nb;
+        s->cur[i] = 0;
+    }
+    s->cap = cap;
+    return CS_OK;
+}
+
+int read_states(cs_sketch* s) {
+    CS_CUDA(cudaMemcpyAsync(s->st_host, s->st_dev, sizeof(ScanState) * s->n_scales, cudaMemcpyDeviceToHost, s->stream));
+    CS_CUDA(cudaStreamSynchronize(s->stream));
+    return CS_OK;
+}
+
+/* Sort + dedupe + cut the candidate list of one scale (device side only; caller reads the states back). */
+int compact_scale(cs_sketch* s, int i) {
+    const ScanState& h = s->st_host[i];
+    const uint32_t n = h.count < s->cap ? h.count : s->cap;
+    cudaError_t e;
+    s->cur[i] = select_compact(s->sb[i], s->cur[i], n, s->id_bits[i], h.est_min, h.est_max, s->st_dev + i, s->k_max,
+                               s->thr_min, s->stream, &s->launches, &e);
+    if (e != cudaSuccess) return fail(CS_ERR_CUDA, "select_compact: %s", cudaGetErrorString(e));
+    s->dirty[i] = false;
+    s->n_compactions[i] += 1;
+    return CS_OK;
+}
+
+void fill_scan_params(cs_sketch* s, ScanParams* S) {
+    memset(S, 0, sizeof(*S));
+    for (int i = 0; i < s->n_scales; ++i) {
+        S->tg[i].id = s->sb[i].id[s->cur[i]];
+        S->tg[i].ek = s->sb[i].ek[s->cur[i]];
+        S->tg[i].st = s->st_dev + i;
+        S->tg[i].cap = s->cap;
+    }
+}
+
+PassParams pass_params(const cs_sketch* s, uint64_t index0, double sample_p) {
+    PassParams P = s->P;
+    P.index0 = index0;
+    P.sample = sample_p < 1.0 ? 1 : 0;
+    P.Tp = sample_threshold(sample_p);
+    return P;
+}
+
+bool bad_p(double p) { return !(p > 0.0) || p > 1.0; }
+
+}  // namespace
+
+namespace {
+
+/* After a chunk: which scales must be compacted now (list past half the buffer, or doubled since last time). */
+bool wants_compaction(const cs_sketch* s, int i) {
+    const uint32_t c = s->st_host[i].count;
+    uint64_t base = s->last_compact[i];
+    if (base < s->k_max) base = s->k_max;
+    if (base < 65536) base = 65536;
+    return s->dirty[i] && (c > s->cap / 2 || c >= 2 * base);
+}
+
+/* Replay n device-resident particles against the tables, collecting candidates.
+ * Invariant that makes overflow impossible on a retry: a chunk of at most `free` particles cannot append more
+ * than `free` entries to any scale. */
+int scan_device(cs_sketch* s, const float* xyz, uint64_t n, double sample_p) {
+    uint64_t done = 0;
+    while (done < n) {
+        uint32_t free_min = s->cap;
+        for (int i = 0; i < s->n_scales; ++i) {
+            uint32_t held = s->st_host[i].count;
+            uint32_t fr = held < s->cap ? s->cap - held : 0;
+            if (fr < free_min) free_min = fr;
+        }
+        if (free_min < s->cap / 2) {                     /* lists are legitimately large: make room */
+            bool any = false;
+            for (int i = 0; i < s->n_scales; ++i)
+                if (s->dirty[i] && s->st_host[i].count > s->cap / 2) {
+                    int rc = compact_scale(s, i);
+                    if (rc) return rc;
+                    any = true;
+                }
+            if (any) {
+                int rc = read_states(s);
+                if (rc) return rc;
+                for (int i = 0; i < s->n_scales; ++i) s->last_compact[i] = s->st_host[i].count;
+                continue;
+            }
+            int rc = grow_candidates(s);
+            if (rc) return rc;
+            continue;
+        }
+        /* optimistic chunk: expect at most rate * chunk new entries per scale, keep a factor 2 of slack */
+        double want = (double)free_min / (2.0 * (s->rate > 1e-9 ? s->rate : 1e-9));
+        uint64_t chunk = want >= (double)MAX_CHUNK ? MAX_CHUNK : (uint64_t)want;
+        if (s->first_chunk && s->k_max) {                /* a small first chunk fixes a first tau cheaply */
+            uint64_t c0 = 8 * s->k_max > (1u << 18) ? 8 * s->k_max : (1u << 18);
+            if (chunk > c0) chunk = c0;
+        }
+        if (chunk > n - done) chunk = n - done;
+        if (chunk < n - done) chunk &= ~(uint64_t)3;     /* keep the 16-byte phase of the remaining stream */
+        if (chunk == 0) chunk = (n - done) < 4 ? (n - done) : 4;
+
+        for (;;) {
+            uint32_t before[CS_MAX_SCALES];
+            for (int i = 0; i < s->n_scales; ++i) before[i] = s->st_host[i].count;
+            ScanParams S;
+            fill_scan_params(s, &S);
+            PassParams P = pass_params(s, s->scan_index + done, sample_p);
+            cudaError_t e = launch_scan(P, S, xyz + 3 * done, chunk, s->sm_count, s->stream);
+            if (e != cudaSuccess) return fail(CS_ERR_CUDA, "scan kernel: %s", cudaGetErrorString(e));
+            s->launches += 1;
+            s->n_scan_launches += 1;
+            int rc = read_states(s);
+            if (rc) return rc;
+            bool overflow = false;
+            double r = 0.0;
+            for (int i = 0; i < s->n_scales; ++i) {
+                if (s->st_host[i].count != before[i]) s->dirty[i] = true;
+                if (s->st_host[i].count > s->cap) overflow = true;
+                double ri = (double)(s->st_host[i].count - before[i]) / (double)chunk;
+                if (ri > r) r = ri;
+            }
+            s->rate = r;
+            if (!overflow) break;
+            /* Entries past the capacity were dropped: dedupe / cut every list, then re-run this chunk with a
+             * size that cannot overflow.  What the failed run appended is valid and is deduplicated later. */
+            for (int i = 0; i < s->n_scales; ++i) {
+                rc = compact_scale(s, i);
+                if (rc) return rc;
+            }
+            rc = read_states(s);
+            if (rc) return rc;
+            free_min = s->cap;
+            for (int i = 0; i < s->n_scales; ++i) {
+                s->last_compact[i] = s->st_host[i].count;
+                uint32_t fr = s->cap - s->st_host[i].count;
+                if (fr < free_min) free_min = fr;
+            }
+            while (free_min < s->cap / 2) {
+                rc = grow_candidates(s);
+                if (rc) return rc;
+                free_min = s->cap;
+                for (int i = 0; i < s->n_scales; ++i) {
+                    uint32_t fr = s->cap - s->st_host[i].count;
+                    if (fr < free_min) free_min = fr;
+                }
+            }
+            if (chunk > free_min) chunk = free_min & ~3u;
+        }
+        done += chunk;
+        s->first_chunk = false;
+        bool any = false;
+        for (int i = 0; i < s->n_scales; ++i)
+            if (wants_compaction(s, i)) {
+                int rc = compact_scale(s, i);
+                if (rc) return rc;
+                any = true;
+            }
+        if (any) {
+            int rc = read_states(s);
+            if (rc) return rc;
+            for (int i = 0; i < s->n_scales; ++i)
+                if (!s->dirty[i]) s->last_compact[i] = s->st_host[i].count;
+        }
+    }
+    s->scan_index += n;
+    return CS_OK;
+}
+
+/* Bring the list of one scale into its final form (sorted, unique, cut) if anything was appended. */
+int finalize_scale(cs_sketch* s, int i) {
+    if (!s->dirty[i]) return CS_OK;
+    int rc = compact_scale(s, i);
+    if (rc) return rc;
+    rc = read_states(s);
+    if (rc) return rc;
+    s->last_compact[i] = s->st_host[i].count;
+    return CS_OK;
+}
+
+int ensure_out(cs_sketch* s, uint64_t n) {
+    if (n <= s->out_cap) return CS_OK;
+    if (s->out_ids) cudaFree(s->out_ids);
+    if (s->out_est) cudaFree(s->out_est);
+    s->out_ids = nullptr; s->out_est = nullptr; s->out_cap = 0;
+    CS_CUDA(cudaMalloc(&s->out_ids, n * sizeof(uint64_t)));
+    CS_CUDA(cudaMalloc(&s->out_est, n * sizeof(int32_t)));
+    s->out_cap = n;
+    return CS_OK;
+}
+
+/* First n entries of the final list of scale i -> caller's buffers (device or host). */
+int emit_prefix(cs_sketch* s, int i, uint32_t n, uint64_t* ids_out, int32_t* est_out) {
+    if (!n) return CS_OK;
+    int rc = ensure_out(s, n);
+    if (rc) return rc;
+    cudaError_t e = launch_emit_prefix(s->sb[i].id[s->cur[i]], s->sb[i].ek[s->cur[i]], n, s->out_ids, s->out_est, s->stream);
+    if (e != cudaSuccess) return fail(CS_ERR_CUDA, "emit kernel: %s", cudaGetErrorString(e));
+    s->launches += 1;
+    CS_CUDA(cudaMemcpyAsync(ids_out, s->out_ids, (size_t)n * 8, cudaMemcpyDefault, s->stream));
+    CS_CUDA(cudaMemcpyAsync(est_out, s->out_est, (size_t)n * 4, cudaMemcpyDefault, s->stream));
+    CS_CUDA(cudaStreamSynchronize(s->stream));
+    return CS_OK;
+}
+
+int ensure_staging(cs_sketch* s) {
+    if (s->stage[0]) return CS_OK;
+    CS_CUDA(cudaStreamCreateWithFlags(&s->copy_stream, cudaStreamNonBlocking));
+    for (int k = 0; k < STAGE_SLOTS; ++k) {
+        CS_CUDA(cudaMalloc(&s->stage[k], STAGE_PARTICLES * 12));
+        CS_CUDA(cudaEventCreateWithFlags(&s->ev_full[k], cudaEventDisableTiming));
+        CS_CUDA(cudaEventCreateWithFlags(&s->ev_free[k], cudaEventDisableTiming));
+    }
+    return CS_OK;
+}
+
+/* Issue the host->device copy of batch b into its ring slot (waits for the kernel that last used the slot). */
+int stage_batch(cs_sketch* s, const float* xyz_host, uint64_t n, uint64_t b) {
+    const int slot = (int)(b % STAGE_SLOTS);
+    const uint64_t off = b * STAGE_PARTICLES;
+    const uint64_t m = n - off < STAGE_PARTICLES ? n - off : STAGE_PARTICLES;
+    CS_CUDA(cudaStreamWaitEvent(s->copy_stream, s->ev_free[slot], 0));
+    CS_CUDA(cudaMemcpyAsync(s->stage[slot], xyz_host + 3 * off, m * 12, cudaMemcpyHostToDevice, s->copy_stream));
+    CS_CUDA(cudaEventRecord(s->ev_full[slot], s->copy_stream));
+    return CS_OK;
+}
+
+int check_xyz(const cs_sketch* s, const float* xyz, uint64_t n, double sample_p) {
+    if (!s) return fail(CS_ERR_ARG, "null handle");
+    if (bad_p(sample_p)) return fail(CS_ERR_ARG, "sample_p must be in (0, 1]");
+    if (n && !xyz) return fail(CS_ERR_ARG, "null positions with n > 0");
+    if (reinterpret_cast<uintptr_t>(xyz) & 3u) return fail(CS_ERR_ARG, "positions must be 4-byte aligned");
+    return CS_OK;
+}
+
+}  // namespace
+
+/* =========================================================================================================
+ * C ABI
+ * ========================================================================================================= */
+
+extern "C" {
+
+const char* cs_version(void) { return "cs-b200 0.1 (sm_100a)"; }
+
+const char* cs_last_error(void) { return g_err; }
+
+int cs_derive_coeffs(uint64_t seed, int d, uint64_t* out_4d, uint64_t* K_out) {
+    if (d < 1 || d > CS_MAX_ROWS || !out_4d) return fail(CS_ERR_ARG, "cs_derive_coeffs: bad d or null output");
+    derive_coeffs(seed, d, out_4d, K_out);
+    return CS_OK;
+}
+
+uint64_t cs_sample_threshold(double sample_p) { return sample_threshold(sample_p); }
+
+int cs_create_multi(cs_sketch** out, int n_scales, int d, uint64_t w, const uint32_t* G, double L, uint64_t seed) {
+    if (!out) return fail(CS_ERR_ARG, "null output handle");
+    *out = nullptr;
+    if (!G) return fail(CS_ERR_ARG, "null grid list");
+    if (n_scales < 1 || n_scales > CS_MAX_SCALES) return fail(CS_ERR_ARG, "n_scales must be in [1, %d]", CS_MAX_SCALES);
+    if (d < 1 || d > CS_MAX_ROWS) return fail(CS_ERR_ARG, "d must be in [1, %d]", CS_MAX_ROWS);
+    if (n_scales * d > CS_MAX_HASH_ROWS) return fail(CS_ERR_ARG, "n_scales * d must be <= %d", CS_MAX_HASH_ROWS);
+    if (w < 1 || w > (1ull << 31)) return fail(CS_ERR_ARG, "w must be in [1, 2^31]");
+    if (!(L > 0.0) || !std::isfinite(L)) return fail(CS_ERR_ARG, "L must be finite and > 0");
+    for (int i = 0; i < n_scales; ++i)
+        if (G[i] < 1 || G[i] > (1u << 20)) return fail(CS_ERR_ARG, "G must be in [1, 2^20]");
+
+    int dev = 0;
+    CS_CUDA(cudaGetDevice(&dev));
+    cs_sketch* s = new (std::nothrow) cs_sketch();
+    if (!s) return fail(CS_ERR_NOMEM, "host allocation failed");
+    s->d = d; s->n_scales = n_scales; s->w = w; s->L = L; s->seed = seed; s->device = dev;
+    int sm = 0;
+    if (cudaDeviceGetAttribute(&sm, cudaDevAttrMultiProcessorCount, dev) == cudaSuccess && sm > 0) s->sm_count = sm;
+
+    PassParams& P = s->P;
+    P.w = w; P.d = d; P.n_scales = n_scales;
+    for (int i = 0; i < n_scales; ++i) {
+        uint64_t Ki = 0;
+        derive_coeffs(seed + (uint64_t)i, d, s->coef[i], &Ki);
+        if (i == 0) s->K = Ki;                                        /* one sampling key: scale 0's */
+        for (int j = 0; j < d; ++j) {
+            const uint64_t* c = &s->coef[i][4 * j];
+            P.rows[i * d + j].h = split_coef(c[0], c[1]);
+            P.rows[i * d + j].s = split_coef(c[2], c[3]);
+        }
+        s->G[i] = G[i];
+        const uint64_t cells = (uint64_t)G[i] * G[i] * G[i];
+        s->id_bits[i] = bit_length(cells - 1);
+        P.sc[i].G = G[i];
+        P.sc[i].qscale = (float)((double)G[i] / L);
+        P.sc[i].top = (float)(G[i] - 1);
+        P.sc[i].big = cells > (1ull << 32) ? 1u : 0u;
+    }
+    P.K = s->K;
+
+    auto bail = [&](int rc) { cs_destroy(s); return rc; };
+    for (int i = 0; i < n_scales; ++i) {
+        cudaError_t e = cudaMalloc(&s->T[i], (size_t)d * w * sizeof(int32_t));
+        if (e != cudaSuccess) return bail(fail(e == cudaErrorMemoryAllocation ? CS_ERR_NOMEM : CS_ERR_CUDA,
+                                               "cudaMalloc(table): %s", cudaGetErrorString(e)));
+        e = cudaMemset(s->T[i], 0, (size_t)d * w * sizeof(int32_t));
+        if (e != cudaSuccess) return bail(fail(CS_ERR_CUDA, "cudaMemset(table): %s", cudaGetErrorString(e)));
+        P.sc[i].T = s->T[i];
+    }
+    cudaError_t e = cudaMalloc(&s->st_dev, sizeof(ScanState) * CS_MAX_SCALES);
+    if (e == cudaSuccess) e = cudaMallocHost(&s->st_host, sizeof(ScanState) * CS_MAX_SCALES);
+    if (e == cudaSuccess) e = cudaMalloc(&s->word_dev, 64);
+    if (e == cudaSuccess) e = cudaMallocHost(&s->word_host, 64);
+    if (e != cudaSuccess) return bail(fail(CS_ERR_CUDA, "state allocation: %s", cudaGetErrorString(e)));
+    memset(s->st_host, 0, sizeof(ScanState) * CS_MAX_SCALES);
+    *out = s;
+    return CS_OK;
+}
+
+int cs_create(cs_sketch** out, int d, uint64_t w, uint32_t G, double L, uint64_t seed) {
+    return cs_create_multi(out, 1, d, w, &G, L, seed);
+}
+
+int cs_destroy(cs_sketch* s) {
+    if (!s) return CS_OK;
+    if (s->stream || s->T[0]) cudaStreamSynchronize(s->stream);
+    if (s->copy_stream) cudaStreamSynchronize(s->copy_stream);
+    free_candidates(s);
+    for (int i = 0; i < CS_MAX_SCALES; ++i) if (s->T[i]) cudaFree(s->T[i]);
+    if (s->st_dev) cudaFree(s->st_dev);
+    if (s->st_host) cudaFreeHost(s->st_host);
+    if (s->word_dev) cudaFree(s->word_dev);
+    if (s->word_host) cudaFreeHost(s->word_host);
+    if (s->out_ids) cudaFree(s->out_ids);
+    if (s->out_est) cudaFree(s->out_est);
+    for (int k = 0; k < STAGE_SLOTS; ++k) {
+        if (s->stage[k]) cudaFree(s->stage[k]);
+        if (s->ev_full[k]) cudaEventDestroy(s->ev_full[k]);
+        if (s->ev_free[k]) cudaEventDestroy(s->ev_free[k]);
+    }
+    if (s->copy_stream) cudaStreamDestroy(s->copy_stream);
+    delete s;
+    return CS_OK;
+}
+
+int cs_reset(cs_sketch* s) {
+    if (!s) return fail(CS_ERR_ARG, "null handle");
+    for (int i = 0; i < s->n_scales; ++i)
+        CS_CUDA(cudaMemsetAsync(s->T[i], 0, (size_t)s->d * s->w * sizeof(int32_t), s->stream));
+    s->upd_index = 0; s->scan_index = 0; s->scanning = false;
+    for (int i = 0; i < CS_MAX_SCALES; ++i) { s->dirty[i] = false; s->last_compact[i] = 0; }
+    memset(s->st_host, 0, sizeof(ScanState) * CS_MAX_SCALES);
+    return CS_OK;
+}
+
+int cs_set_stream(cs_sketch* s, void* cuda_stream) {
+    if (!s) return fail(CS_ERR_ARG, "null handle");
+    CS_CUDA(cudaStreamSynchronize(s->stream));           /* work already queued finishes on the old stream */
+    s->stream = (cudaStream_t)cuda_stream;
+    return CS_OK;
+}
+
+int cs_set_update_index(cs_sketch* s, uint64_t index) {
+    if (!s) return fail(CS_ERR_ARG, "null handle");
+    s->upd_index = index;
+    return CS_OK;
+}
+
+int cs_set_scan_index(cs_sketch* s, uint64_t index) {
+    if (!s) return fail(CS_ERR_ARG, "null handle");
+    s->scan_index = index;
+    return CS_OK;
+}
+
+int cs_get_update_index(cs_sketch* s, uint64_t* index_out) {
+    if (!s || !index_out) return fail(CS_ERR_ARG, "null argument");
+    *index_out = s->upd_index;
+    return CS_OK;
+}
+
+int cs_update(cs_sketch* s, const float* xyz_dev, uint64_t n, double sample_p) {
+    int rc = check_xyz(s, xyz_dev, n, sample_p);
+    if (rc) return rc;
+    if (!n) return CS_OK;
+    PassParams P = pass_params(s, s->upd_index, sample_p);
+    cudaError_t e = launch_update(P, xyz_dev, n, s->sm_count, s->stream);
+    if (e != cudaSuccess) return fail(CS_ERR_CUDA, "update kernel: %s", cudaGetErrorString(e));
+    s->launches += 1;
+    s->upd_index += n;
+    return CS_OK;
+}
+
+int cs_update_host(cs_sketch* s, const float* xyz_host, uint64_t n, double sample_p) {
+    int rc = check_xyz(s, xyz_host, n, sample_p);
+    if (rc) return rc;
+    if (!n) return CS_OK;
+    rc = ensure_staging(s);
+    if (rc) return rc;
+    const uint64_t batches = (n + STAGE_PARTICLES - 1) / STAGE_PARTICLES;
+    for (uint64_t b = 0; b < batches; ++b) {
+        rc = stage_batch(s, xyz_host, n, b);
+        if (rc) return rc;
+        const int slot = (int)(b % STAGE_SLOTS);
+        const uint64_t off = b * STAGE_PARTICLES;
+        const uint64_t m = n - off < STAGE_PARTICLES ? n - off : STAGE_PARTICLES;
+        CS_CUDA(cudaStreamWaitEvent(s->stream, s->ev_full[slot], 0));
+        PassParams P = pass_params(s, s->upd_index + off, sample_p);
+        cudaError_t e = launch_update(P, s->stage[slot], m, s->sm_count, s->stream);
+        if (e != cudaSuccess) return fail(CS_ERR_CUDA, "update kernel: %s", cudaGetErrorString(e));
+        s->launches += 1;
+        CS_CUDA(cudaEventRecord(s->ev_free[slot], s->stream));
+    }
+    CS_CUDA(cudaStreamSynchronize(s->copy_stream));      /* the host buffer may be reused on return */
+    s->upd_index += n;
+    return CS_OK;
+}
+
+int cs_estimate(cs_sketch* s, int scale, const uint64_t* cells_dev, uint64_t m, int32_t* est_dev) {
+    if (!s) return fail(CS_ERR_ARG, "null handle");
+    if (scale < 0 || scale >= s->n_scales) return fail(CS_ERR_ARG, "scale out of range");
+    if (m && (!cells_dev || !est_dev)) return fail(CS_ERR_ARG, "null buffer with m > 0");
+    if (!m) return CS_OK;
+    PassParams P = pass_params(s, 0, 1.0);
+    cudaError_t e = launch_estimate(P, scale, cells_dev, m, est_dev, s->stream);
+    if (e != cudaSuccess) return fail(CS_ERR_CUDA, "estimate kernel: %s", cudaGetErrorString(e));
+    s->launches += 1;
+    return CS_OK;
+}
+
+int cs_scan_begin(cs_sketch* s, uint64_t k_max, int32_t thr_min) {
+    if (!s) return fail(CS_ERR_ARG, "null handle");
+    if (k_max > (1ull << 28)) return fail(CS_ERR_ARG, "k_max must be <= 2^28");
+    uint64_t want = 16 * k_max;
+    if (want < MIN_CAP) want = MIN_CAP;
+    uint32_t cap = MIN_CAP;
+    while (cap < want) cap *= 2;
+    if (s->cap < cap) {
+        int rc = alloc_candidates(s, cap);
+        if (rc) return rc;
+    }
+    s->k_max = k_max; s->thr_min = thr_min;
+    s->scan_index = 0; s->rate = 1.0; s->first_chunk = true; s->n_scan_launches = 0;
+    for (int i = 0; i < s->n_scales; ++i) {
+        s->st_host[i].count = 0;
+        s->st_host[i].tau = k_max ? INT32_MIN : thr_min;
+        s->st_host[i].est_min = INT32_MAX;
+        s->st_host[i].est_max = INT32_MIN;
+        s->st_host[i].uniq = 0;
+        s->dirty[i] = false; s->last_compact[i] = 0; s->n_compactions[i] = 0;
+    }
+    CS_CUDA(cudaMemcpyAsync(s->st_dev, s->st_host, sizeof(ScanState) * s->n_scales, cudaMemcpyHostToDevice, s->stream));
+    CS_CUDA(cudaStreamSynchronize(s->stream));
+    s->scanning = true;
+    return CS_OK;
+}
+
+int cs_scan(cs_sketch* s, const float* xyz_dev, uint64_t n, double sample_p) {
+    int rc = check_xyz(s, xyz_dev, n, sample_p);
+    if (rc) return rc;
+    if (!s->scanning) return fail(CS_ERR_STATE, "cs_scan before cs_scan_begin");
+    if (!n) return CS_OK;
+    return scan_device(s, xyz_dev, n, sample_p);
+}
+
+int cs_scan_host(cs_sketch* s, const float* xyz_host, uint64_t n, double sample_p) {
+    int rc = check_xyz(s, xyz_host, n, sample_p);
+    if (rc) return rc;
+    if (!s->scanning) return fail(CS_ERR_STATE, "cs_scan_host before cs_scan_begin");
+    if (!n) return CS_OK;
+    rc = ensure_staging(s);
+    if (rc) return rc;
+    const uint64_t batches = (n + STAGE_PARTICLES - 1) / STAGE_PARTICLES;
+    rc = stage_batch(s, xyz_host, n, 0);
+    if (rc) return rc;
+    for (uint64_t b = 0; b < batches; ++b) {
+        if (b + 1 < batches) {                           /* next copy runs while this batch is scanned */
+            rc = stage_batch(s, xyz_host, n, b + 1);
+            if (rc) return rc;
+        }
+        const int slot = (int)(b % STAGE_SLOTS);
+        const uint64_t off = b * STAGE_PARTICLES;
+        const uint64_t m = n - off < STAGE_PARTICLES ? n - off : STAGE_PARTICLES;
+        CS_CUDA(cudaStreamWaitEvent(s->stream, s->ev_full[slot], 0));
+        rc = scan_device(s, s->stage[slot], m, sample_p);
+        if (rc) return rc;
+        CS_CUDA(cudaEventRecord(s->ev_free[slot], s->stream));
+    }
+    CS_CUDA(cudaStreamSynchronize(s->copy_stream));
+    return CS_OK;
+}
+
+int cs_scan_cells(cs_sketch* s, int scale, const uint64_t* cells_dev, uint64_t m) {
+    if (!s) return fail(CS_ERR_ARG, "null handle");
+    if (scale < 0 || scale >= s->n_scales) return fail(CS_ERR_ARG, "scale out of range");
+    if (m && !cells_dev) return fail(CS_ERR_ARG, "null cells with m > 0");
+    if (!s->scanning) return fail(CS_ERR_STATE, "cs_scan_cells before cs_scan_begin");
+    uint64_t done = 0;
+    while (done < m) {
+        uint32_t held = s->st_host[scale].count;
+        uint32_t fr = held < s->cap ? s->cap - held : 0;
+        if (fr < s->cap / 2) {
+            if (s->dirty[scale]) {
+                int rc = finalize_scale(s, scale);
+                if (rc) return rc;
+                continue;
+            }
+            int rc = grow_candidates(s);
+            if (rc) return rc;
+            continue;
+        }
+        uint64_t chunk = m - done < fr ? m - done : fr;      /* cannot overflow: one entry per cell at most */
+        ScanParams S;
+        fill_scan_params(s, &S);
+        PassParams P = pass_params(s, 0, 1.0);
+        cudaError_t e = launch_scan_cells(P, S, scale, cells_dev + done, chunk, s->stream);
+        if (e != cudaSuccess) return fail(CS_ERR_CUDA, "scan_cells kernel: %s", cudaGetErrorString(e));
+        s->launches += 1;
+        int rc = read_states(s);
+        if (rc) return rc;
+        if (s->st_host[scale].count != held) s->dirty[scale] = true;
+        done += chunk;
+    }
+    return CS_OK;
+}
+
+int cs_topk(cs_sketch* s, int scale, uint64_t k, uint64_t* ids_out, int32_t* est_out, uint64_t* n_out) {
+    if (!s || !n_out) return fail(CS_ERR_ARG, "null argument");
+    if (scale < 0 || scale >= s->n_scales) return fail(CS_ERR_ARG, "scale out of range");
+    if (k && (!ids_out || !est_out)) return fail(CS_ERR_ARG, "null output with k > 0");
+    if (!s->scanning) return fail(CS_ERR_STATE, "cs_topk before cs_scan_begin");
+    if (k > s->k_max) return fail(CS_ERR_ARG, "k exceeds the k_max given to cs_scan_begin");
+    int rc = finalize_scale(s, scale);
+    if (rc) return rc;
+    const uint32_t held = s->st_host[scale].count;
+    const uint32_t n = k < held ? (uint32_t)k : held;
+    rc = emit_prefix(s, scale, n, ids_out, est_out);
+    if (rc) return rc;
+    *n_out = n;
+    return CS_OK;
+}
+
+int cs_excursion(cs_sketch* s, int scale, int32_t thr, uint64_t cap, uint64_t* ids_out, int32_t* est_out,
+                 uint64_t* n_total) {
+    if (!s || !n_total) return fail(CS_ERR_ARG, "null argument");
+    if (scale < 0 || scale >= s->n_scales) return fail(CS_ERR_ARG, "scale out of range");
+    if (cap && (!ids_out || !est_out)) return fail(CS_ERR_ARG, "null output with cap > 0");
+    if (!s->scanning) return fail(CS_ERR_STATE, "cs_excursion before cs_scan_begin");
+    if (thr < s->thr_min) return fail(CS_ERR_ARG, "thr is below the thr_min given to cs_scan_begin");
+    int rc = finalize_scale(s, scale);
+    if (rc) return rc;
+    const uint32_t held = s->st_host[scale].count;
+    cudaError_t e = launch_count_ge(s->sb[scale].ek[s->cur[scale]], held, thr, s->word_dev, s->stream);
+    if (e != cudaSuccess) return fail(CS_ERR_CUDA, "count kernel: %s", cudaGetErrorString(e));
+    s->launches += 1;
+    CS_CUDA(cudaMemcpyAsync(s->word_host, s->word_dev, 4, cudaMemcpyDeviceToHost, s->stream));
+    CS_CUDA(cudaStreamSynchronize(s->stream));
+    const uint32_t total = *s->word_host;
+    const uint32_t n = cap < total ? (uint32_t)cap : total;
+    rc = emit_prefix(s, scale, n, ids_out, est_out);
+    if (rc) return rc;
+    *n_total = total;
+    return CS_OK;
+}
+
+int cs_scan_stats(cs_sketch* s, int scale, uint64_t* out4_host) {
+    if (!s || !out4_host) return fail(CS_ERR_ARG, "null argument");
+    if (scale < 0 || scale >= s->n_scales) return fail(CS_ERR_ARG, "scale out of range");
+    if (!s->scanning) return fail(CS_ERR_STATE, "cs_scan_stats before cs_scan_begin");
+    int rc = read_states(s);
+    if (rc) return rc;
+    out4_host[0] = s->st_host[scale].count;
+    out4_host[1] = (uint64_t)(int64_t)s->st_host[scale].tau;
+    out4_host[2] = s->n_compactions[scale];
+    out4_host[3] = s->n_scan_launches;
+    return CS_OK;
+}
+
+int cs_sketch_read(cs_sketch* s, int scale, int32_t* out_d_by_w) {
+    if (!s || !out_d_by_w) return fail(CS_ERR_ARG, "null argument");
+    if (scale < 0 || scale >= s->n_scales) return fail(CS_ERR_ARG, "scale out of range");
+    CS_CUDA(cudaMemcpyAsync(out_d_by_w, s->T[scale], (size_t)s->d * s->w * sizeof(int32_t), cudaMemcpyDefault, s->stream));
+    CS_CUDA(cudaStreamSynchronize(s->stream));
+    return CS_OK;
+}
+
+int cs_sketch_add(cs_sketch* s, int scale, const int32_t* in_d_by_w) {
+    if (!s || !in_d_by_w) return fail(CS_ERR_ARG, "null argument");
+    if (scale < 0 || scale >= s->n_scales) return fail(CS_ERR_ARG, "scale out of range");
+    const uint64_t n = (uint64_t)s->d * s->w;
+    cudaPointerAttributes at;
+    const int32_t* src = in_d_by_w;
+    int32_t* tmp = nullptr;
+    cudaError_t e = cudaPointerGetAttributes(&at, in_d_by_w);
+    if (e != cudaSuccess || at.type != cudaMemoryTypeDevice) {        /* host input: stage it on the device */
+        cudaGetLastError();
+        CS_CUDA(cudaMalloc(&tmp, n * sizeof(int32_t)));
+        e = cudaMemcpyAsync(tmp, in_d_by_w, n * sizeof(int32_t), cudaMemcpyHostToDevice, s->stream);
+        if (e != cudaSuccess) { cudaFree(tmp); return fail(CS_ERR_CUDA, "cudaMemcpyAsync: %s", cudaGetErrorString(e)); }
+        src = tmp;
+    }
+    e = launch_table_add(s->T[scale], src, n, s->stream);
+    s->launches += 1;
+    if (tmp) {
+        cudaStreamSynchronize(s->stream);
+        cudaFree(tmp);
+    }
+    if (e != cudaSuccess) return fail(CS_ERR_CUDA, "table add kernel: %s", cudaGetErrorString(e));
+    return CS_OK;
+}
+
+int cs_coeffs(cs_sketch* s, int scale, uint64_t* out_4d_host, uint64_t* K_out_host) {
+    if (!s || !out_4d_host) return fail(CS_ERR_ARG, "null argument");
+    if (scale < 0 || scale >= s->n_scales) return fail(CS_ERR_ARG, "scale out of range");
+    memcpy(out_4d_host, s->coef[scale], sizeof(uint64_t) * 4 * s->d);
+    if (K_out_host) *K_out_host = s->K;
+    return CS_OK;
+}
+
+int cs_launch_count(cs_sketch* s, uint64_t* n_out) {
+    if (!s || !n_out) return fail(CS_ERR_ARG, "null argument");
+    *n_out = s->launches;
+    return CS_OK;
+}
+
+}  /* extern "C" */

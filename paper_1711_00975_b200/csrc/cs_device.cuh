@@ -1,0 +1,140 @@
+/*
+ * cs_device.cuh -- device-side arithmetic of the Count-Sketch pass (sm_100a): quantise, sampling hash,
+ * affine hashes mod 2^61-1 built from 32x32->64 multiplies, median of d.
+ * Restates the arithmetic contract of include/cs.h; shares nothing with oracle/.
+ */
+#ifndef CS_DEVICE_CUH_
+#define CS_DEVICE_CUH_
+
+#include "cs_internal.h"
+
+namespace cs {
+
+__device__ __forceinline__ uint64_t mix64(uint64_t z) {
+    z ^= z >> 30;
+    z *= 0xBF58476D1CE4E5B9ULL;
+    z ^= z >> 27;
+    z *= 0x94D049BB133111EBULL;
+    z ^= z >> 31;
+    return z;
+}
+
+/* Sampling (R13): keep iff mix64(K + (i+1)*gamma) < floor(p * 2^64). */
+__device__ __forceinline__ bool keep_particle(uint64_t K, uint64_t index, uint64_t Tp) {
+    return mix64(K + (index + 1) * GAMMA) < Tp;
+}
+
+/* Stage 1 "compute cell ID from XYZ": one binary32 multiply (no FMA), floor, saturate. */
+__device__ __forceinline__ uint32_t quantise_axis(float x, float qscale, float top) {
+    float f = floorf(__fmul_rn(x, qscale));
+    f = fminf(fmaxf(f, 0.0f), top);          // fmaxf(NaN, 0) = 0
+    return __float2uint_rz(f);
+}
+
+__device__ __forceinline__ uint64_t cell_of(float x, float y, float z, const ScaleParams& sp) {
+    uint32_t ix = quantise_axis(x, sp.qscale, sp.top);
+    uint32_t iy = quantise_axis(y, sp.qscale, sp.top);
+    uint32_t iz = quantise_axis(z, sp.qscale, sp.top);
+    return (uint64_t)ix + (uint64_t)sp.G * ((uint64_t)iy + (uint64_t)sp.G * (uint64_t)iz);
+}
+
+__device__ __forceinline__ uint64_t mad_wide(uint32_t a, uint32_t b, uint64_t c) {
+    return (uint64_t)a * (uint64_t)b + c;     // IMAD.WIDE.U32
+}
+
+/* (a*c + b) mod (2^61-1), canonical residue, for c = c1*2^32 + c0 < 2^60.
+ *   a*c + b == a*c0 + A*c1 + b (mod p)  with A = a*2^32 mod p,
+ *   = hi*2^31 + lo,  lo = a0*c0 + A0*c1 + b < 2^64,  hi = ah*c0 + Ah*c1 < 2^63,
+ *   hi*2^31 = (hi>>30)*2^61 + (hi & (2^30-1))*2^31 == (hi>>30) + (hi & (2^30-1))*2^31   (2^61 == 1). */
+template <bool BIG>
+__device__ __forceinline__ uint64_t affine_mod_p(const HashCoef& k, uint32_t c0, uint32_t c1) {
+    uint64_t lo = mad_wide(k.a0, c0, k.b);
+    uint64_t hi = (uint64_t)k.ah * (uint64_t)c0;
+    if (BIG) {
+        lo = mad_wide(k.A0, c1, lo);
+        hi = mad_wide(k.Ah, c1, hi);
+    }
+    uint64_t r = (hi >> 30) + ((hi & 0x3FFFFFFFULL) << 31) + (lo & P61) + (lo >> 61);   // < 2^62 + 2^34
+    r = (r & P61) + (r >> 61);                                                           // <= p + 2
+    r = (r + ((r + 1) >> 61)) & P61;                                                     // r >= p -> r - p
+    return r;
+}
+
+/* General form for any 64-bit c (used when a caller-supplied cell id is >= 2^60): 128-bit product through
+ * __umul64hi, 2^64 == 8 (mod p). */
+__device__ __forceinline__ uint64_t affine_mod_p_wide(uint64_t a, uint64_t b, uint64_t c) {
+    uint64_t lo = a * c;
+    uint64_t hi = __umul64hi(a, c);           // < 2^61
+    uint64_t r = (lo & P61) + (lo >> 61) + ((hi << 3) & P61) + (hi >> 58) + b;   // < 3*2^61 + 16
+    r = (r & P61) + (r >> 61);
+    r = (r + ((r + 1) >> 61)) & P61;
+    return r;
+}
+
+__device__ __forceinline__ uint64_t coef_a(const HashCoef& k) { return ((uint64_t)k.ah << 31) | k.a0; }
+
+/* Bucket index and sign of row `rc` for cell c. */
+template <bool BIG, bool POW2>
+__device__ __forceinline__ void bucket_sign(const RowCoef& rc, uint32_t c0, uint32_t c1, uint64_t w,
+                                            uint32_t& bucket, int32_t& sign) {
+    uint64_t r = affine_mod_p<BIG>(rc.h, c0, c1);
+    bucket = POW2 ? ((uint32_t)r & (uint32_t)(w - 1)) : (uint32_t)(r % w);
+    uint64_t r2 = affine_mod_p<BIG>(rc.s, c0, c1);
+    sign = 1 - 2 * (int32_t)((uint32_t)r2 & 1u);
+}
+
+__device__ __forceinline__ int32_t mul_sign(int32_t t, int32_t sign) {
+    return sign > 0 ? t : (int32_t)(0u - (uint32_t)t);      // two's-complement wrap (R16)
+}
+
+__device__ __forceinline__ void cswap(int32_t& a, int32_t& b) {
+    int32_t lo = min(a, b), hi = max(a, b);
+    a = lo; b = hi;
+}
+
+/* floor((D-1)/2)-th smallest of v[0..D-1]: odd-even transposition network, fully unrolled for D <= 8. */
+template <int D>
+__device__ __forceinline__ int32_t median_of(int32_t (&v)[D]) {
+#pragma unroll
+    for (int r = 0; r < D; ++r) {
+#pragma unroll
+        for (int i = (r & 1); i + 1 < D; i += 2) cswap(v[i], v[i + 1]);
+    }
+    return v[(D - 1) / 2];
+}
+
+__device__ __forceinline__ int32_t median_rt(int32_t* v, int d) {
+    for (int i = 1; i < d; ++i) {
+        int32_t x = v[i];
+        int j = i - 1;
+        while (j >= 0 && v[j] > x) { v[j + 1] = v[j]; --j; }
+        v[j + 1] = x;
+    }
+    return v[(d - 1) / 2];
+}
+
+__host__ __device__ __forceinline__ uint32_t est_to_key(int32_t est) { return 0x7FFFFFFFu - (uint32_t)est; }
+__host__ __device__ __forceinline__ int32_t key_to_est(uint32_t ek) { return (int32_t)(0x7FFFFFFFu - ek); }
+
+constexpr int PASS_THREADS = 256;
+
+/* 16-byte streaming load of positions: read once, do not keep in L1, first to leave L2 (the sketch lives there). */
+__device__ __forceinline__ float4 ld_stream16(const float4* p) {
+    float4 v;
+    asm volatile("ld.global.cs.v4.f32 {%0, %1, %2, %3}, [%4];"
+                 : "=f"(v.x), "=f"(v.y), "=f"(v.z), "=f"(v.w) : "l"(p));
+    return v;
+}
+__device__ __forceinline__ float ld_stream4(const float* p) {
+    float v;
+    asm volatile("ld.global.cs.f32 %0, [%1];" : "=f"(v) : "l"(p));
+    return v;
+}
+
+/* T[j][h] += s without a return value: RED.E.ADD at L2. */
+__device__ __forceinline__ void red_add(int32_t* addr, int32_t v) {
+    asm volatile("red.global.add.s32 [%0], %1;" :: "l"(addr), "r"(v) : "memory");
+}
+
+}  // namespace cs
+#endif

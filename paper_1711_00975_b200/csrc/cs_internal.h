@@ -1,0 +1,105 @@
+/*
+ * cs_internal.h -- structures shared by the host runtime (cs_api.cu) and the kernels (cs_kernels.cu,
+ * cs_select.cu) of libcs.so.  Nothing in oracle/ includes this file.
+ */
+#ifndef CS_INTERNAL_H_
+#define CS_INTERNAL_H_
+
+#include <cuda_runtime.h>
+#include <stdint.h>
+
+#include "../../include/cs.h"
+
+namespace cs {
+
+constexpr uint64_t P61 = (1ULL << 61) - 1;            // Mersenne prime 2^61 - 1
+constexpr uint64_t GAMMA = 0x9E3779B97F4A7C15ULL;     // splitmix64 increment
+
+/* One affine hash x -> (a*x + b) mod p, pre-split on the host for 32-bit multiplies:
+ * a = ah*2^31 + a0 (a0 < 2^31, ah < 2^30) multiplies the low 32 bits of the cell id;
+ * A = (a * 2^32) mod p = Ah*2^31 + A0 multiplies the high bits (cell ids >= 2^32 only). */
+struct HashCoef {
+    uint32_t a0, ah, A0, Ah;
+    uint64_t b;
+};
+
+struct RowCoef {
+    HashCoef h;   // bucket hash
+    HashCoef s;   // sign hash
+};
+
+struct ScaleParams {
+    int32_t* T;        // d*w counters of this scale, row-major T[j*w + b]
+    float qscale;      // (float)((double)G / L)
+    float top;         // (float)(G - 1)
+    uint32_t G;
+    uint32_t big;      // 1 if G^3 > 2^32 (cell ids need the high-word multiplies)
+};
+
+/* Per-scale candidate collection state, in device memory, mirrored to pinned host memory after each chunk. */
+struct ScanState {
+    uint32_t count;    // entries appended (may exceed cap: the excess was dropped -> chunk is re-run)
+    int32_t tau;       // current collection threshold: only estimates >= tau are collected
+    int32_t est_min;   // min / max estimate among the entries held (bounds the radix passes over the estimate)
+    int32_t est_max;
+    uint32_t uniq;     // scratch: number of unique entries after the last compaction, before the cut
+    uint32_t pad[3];
+};
+
+struct ScanTarget {
+    uint64_t* id;      // candidate cell ids      (current ping-pong half)
+    uint32_t* ek;      // candidate keys: 0x7FFFFFFF - est  (ascending key = descending estimate)
+    ScanState* st;
+    uint32_t cap;
+    uint32_t pad;
+};
+
+/* Everything a pass over particles needs, passed by value as a __grid_constant__ kernel parameter
+ * (constant bank -> uniform registers; < 4 KB). */
+struct PassParams {
+    RowCoef rows[CS_MAX_HASH_ROWS];     // rows[s*d + j]
+    ScaleParams sc[CS_MAX_SCALES];
+    uint64_t w;                          // counters per row
+    uint64_t K;                          // sampling key
+    uint64_t Tp;                         // floor(sample_p * 2^64)
+    uint64_t index0;                     // running index of particle 0 of this launch
+    int32_t d;
+    int32_t n_scales;
+    int32_t sample;                      // 0: keep everything (sample_p >= 1)
+    int32_t pad;
+};
+
+struct ScanParams {
+    ScanTarget tg[CS_MAX_SCALES];
+};
+
+/* kernel launchers (cs_kernels.cu) */
+cudaError_t launch_update(const PassParams& P, const float* xyz, uint64_t n, int sm_count, cudaStream_t st);
+cudaError_t launch_scan(const PassParams& P, const ScanParams& S, const float* xyz, uint64_t n, int sm_count,
+                        cudaStream_t st);
+cudaError_t launch_scan_cells(const PassParams& P, const ScanParams& S, int scale, const uint64_t* cells,
+                              uint64_t m, cudaStream_t st);
+cudaError_t launch_estimate(const PassParams& P, int scale, const uint64_t* cells, uint64_t m, int32_t* est,
+                            cudaStream_t st);
+cudaError_t launch_table_add(int32_t* T, const int32_t* in, uint64_t n, cudaStream_t st);
+
+/* selection (cs_select.cu): sort the first n candidates of `src` by (ek ascending, id ascending), drop
+ * duplicate ids, cut to the entries that can still matter and update *st (count, tau, est_min, est_max).
+ * The result is left in `dst`.  scratch: at least select_scratch_words(n) uint32 words. */
+struct SelectBuffers {
+    uint64_t* id[2];
+    uint32_t* ek[2];
+    uint32_t* scratch;
+};
+uint64_t select_scratch_words(uint64_t n);
+/* returns the index (0/1) of the half that holds the result; *launches += kernels launched */
+int select_compact(const SelectBuffers& B, int src, uint32_t n, int id_bits, int32_t est_min, int32_t est_max,
+                   ScanState* st_dev, uint64_t k_max, int32_t thr_min, cudaStream_t stream, uint64_t* launches,
+                   cudaError_t* err);
+cudaError_t launch_emit_prefix(const uint64_t* id, const uint32_t* ek, uint32_t n, uint64_t* ids_out,
+                               int32_t* est_out, cudaStream_t st);
+/* number of leading entries (sorted by ek ascending) with estimate >= thr, written to *n_out_dev */
+cudaError_t launch_count_ge(const uint32_t* ek, uint32_t n, int32_t thr, uint32_t* n_out_dev, cudaStream_t st);
+
+}  // namespace cs
+#endif

@@ -1,0 +1,127 @@
+/*
+ * cs_kernels.cu -- the particle passes of libcs.so, hand-written for sm_100a:
+ *   k_update   quantise + (sample) + 2d hashes + d red.global.add.s32 per kept particle
+ *   k_scan     the same front end, d gathers with early exit against tau, median, append   (a5-a6)
+ *   k_estimate one thread per cell id: 2d hashes, d gathers, median network                (a5)
+ * Paper passages: Add / Estimate PAPER.md:134-139; UPDATE / Estimate thread code PAPER.md:326-373 (prior
+ * art: one block per item with t threads on a GTX 1080 -- here one thread owns whole particles, 4 at a time,
+ * loaded as three 16-byte vectors, and all hash coefficients sit in the constant bank as kernel parameters).
+ */
+#include "cs_device.cuh"
+#include "cs_launch.cuh"
+
+namespace cs {
+
+/* ------------------------------------------------------------------------------------------------------
+ * update
+ * ------------------------------------------------------------------------------------------------------ */
+
+template <int D, bool POW2, bool BIG>
+__device__ __forceinline__ void add_rows(const PassParams& P, int s, uint64_t c) {
+    const int d = D ? D : P.d;
+    const uint32_t c0 = (uint32_t)c, c1 = (uint32_t)(c >> 32);
+    int32_t* T = P.sc[s].T;
+    const RowCoef* rows = &P.rows[s * d];
+#pragma unroll
+    for (int j = 0; j < d; ++j) {
+        uint32_t b;
+        int32_t sg;
+        bucket_sign<BIG, POW2>(rows[j], c0, c1, P.w, b, sg);
+        red_add(T + (uint64_t)j * P.w + b, sg);
+    }
+}
+
+template <int D, bool POW2>
+__device__ __forceinline__ void add_particle(const PassParams& P, float x, float y, float z) {
+    for (int s = 0; s < P.n_scales; ++s) {
+        uint64_t c = cell_of(x, y, z, P.sc[s]);
+        if (P.sc[s].big) add_rows<D, POW2, true>(P, s, c);
+        else             add_rows<D, POW2, false>(P, s, c);
+    }
+}
+
+/* Particles [head, head + 4*groups) are read as groups of 4 (3 x 16 B per thread, 16-byte aligned);
+ * the <= 3 particles before and the <= 3 after are read with scalar loads by block 0. */
+template <int D, bool POW2>
+__global__ void __launch_bounds__(PASS_THREADS)
+k_update(const __grid_constant__ PassParams P, const float* __restrict__ xyz, uint64_t n, uint32_t head,
+         uint64_t groups) {
+    const uint64_t stride = (uint64_t)gridDim.x * PASS_THREADS;
+    const float4* body = reinterpret_cast<const float4*>(xyz + 3 * (uint64_t)head);
+    for (uint64_t g = (uint64_t)blockIdx.x * PASS_THREADS + threadIdx.x; g < groups; g += stride) {
+        float4 q0 = ld_stream16(body + 3 * g);
+        float4 q1 = ld_stream16(body + 3 * g + 1);
+        float4 q2 = ld_stream16(body + 3 * g + 2);
+        const uint64_t i0 = P.index0 + head + 4 * g;
+        if (!P.sample) {
+            add_particle<D, POW2>(P, q0.x, q0.y, q0.z);
+            add_particle<D, POW2>(P, q0.w, q1.x, q1.y);
+            add_particle<D, POW2>(P, q1.z, q1.w, q2.x);
+            add_particle<D, POW2>(P, q2.y, q2.z, q2.w);
+        } else {
+            if (keep_particle(P.K, i0 + 0, P.Tp)) add_particle<D, POW2>(P, q0.x, q0.y, q0.z);
+            if (keep_particle(P.K, i0 + 1, P.Tp)) add_particle<D, POW2>(P, q0.w, q1.x, q1.y);
+            if (keep_particle(P.K, i0 + 2, P.Tp)) add_particle<D, POW2>(P, q1.z, q1.w, q2.x);
+            if (keep_particle(P.K, i0 + 3, P.Tp)) add_particle<D, POW2>(P, q2.y, q2.z, q2.w);
+        }
+    }
+    if (blockIdx.x == 0) {
+        const uint64_t tail0 = (uint64_t)head + 4 * groups;
+        const uint64_t n_edge = (uint64_t)head + (n - tail0);          // <= 6
+        if (threadIdx.x < n_edge) {
+            uint64_t i = threadIdx.x < head ? threadIdx.x : tail0 + (threadIdx.x - head);
+            if (!P.sample || keep_particle(P.K, P.index0 + i, P.Tp)) {
+                const float* p = xyz + 3 * i;
+                add_particle<D, POW2>(P, ld_stream4(p), ld_stream4(p + 1), ld_stream4(p + 2));
+            }
+        }
+    }
+}
+
+template <int D, bool POW2>
+static cudaError_t launch_update_t(const PassParams& P, const float* xyz, uint64_t n, int sm_count,
+                                   cudaStream_t st) {
+    uint32_t head;
+    uint64_t groups;
+    split_aligned(xyz, n, &head, &groups);
+    int blocks = blocks_for(k_update<D, POW2>, sm_count, groups);
+    k_update<D, POW2><<<blocks, PASS_THREADS, 0, st>>>(P, xyz, n, head, groups);
+    return cudaGetLastError();
+}
+
+template <bool POW2>
+static cudaError_t launch_update_d(const PassParams& P, const float* xyz, uint64_t n, int sm, cudaStream_t st) {
+    switch (P.d) {
+        case 1: return launch_update_t<1, POW2>(P, xyz, n, sm, st);
+        case 2: return launch_update_t<2, POW2>(P, xyz, n, sm, st);
+        case 3: return launch_update_t<3, POW2>(P, xyz, n, sm, st);
+        case 4: return launch_update_t<4, POW2>(P, xyz, n, sm, st);
+        case 5: return launch_update_t<5, POW2>(P, xyz, n, sm, st);
+        case 6: return launch_update_t<6, POW2>(P, xyz, n, sm, st);
+        case 7: return launch_update_t<7, POW2>(P, xyz, n, sm, st);
+        case 8: return launch_update_t<8, POW2>(P, xyz, n, sm, st);
+        default: return launch_update_t<0, POW2>(P, xyz, n, sm, st);   // 9..32 rows: runtime loop
+    }
+}
+
+cudaError_t launch_update(const PassParams& P, const float* xyz, uint64_t n, int sm_count, cudaStream_t st) {
+    const bool pow2 = (P.w & (P.w - 1)) == 0;
+    return pow2 ? launch_update_d<true>(P, xyz, n, sm_count, st) : launch_update_d<false>(P, xyz, n, sm_count, st);
+}
+
+/* T += in (merge / restore by linearity), wraparound. */
+__global__ void __launch_bounds__(256) k_table_add(int32_t* __restrict__ T, const int32_t* __restrict__ in, uint64_t n) {
+    const uint64_t stride = (uint64_t)gridDim.x * blockDim.x;
+    for (uint64_t i = (uint64_t)blockIdx.x * blockDim.x + threadIdx.x; i < n; i += stride)
+        T[i] = (int32_t)((uint32_t)T[i] + (uint32_t)in[i]);
+}
+
+cudaError_t launch_table_add(int32_t* T, const int32_t* in, uint64_t n, cudaStream_t st) {
+    if (!n) return cudaSuccess;
+    uint64_t blocks = (n + 255) / 256;
+    if (blocks > 148 * 8) blocks = 148 * 8;
+    k_table_add<<<(int)blocks, 256, 0, st>>>(T, in, n);
+    return cudaGetLastError();
+}
+
+}  // namespace cs

@@ -1,0 +1,127 @@
+/*
+ * cs_probe.cu -- measurement probes behind cs_probe_l2 / cs_probe_stream: the roofline
+ * denominators of the update pass are measured on the box, not assumed.
+ *   mode 0: red.global.add.s32 of +-1 to addresses generated in registers, uniform over a table
+ *   mode 1: the same with the returning atom.global.add.s32
+ *   mode 2: 4-byte ld.global gathers at the same addresses
+ *   stream: the update kernel's 3 x 16-byte position loads with nothing behind them
+ */
+#include "cs_device.cuh"
+
+namespace cs {
+
+__device__ __forceinline__ uint64_t probe_rng(uint64_t x) { return mix64(x); }
+
+template <int MODE>
+__global__ void __launch_bounds__(256)
+k_probe_l2(int32_t* __restrict__ table, uint64_t words, uint64_t n_ops, uint64_t salt, int32_t* sink) {
+    const uint64_t stride = (uint64_t)gridDim.x * blockDim.x;
+    const uint32_t mask = (uint32_t)(words - 1);             /* words is a power of two */
+    int32_t acc = 0;
+    /* one 64-bit mix gives two addresses (the real kernel spends more ALU per atomic than this) */
+    for (uint64_t i = (uint64_t)blockIdx.x * blockDim.x + threadIdx.x; 2 * i < n_ops; i += stride) {
+        uint64_t r = probe_rng(i + salt);
+        uint32_t a0 = (uint32_t)r & mask, a1 = (uint32_t)(r >> 32) & mask;
+        int32_t v = 1 - 2 * (int32_t)((r >> 31) & 1u);
+        if (MODE == 0) {
+            red_add(table + a0, v);
+            red_add(table + a1, -v);
+        } else if (MODE == 1) {
+            acc += atomicAdd(table + a0, v);
+            acc += atomicAdd(table + a1, -v);
+        } else {
+            int32_t x, y;
+            asm volatile("ld.global.relaxed.gpu.s32 %0, [%1];" : "=r"(x) : "l"(table + a0));
+            asm volatile("ld.global.relaxed.gpu.s32 %0, [%1];" : "=r"(y) : "l"(table + a1));
+            acc += x + y;
+        }
+    }
+    if (MODE != 0 && acc == 0x7FFFFFFF) *sink = acc;         /* keep the loads / returns alive */
+}
+
+__global__ void __launch_bounds__(PASS_THREADS)
+k_probe_stream(const float* __restrict__ xyz, uint64_t groups, float* sink) {
+    const uint64_t stride = (uint64_t)gridDim.x * PASS_THREADS;
+    const float4* body = reinterpret_cast<const float4*>(xyz);
+    float acc = 0.f;
+    for (uint64_t g = (uint64_t)blockIdx.x * PASS_THREADS + threadIdx.x; g < groups; g += stride) {
+        float4 q0 = ld_stream16(body + 3 * g);
+        float4 q1 = ld_stream16(body + 3 * g + 1);
+        float4 q2 = ld_stream16(body + 3 * g + 2);
+        acc += q0.x + q0.w + q1.z + q2.y + q2.w;
+    }
+    if (acc == 1.2345e38f) *sink = acc;
+}
+
+}  // namespace cs
+
+using namespace cs;
+
+extern "C" int cs_probe_l2(int mode, uint64_t table_bytes, uint64_t n_ops, int reps, void* cuda_stream,
+                           double* ms_out) {
+    if (mode < 0 || mode > 2 || !ms_out || reps < 1 || table_bytes < 4) return CS_ERR_ARG;
+    uint64_t words = 1;
+    while (words * 2 * 4 <= table_bytes) words *= 2;         /* largest power of two that fits */
+    if (words > (1ull << 32)) return CS_ERR_ARG;
+    cudaStream_t st = (cudaStream_t)cuda_stream;
+    int32_t* table = nullptr;
+    int32_t* sink = nullptr;
+    cudaEvent_t e0 = nullptr, e1 = nullptr;
+    int rc = CS_OK;
+    int sm = 148;
+    int dev = 0;
+    cudaGetDevice(&dev);
+    cudaDeviceGetAttribute(&sm, cudaDevAttrMultiProcessorCount, dev);
+    if (cudaMalloc(&table, words * 4) != cudaSuccess || cudaMalloc(&sink, 4) != cudaSuccess) { rc = CS_ERR_NOMEM; goto out; }
+    if (cudaMemsetAsync(table, 0, words * 4, st) != cudaSuccess) { rc = CS_ERR_CUDA; goto out; }
+    cudaEventCreate(&e0);
+    cudaEventCreate(&e1);
+    for (int r = -1; r < reps; ++r) {                         /* r = -1: warm-up (brings the table into L2) */
+        if (r == 0) cudaEventRecord(e0, st);
+        const int blocks = sm * 8;
+        if (mode == 0) k_probe_l2<0><<<blocks, 256, 0, st>>>(table, words, n_ops, (uint64_t)(r + 7) << 40, sink);
+        else if (mode == 1) k_probe_l2<1><<<blocks, 256, 0, st>>>(table, words, n_ops, (uint64_t)(r + 7) << 40, sink);
+        else k_probe_l2<2><<<blocks, 256, 0, st>>>(table, words, n_ops, (uint64_t)(r + 7) << 40, sink);
+    }
+    cudaEventRecord(e1, st);
+    if (cudaEventSynchronize(e1) != cudaSuccess || cudaGetLastError() != cudaSuccess) { rc = CS_ERR_CUDA; goto out; }
+    {
+        float ms = 0.f;
+        cudaEventElapsedTime(&ms, e0, e1);
+        *ms_out = (double)ms / reps;
+    }
+out:
+    if (e0) cudaEventDestroy(e0);
+    if (e1) cudaEventDestroy(e1);
+    if (table) cudaFree(table);
+    if (sink) cudaFree(sink);
+    return rc;
+}
+
+extern "C" int cs_probe_stream(const float* xyz_dev, uint64_t n, int reps, void* cuda_stream, double* ms_out) {
+    if (!xyz_dev || !ms_out || reps < 1 || (reinterpret_cast<uintptr_t>(xyz_dev) & 15u)) return CS_ERR_ARG;
+    cudaStream_t st = (cudaStream_t)cuda_stream;
+    float* sink = nullptr;
+    if (cudaMalloc(&sink, 4) != cudaSuccess) return CS_ERR_NOMEM;
+    int sm = 148, dev = 0;
+    cudaGetDevice(&dev);
+    cudaDeviceGetAttribute(&sm, cudaDevAttrMultiProcessorCount, dev);
+    cudaEvent_t e0, e1;
+    cudaEventCreate(&e0);
+    cudaEventCreate(&e1);
+    const uint64_t groups = n / 4;
+    for (int r = -1; r < reps; ++r) {
+        if (r == 0) cudaEventRecord(e0, st);
+        k_probe_stream<<<sm * 8, PASS_THREADS, 0, st>>>(xyz_dev, groups, sink);
+    }
+    cudaEventRecord(e1, st);
+    int rc = CS_OK;
+    if (cudaEventSynchronize(e1) != cudaSuccess || cudaGetLastError() != cudaSuccess) rc = CS_ERR_CUDA;
+    float ms = 0.f;
+    cudaEventElapsedTime(&ms, e0, e1);
+    *ms_out = (double)ms / reps;
+    cudaEventDestroy(e0);
+    cudaEventDestroy(e1);
+    cudaFree(sink);
+    return rc;
+}
