@@ -114,8 +114,7 @@ int cs_update_host(cs_sketch* s, const float* xyz_host, uint64_t n, double sampl
 /* ---- queries ------------------------------------------------------------------------------------------ */
 
 /* est_dev[i] = Estimate(cells_dev[i]) against scale `scale`.  m = 0 is a no-op.
- * Cells >= G^3 are hashed like any other 64-bit id below 2^61 (ids >= 2^61 give CS_ERR_ARG is NOT checked on
- * the device: the caller passes ids < G^3). */
+ * Any 64-bit id is accepted and hashed as (a*c + b) mod p; ids of this mesh are < G^3. */
 int cs_estimate(cs_sketch* s, int scale, const uint64_t* cells_dev, uint64_t m, int32_t* est_dev);
 
 /* Candidate re-scan (estimate mode restricted to the cells that occur in the replayed stream; R10).
@@ -127,6 +126,10 @@ int cs_estimate(cs_sketch* s, int scale, const uint64_t* cells_dev, uint64_t m, 
  * still matter are collected, deduplicated and kept ordered by (estimate descending, cell id ascending).
  * The tables must not change between cs_scan_begin and the last cs_topk / cs_excursion. */
 int cs_scan_begin(cs_sketch* s, uint64_t k_max, int32_t thr_min);
+/* Initial capacity (entries per scale, a power of two in [2^10, 2^30]; default 2^22) of the candidate list the
+ * next cs_scan_begin allocates: max(entries, 16*k_max rounded up to a power of two).  The list still grows by
+ * doubling when the cells that must be kept do not fit; a small value only costs more compactions. */
+int cs_set_candidate_capacity(cs_sketch* s, uint64_t entries);
 int cs_scan(cs_sketch* s, const float* xyz_dev, uint64_t n, double sample_p);
 int cs_scan_host(cs_sketch* s, const float* xyz_host, uint64_t n, double sample_p);
 

@@ -35,6 +35,7 @@ SIGNATURES = {
     "cs_update_host": (ci, [vp, vp, u64, dbl]),
     "cs_estimate": (ci, [vp, ci, vp, u64, vp]),
     "cs_scan_begin": (ci, [vp, u64, i32]),
+    "cs_set_candidate_capacity": (ci, [vp, u64]),
     "cs_scan": (ci, [vp, vp, u64, dbl]),
     "cs_scan_host": (ci, [vp, vp, u64, dbl]),
     "cs_scan_cells": (ci, [vp, ci, vp, u64]),
@@ -171,6 +172,9 @@ class CountSketch:
 
     def scan_begin(self, k_max: int, thr_min: int = INT32_MAX):
         _chk(lib().cs_scan_begin(self._h, k_max, thr_min), "cs_scan_begin")
+
+    def set_candidate_capacity(self, entries: int):
+        _chk(lib().cs_set_candidate_capacity(self._h, entries), "cs_set_candidate_capacity")
 
     def scan(self, xyz: torch.Tensor, sample_p: float = 1.0):
         p, n = _dev_xyz(xyz)

@@ -103,6 +103,7 @@ struct cs_sketch {
     uint64_t k_max = 0;
     int32_t thr_min = INT32_MAX;
     uint32_t cap = 0;
+    uint32_t cap_min = MIN_CAP;        /* cs_set_candidate_capacity */
     SelectBuffers sb[CS_MAX_SCALES] = {};
     int cur[CS_MAX_SCALES] = {};
     bool dirty[CS_MAX_SCALES] = {};
@@ -601,10 +602,10 @@ int cs_scan_begin(cs_sketch* s, uint64_t k_max, int32_t thr_min) {
     if (!s) return fail(CS_ERR_ARG, "null handle");
     if (k_max > (1ull << 28)) return fail(CS_ERR_ARG, "k_max must be <= 2^28");
     uint64_t want = 16 * k_max;
-    if (want < MIN_CAP) want = MIN_CAP;
-    uint32_t cap = MIN_CAP;
+    if (want < s->cap_min) want = s->cap_min;
+    uint32_t cap = s->cap_min;
     while (cap < want) cap *= 2;
-    if (s->cap < cap) {
+    if (s->cap != cap) {
         int rc = alloc_candidates(s, cap);
         if (rc) return rc;
     }
@@ -621,6 +622,14 @@ int cs_scan_begin(cs_sketch* s, uint64_t k_max, int32_t thr_min) {
     CS_CUDA(cudaMemcpyAsync(s->st_dev, s->st_host, sizeof(ScanState) * s->n_scales, cudaMemcpyHostToDevice, s->stream));
     CS_CUDA(cudaStreamSynchronize(s->stream));
     s->scanning = true;
+    return CS_OK;
+}
+
+int cs_set_candidate_capacity(cs_sketch* s, uint64_t entries) {
+    if (!s) return fail(CS_ERR_ARG, "null handle");
+    if (entries < 1024 || entries > (1ull << 30) || (entries & (entries - 1)))
+        return fail(CS_ERR_ARG, "capacity must be a power of two in [2^10, 2^30]");
+    s->cap_min = (uint32_t)entries;
     return CS_OK;
 }
 

@@ -1,0 +1,292 @@
+"""GPU parity tests: the CUDA path (through the C ABI, include/cs.h) against the CPU oracle, element by element,
+on the same seeded inputs.  Bar: bit-exact -- the int32 sketch, the estimates, the top-k / excursion ids and
+values (BASELINE.json north_star).  Run on the B200 box with `-m gpu`.
+"""
+import numpy as np
+import pytest
+import torch
+
+from oracle import cs_oracle as ora
+
+pytestmark = pytest.mark.gpu
+
+INT32_MAX = 2 ** 31 - 1
+
+
+@pytest.fixture(scope="module")
+def cs():
+    if not torch.cuda.is_available():
+        pytest.skip("no CUDA device")
+    from paper_1711_00975_b200 import build, binding
+    build.build_libcs()
+    binding.lib()
+    return binding
+
+
+def _gen(name, n=None, **kw):
+    from paper_1711_00975_b200 import synth
+    wl = synth.CONFIGS[name]
+    if n is not None:
+        wl = wl.scaled(n, **kw)
+    xyz = synth.generate(wl, device="cuda")
+    return wl, xyz
+
+
+def _ids(t):
+    return t.cpu().numpy().view(np.uint64)
+
+
+def _check_all(cs, wl, xyz, sample_p=1.0, k=None, thresholds=(), probe_cells=4096, split=None, cap=None):
+    """Update + estimate + scan + top-k (+ excursion) on both sides; everything must be identical."""
+    k = wl.k if k is None else k
+    host = xyz.cpu().numpy()
+    o = ora.OracleSketch(wl.d, wl.w, wl.G, wl.L, wl.seed)
+    g = cs.CountSketch(wl.d, wl.w, list(wl.G), wl.L, wl.seed)
+    n = host.shape[0]
+    cuts = [0, n] if not split else [0] + sorted(split) + [n]
+    for a, b in zip(cuts[:-1], cuts[1:]):
+        o.update(host[a:b], sample_p)
+        g.update(xyz[a:b], sample_p)
+    thr_min = min(thresholds) if thresholds else INT32_MAX
+    if cap:
+        g.set_candidate_capacity(cap)
+    o.scan_begin()
+    g.scan_begin(k, thr_min)
+    for a, b in zip(cuts[:-1], cuts[1:]):
+        o.scan(host[a:b], sample_p)
+        g.scan(xyz[a:b], sample_p)
+    rng = np.random.default_rng(7)
+    for s in range(len(wl.G)):
+        assert np.array_equal(g.sketch(s).cpu().numpy(), o.sketch(s)), f"sketch differs at scale {s}"
+        G = wl.G[s]
+        occ = ora.quantise(host[: min(n, probe_cells)], G, wl.L)
+        cells = np.concatenate([occ, rng.integers(0, G ** 3, size=probe_cells, dtype=np.uint64)])
+        ge = g.estimate(torch.from_numpy(cells.view(np.int64)).cuda(), s).cpu().numpy()
+        assert np.array_equal(ge, o.estimate(cells, s)), f"estimates differ at scale {s}"
+        if k:
+            gi, gv = g.topk(k, s)
+            oi, ov = o.topk(k, s)
+            assert np.array_equal(_ids(gi), oi) and np.array_equal(gv.cpu().numpy(), ov), f"top-k differs at scale {s}"
+            k2 = max(1, k // 3)
+            gi, gv = g.topk(k2, s, device="cpu")
+            assert np.array_equal(_ids(gi), oi[:k2]) and np.array_equal(gv.numpy(), ov[:k2])
+        for thr in thresholds:
+            gi, gv, gt = g.excursion(thr, s)
+            oi, ov, ot = o.excursion(thr, s)
+            assert gt == ot, f"excursion size differs at scale {s}, thr {thr}"
+            assert np.array_equal(_ids(gi), oi) and np.array_equal(gv.cpu().numpy(), ov)
+    st = g.scan_stats(0)
+    g.close()
+    o.close()
+    return st
+
+
+# ---- the worked examples of tests/golden ------------------------------------------------------------------
+
+def test_mini_pipeline_golden(cs, golden):
+    """8-particle whole-pipeline example: seed 1, d 3, w 8, G 4, L 4."""
+    m = golden["mini_pipeline"]
+    cells = np.array(m["stream_cells"], dtype=np.int64)
+    pos = np.stack([(cells % 4) + 0.5, (cells // 4) % 4 + 0.5, cells // 16 + 0.5], axis=1).astype(np.float32)
+    g = cs.CountSketch(3, 8, 4, 4.0, 1)
+    g.update(torch.from_numpy(pos).cuda())
+    assert g.sketch().cpu().numpy().tolist() == m["T"]
+    q = torch.tensor([0, 18, 57, 63, 1], dtype=torch.int64, device="cuda")
+    assert g.estimate(q).cpu().tolist() == [3, 2, 2, -1, 0]
+    g.scan_begin(2, 2)
+    g.scan(torch.from_numpy(pos).cuda())
+    ids, est = g.topk(2)
+    assert list(zip(ids.cpu().tolist(), est.cpu().tolist())) == [(0, 3), (18, 2)]
+    ids, est, tot = g.excursion(2)
+    assert tot == 3 and list(zip(ids.cpu().tolist(), est.cpu().tolist())) == [(0, 3), (18, 2), (57, 2)]
+    g.close()
+
+
+def test_hash_example_golden(cs, golden):
+    """Hand-worked particle (123.456, 250.0, 499.99): one Add touches exactly the pinned buckets with the pinned signs."""
+    h = golden["hash_example"]
+    g = cs.CountSketch(5, 1 << 16, 256, 500.0, 1)
+    g.update(torch.tensor([[123.456, 250.0, 499.99]], dtype=torch.float32, device="cuda"))
+    T = g.sketch().cpu().numpy()
+    for j in range(5):
+        nz = np.nonzero(T[j])[0]
+        assert nz.tolist() == [h["h"][j]] and T[j, nz[0]] == h["s"][j]
+    assert g.estimate(torch.tensor([int(h["cell"])], dtype=torch.int64, device="cuda")).item() == 1
+    g.close()
+
+
+# ---- BASELINE.json configs ---------------------------------------------------------------------------------
+
+def test_cfg1_full(cs):
+    wl, xyz = _gen("cfg1")
+    st = _check_all(cs, wl, xyz, thresholds=(40, 64))
+    assert st["candidates"] >= wl.k
+
+
+def test_cfg2_reduced(cs):
+    wl, xyz = _gen("cfg2", 1 << 22)
+    _check_all(cs, wl, xyz, thresholds=(6,))
+
+
+def test_cfg3_reduced_big_cell_ids(cs):
+    """G = 4096: cell ids need the high-word multiplies; d = 7."""
+    wl, xyz = _gen("cfg3", (1 << 22) + 3)
+    _check_all(cs, wl, xyz, k=3000, thresholds=(5,))
+
+
+def test_cfg4_reduced_non_pow2_grid(cs):
+    wl, xyz = _gen("cfg4", 1 << 21)
+    _check_all(cs, wl, xyz, k=3000)
+
+
+def test_cfg5_reduced_multiscale_sampled(cs):
+    """4 nested grids in one pass, hash-Bernoulli sampling p = 0.1, thresholds and top-k per scale."""
+    wl, xyz = _gen("cfg5", 1 << 22)
+    _check_all(cs, wl, xyz, sample_p=wl.sample_p, k=1000, thresholds=(3, 4, 6), split=[1000001, 3000000])
+
+
+# ---- randomised small configs and edge cases ------------------------------------------------------------------
+
+@pytest.mark.parametrize("d,w,G,n,p", [
+    (1, 1, 1, 5, 1.0), (2, 7, 3, 1, 1.0), (3, 1000, 17, 4097, 1.0), (4, 4096, 64, 10007, 1.0),
+    (5, 65537, 300, 50001, 0.5), (6, 1 << 12, 2000, 30000, 1.0), (8, 12345, 1 << 20, 20003, 0.25),
+    (9, 999, 40, 7777, 1.0), (16, 1 << 10, 1700, 9999, 0.7), (32, 513, 5000, 5001, 1.0),
+])
+def test_random_small_configs(cs, d, w, G, n, p):
+    from paper_1711_00975_b200 import synth
+    wl = synth.Workload("rnd", N=n, G=(G,), d=d, w=w, k=min(50, n), H=16, f_bg=0.3, m_min=0, L=100.0, seed=d * 131 + w,
+                        gen_seed=G + n)
+    xyz = synth.generate(wl, device="cuda")
+    _check_all(cs, wl, xyz, sample_p=p, thresholds=(1,), probe_cells=512, split=[n // 3] if n > 10 else None)
+
+
+def test_edge_positions_and_alignment(cs):
+    """0, L, nextafter(L, 0), negative, NaN, +-inf; every 4-byte alignment phase of the position pointer."""
+    L, G = 500.0, 256
+    vals = np.array([0.0, -0.0, L, np.nextafter(np.float32(L), np.float32(0)), -1e-9, -5.0, np.nan, np.inf, -np.inf,
+                     123.456, 499.99, 250.0, 1e-30, 1e30], dtype=np.float32)
+    rng = np.random.default_rng(3)
+    pos = vals[rng.integers(0, len(vals), size=(1003, 3))]
+    pos = np.concatenate([pos, (rng.random((3000, 3)) * L).astype(np.float32)])
+    base = torch.from_numpy(pos).cuda()
+    for off in range(0, 5):
+        for n in (0, 1, 2, 3, 4, 5, 7, 8, 1000, 4003 - off):
+            sub_h = pos[off:off + n]
+            sub_d = base[off:off + n]          # data_ptr advances by 12*off bytes
+            o = ora.OracleSketch(5, 1 << 10, G, L, 9)
+            g = cs.CountSketch(5, 1 << 10, G, L, 9)
+            o.update(sub_h)
+            g.update(sub_d)
+            assert np.array_equal(g.sketch().cpu().numpy(), o.sketch()), (off, n)
+            o.scan_begin()
+            g.scan_begin(20)
+            o.scan(sub_h)
+            g.scan(sub_d)
+            gi, gv = g.topk(20)
+            oi, ov = o.topk(20)
+            assert np.array_equal(_ids(gi), oi) and np.array_equal(gv.cpu().numpy(), ov), (off, n)
+            g.close()
+            o.close()
+
+
+def test_wide_cell_ids_in_estimate(cs):
+    """cs_estimate takes any 64-bit id: below 2^32, below 2^60 and above (the __umul64hi form)."""
+    o = ora.OracleSketch(7, 1 << 12, 64, 10.0, 5)
+    g = cs.CountSketch(7, 1 << 12, 64, 10.0, 5)
+    pos = (np.random.default_rng(1).random((20000, 3)) * 10).astype(np.float32)
+    o.update(pos)
+    g.update(torch.from_numpy(pos).cuda())
+    cells = np.array([0, 1, 2 ** 32 - 1, 2 ** 32, 2 ** 36 + 12345, 2 ** 60 - 1, 2 ** 60, 2 ** 61 - 2, 2 ** 61 - 1,
+                      2 ** 61, 2 ** 63 + 99, 2 ** 64 - 1], dtype=np.uint64)
+    ge = g.estimate(torch.from_numpy(cells.view(np.int64)).cuda()).cpu().numpy()
+    assert np.array_equal(ge, o.estimate(cells))
+    g.close()
+
+
+# ---- candidate-list machinery: overflow, retry, growth ----------------------------------------------------------
+
+def test_small_candidate_capacity_forces_overflow_and_growth(cs):
+    """Capacity 1024 with ~10^5 occupied cells, k = 5000 and a low excursion threshold: the list overflows,
+    is compacted, the chunk is re-run, and the list grows; the result must not change."""
+    wl, xyz = _gen("cfg1", 1 << 18)
+    st = _check_all(cs, wl, xyz, k=5000, thresholds=(2,), cap=1024)
+    assert st["compactions"] >= 2
+
+
+def test_heavy_duplication_single_cell(cs):
+    """All particles in one cell: every scanned particle is a duplicate candidate."""
+    from paper_1711_00975_b200 import synth
+    pos = np.full((300000, 3), 3.3, dtype=np.float32)
+    wl = synth.Workload("one", N=len(pos), G=(32,), d=5, w=1 << 10, k=10, H=1, f_bg=0.0, m_min=0, L=10.0)
+    _check_all(cs, wl, torch.from_numpy(pos).cuda(), k=10, cap=4096)
+
+
+def test_scan_cells_merges_candidates(cs):
+    """cs_scan_cells: candidates given as ids give the same selection as scanning the particles."""
+    wl, xyz = _gen("cfg1", 1 << 18)
+    host = xyz.cpu().numpy()
+    o = ora.OracleSketch(wl.d, wl.w, wl.G, wl.L, wl.seed)
+    g = cs.CountSketch(wl.d, wl.w, list(wl.G), wl.L, wl.seed)
+    o.update(host)
+    g.update(xyz)
+    o.scan_begin()
+    o.scan(host)
+    cells = ora.quantise(host, wl.G[0], wl.L)
+    g.scan_begin(100)
+    half = len(cells) // 2
+    g.scan(xyz[:half])
+    g.scan_cells(torch.from_numpy(cells[half:].view(np.int64)).cuda())
+    gi, gv = g.topk(100)
+    oi, ov = o.topk(100)
+    assert np.array_equal(_ids(gi), oi) and np.array_equal(gv.cpu().numpy(), ov)
+    g.close()
+
+
+# ---- table access, linearity, state ------------------------------------------------------------------------------
+
+def test_sketch_add_reset_and_sharded_indices(cs):
+    """sketches of stream shards sum to the sketch of the stream (also under sampling when each
+    shard continues the running index)."""
+    wl, xyz = _gen("cfg1", 200001)
+    host = xyz.cpu().numpy()
+    p = 0.3
+    o = ora.OracleSketch(wl.d, wl.w, wl.G, wl.L, wl.seed)
+    o.update(host, p)
+    a = cs.CountSketch(wl.d, wl.w, list(wl.G), wl.L, wl.seed)
+    b = cs.CountSketch(wl.d, wl.w, list(wl.G), wl.L, wl.seed)
+    cut = 77777
+    a.update(xyz[:cut], p)
+    b.set_update_index(cut)
+    b.update(xyz[cut:], p)
+    assert b.update_index() == len(host)
+    a.sketch_add(b.sketch())                 # device table
+    assert np.array_equal(a.sketch().cpu().numpy(), o.sketch())
+    a.sketch_add(b.sketch(device="cpu"))     # host table
+    a.reset()
+    assert int(a.sketch().abs().sum()) == 0 and a.update_index() == 0
+    a.update(xyz, p)
+    assert np.array_equal(a.sketch(device="cpu").numpy(), o.sketch())
+    a.close()
+    b.close()
+
+
+def test_call_order_and_argument_errors(cs):
+    g = cs.CountSketch(3, 64, 8, 1.0, 1)
+    xyz = torch.rand(100, 3, device="cuda")
+    with pytest.raises(cs.CsError) as e:
+        g.scan(xyz)
+    assert e.value.code == cs.CS_ERR_STATE
+    with pytest.raises(cs.CsError) as e:
+        g.topk(1)
+    assert e.value.code == cs.CS_ERR_STATE
+    g.scan_begin(5, 3)
+    g.scan(xyz)
+    for bad in (lambda: g.topk(6), lambda: g.excursion(2), lambda: g.update(xyz, 0.0), lambda: g.update(xyz, 1.5),
+                lambda: g.estimate(torch.zeros(1, dtype=torch.int64, device="cuda"), scale=1)):
+        with pytest.raises(cs.CsError) as e:
+            bad()
+        assert e.value.code == cs.CS_ERR_ARG
+    ids, est = g.topk(5)
+    assert len(ids) == 5
+    assert g.launch_count() > 0
+    g.close()
