@@ -94,6 +94,11 @@ int cs_reset(cs_sketch* s);
 /* Use `cuda_stream` (a cudaStream_t, e.g. torch.cuda.current_stream().cuda_stream) for all later work. */
 int cs_set_stream(cs_sketch* s, void* cuda_stream);
 
+/* Bytes of counters one update pass may touch (default 64 MiB).  When d*w*4*n_scales exceeds it, cs_update
+ * splits the rows (or scales) into groups of at most this size and re-reads the positions once per group, so
+ * that the red.global.add traffic of each pass stays L2-resident.  The result does not depend on it. */
+int cs_set_table_budget(cs_sketch* s, uint64_t bytes);
+
 /* Running particle index of the update stream / of the current scan (sampling, R13, R17).
  * Setting it lets a stream shard (multi-GPU) reproduce the single-stream sampling decisions. */
 int cs_set_update_index(cs_sketch* s, uint64_t index);

@@ -28,6 +28,7 @@ SIGNATURES = {
     "cs_destroy": (ci, [vp]),
     "cs_reset": (ci, [vp]),
     "cs_set_stream": (ci, [vp, vp]),
+    "cs_set_table_budget": (ci, [vp, u64]),
     "cs_set_update_index": (ci, [vp, u64]),
     "cs_set_scan_index": (ci, [vp, u64]),
     "cs_get_update_index": (ci, [vp, vp]),
@@ -141,6 +142,9 @@ class CountSketch:
     def set_stream(self, stream: torch.cuda.Stream):
         self._stream = stream
         _chk(lib().cs_set_stream(self._h, vp(stream.cuda_stream)), "cs_set_stream")
+
+    def set_table_budget(self, nbytes: int):
+        _chk(lib().cs_set_table_budget(self._h, nbytes), "cs_set_table_budget")
 
     def set_update_index(self, index: int):
         _chk(lib().cs_set_update_index(self._h, index), "cs_set_update_index")

@@ -16,12 +16,12 @@ template <int MODE>
 __global__ void __launch_bounds__(256)
 k_probe_l2(int32_t* __restrict__ table, uint64_t words, uint64_t n_ops, uint64_t salt, int32_t* sink) {
     const uint64_t stride = (uint64_t)gridDim.x * blockDim.x;
-    const uint32_t mask = (uint32_t)(words - 1);             /* words is a power of two */
+    const uint32_t nw = (uint32_t)words;                     /* address = (rand32 * words) >> 32: any table size */
     int32_t acc = 0;
     /* one 64-bit mix gives two addresses (the real kernel spends more ALU per atomic than this) */
     for (uint64_t i = (uint64_t)blockIdx.x * blockDim.x + threadIdx.x; 2 * i < n_ops; i += stride) {
         uint64_t r = probe_rng(i + salt);
-        uint32_t a0 = (uint32_t)r & mask, a1 = (uint32_t)(r >> 32) & mask;
+        uint32_t a0 = __umulhi((uint32_t)r, nw), a1 = __umulhi((uint32_t)(r >> 32), nw);
         int32_t v = 1 - 2 * (int32_t)((r >> 31) & 1u);
         if (MODE == 0) {
             red_add(table + a0, v);
@@ -60,9 +60,8 @@ using namespace cs;
 extern "C" int cs_probe_l2(int mode, uint64_t table_bytes, uint64_t n_ops, int reps, void* cuda_stream,
                            double* ms_out) {
     if (mode < 0 || mode > 2 || !ms_out || reps < 1 || table_bytes < 4) return CS_ERR_ARG;
-    uint64_t words = 1;
-    while (words * 2 * 4 <= table_bytes) words *= 2;         /* largest power of two that fits */
-    if (words > (1ull << 32)) return CS_ERR_ARG;
+    const uint64_t words = table_bytes / 4;
+    if (words >= (1ull << 32)) return CS_ERR_ARG;
     cudaStream_t st = (cudaStream_t)cuda_stream;
     int32_t* table = nullptr;
     int32_t* sink = nullptr;

@@ -12,78 +12,9 @@
  */
 #include "cs_device.cuh"
 #include "cs_launch.cuh"
+#include "cs_scan_common.cuh"
 
 namespace cs {
-
-__device__ __forceinline__ int32_t ld_table(const int32_t* p) {
-    int32_t v;
-    asm volatile("ld.global.relaxed.gpu.s32 %0, [%1];" : "=r"(v) : "l"(p));   // L2 is the point of coherence
-    return v;
-}
-
-/* s_j(c) * T[j][h_j(c)] for row j of scale s */
-template <bool BIG, bool POW2>
-__device__ __forceinline__ int32_t row_value(const PassParams& P, const int32_t* T, const RowCoef& rc, int j,
-                                             uint32_t c0, uint32_t c1) {
-    uint32_t b;
-    int32_t sg;
-    bucket_sign<BIG, POW2>(rc, c0, c1, P.w, b, sg);
-    return mul_sign(ld_table(T + (uint64_t)j * P.w + b), sg);
-}
-
-/* Estimate with early exit.  Returns true iff Estimate(c) >= tau; then est holds the estimate. */
-template <int D, bool POW2, bool BIG>
-__device__ __forceinline__ bool estimate_ge(const PassParams& P, int s, uint64_t c, int32_t tau, int32_t& est) {
-    const int d = D ? D : P.d;
-    const int max_fail = (d - 1) / 2;            // est >= tau  <=>  at most (d-1)/2 row values are < tau
-    const uint32_t c0 = (uint32_t)c, c1 = (uint32_t)(c >> 32);
-    const int32_t* T = P.sc[s].T;
-    const RowCoef* rows = &P.rows[s * d];
-    int32_t v[D ? D : CS_MAX_ROWS];
-    int fail = 0;
-#pragma unroll
-    for (int j = 0; j < d; ++j) {
-        if (fail <= max_fail) {
-            v[j] = row_value<BIG, POW2>(P, T, rows[j], j, c0, c1);
-            fail += (v[j] < tau);
-        }
-    }
-    if (fail > max_fail) return false;
-    if constexpr (D > 0) est = median_of<D>(v);
-    else                 est = median_rt(v, d);
-    return true;
-}
-
-template <int D, bool POW2, bool BIG>
-__device__ __forceinline__ int32_t estimate_full(const PassParams& P, int s, uint64_t c) {
-    int32_t est = 0;
-    estimate_ge<D, POW2, BIG>(P, s, c, INT32_MIN, est);
-    return est;
-}
-
-/* Warp-aggregated append of (c, est) to the candidate list of one scale.  Must be reached by all 32 lanes. */
-__device__ __forceinline__ void append_candidate(const ScanTarget& tg, bool emit, uint64_t c, int32_t est) {
-    const uint32_t mask = __ballot_sync(0xFFFFFFFFu, emit);
-    if (mask == 0) return;
-    const uint32_t lane = threadIdx.x & 31u;
-    const int leader = __ffs(mask) - 1;
-    int32_t lo = __reduce_min_sync(0xFFFFFFFFu, emit ? est : INT32_MAX);
-    int32_t hi = __reduce_max_sync(0xFFFFFFFFu, emit ? est : INT32_MIN);
-    uint32_t base = 0;
-    if ((int)lane == leader) {
-        base = atomicAdd(&tg.st->count, (uint32_t)__popc(mask));
-        atomicMin(&tg.st->est_min, lo);
-        atomicMax(&tg.st->est_max, hi);
-    }
-    base = __shfl_sync(0xFFFFFFFFu, base, leader);
-    if (emit) {
-        uint64_t pos = (uint64_t)base + __popc(mask & ((1u << lane) - 1u));
-        if (pos < tg.cap) {
-            tg.id[pos] = c;
-            tg.ek[pos] = est_to_key(est);
-        }
-    }
-}
 
 template <int D, bool POW2>
 __device__ __forceinline__ void scan_particle(const PassParams& P, const ScanParams& S, const int32_t* tau,
@@ -152,23 +83,6 @@ k_scan(const __grid_constant__ PassParams P, const __grid_constant__ ScanParams 
     }
 }
 
-/* Estimate of an arbitrary caller-supplied 64-bit cell id (any value: ids >= 2^60 take the __umul64hi form). */
-template <int D, bool POW2>
-__device__ __forceinline__ int32_t estimate_any(const PassParams& P, int s, uint64_t c) {
-    if ((c >> 32) == 0) return estimate_full<D, POW2, false>(P, s, c);
-    if ((c >> 60) == 0) return estimate_full<D, POW2, true>(P, s, c);
-    const int d = D ? D : P.d;
-    int32_t v[CS_MAX_ROWS];
-    for (int j = 0; j < d; ++j) {
-        const RowCoef& rc = P.rows[s * d + j];
-        uint64_t r = affine_mod_p_wide(coef_a(rc.h), rc.h.b, c);
-        uint64_t r2 = affine_mod_p_wide(coef_a(rc.s), rc.s.b, c);
-        uint32_t b = POW2 ? ((uint32_t)r & (uint32_t)(P.w - 1)) : (uint32_t)(r % P.w);
-        v[j] = mul_sign(ld_table(P.sc[s].T + (uint64_t)j * P.w + b), 1 - 2 * (int32_t)((uint32_t)r2 & 1u));
-    }
-    return median_rt(v, d);
-}
-
 template <int D, bool POW2>
 __global__ void __launch_bounds__(PASS_THREADS)
 k_estimate(const __grid_constant__ PassParams P, int s, const uint64_t* __restrict__ cells, uint64_t m,
@@ -201,15 +115,6 @@ k_scan_cells(const __grid_constant__ PassParams P, const __grid_constant__ ScanP
 
 /* ---- dispatch on (d, w power of two) ------------------------------------------------------------------ */
 
-#define CS_DISPATCH_D(CALL)                                    \
-    switch (P.d) {                                             \
-        case 1: CALL(1); break;  case 2: CALL(2); break;       \
-        case 3: CALL(3); break;  case 4: CALL(4); break;       \
-        case 5: CALL(5); break;  case 6: CALL(6); break;       \
-        case 7: CALL(7); break;  case 8: CALL(8); break;       \
-        default: CALL(0); break;                               \
-    }
-
 template <bool POW2>
 static cudaError_t launch_scan_p(const PassParams& P, const ScanParams& S, const float* xyz, uint64_t n, int sm,
                                  cudaStream_t st) {
@@ -232,11 +137,6 @@ cudaError_t launch_scan(const PassParams& P, const ScanParams& S, const float* x
     return pow2 ? launch_scan_p<true>(P, S, xyz, n, sm_count, st) : launch_scan_p<false>(P, S, xyz, n, sm_count, st);
 }
 
-static int blocks_1d(uint64_t m) {
-    uint64_t b = (m + PASS_THREADS - 1) / PASS_THREADS;
-    if (b > 148 * 8) b = 148 * 8;
-    return (int)(b < 1 ? 1 : b);
-}
 
 template <bool POW2>
 static cudaError_t launch_estimate_p(const PassParams& P, int scale, const uint64_t* cells, uint64_t m,
