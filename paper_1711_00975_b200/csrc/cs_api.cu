@@ -81,7 +81,7 @@ int bit_length(uint64_t v) {
 
 constexpr int STAGE_SLOTS = 3;
 constexpr uint64_t STAGE_PARTICLES = 1ull << 24;      /* 192 MiB per staging slot */
-constexpr uint64_t MAX_CHUNK = 1ull << 26;            /* particles per scan launch */
+constexpr uint64_t MAX_CHUNK = 1ull << 25;            /* particles per scan launch */
 constexpr uint32_t MIN_CAP = 1u << 22;                /* candidate entries per scale */
 
 }  // namespace
@@ -120,6 +120,9 @@ struct cs_sketch {
     uint64_t* out_ids = nullptr;      /* staging for cs_topk / cs_excursion results */
     int32_t* out_est = nullptr;
     uint64_t out_cap = 0;
+
+    /* survivor lists of the row-partitioned scan */
+    StageBuffers stb = {};
 
     /* host streaming */
     float* stage[STAGE_SLOTS] = {};
@@ -279,6 +282,68 @@ int update_passes(cs_sketch* s, const float* xyz, uint64_t n, uint64_t index0, d
 
 namespace {
 
+void free_stage_lists(cs_sketch* s) {
+    for (int h = 0; h < 2; ++h) {
+        if (s->stb.list[h]) cudaFree(s->stb.list[h]);
+        if (s->stb.cnt[h]) cudaFree(s->stb.cnt[h]);
+        s->stb.list[h] = nullptr;
+        s->stb.cnt[h] = nullptr;
+    }
+    s->stb.cap_entries = 0;
+}
+
+int ensure_stage_lists(cs_sketch* s, uint64_t n) {
+    const uint32_t blocks = (uint32_t)s->sm_count * 8;
+    const uint64_t need = staged_list_entries(n, blocks);
+    if (s->stb.cap_entries >= need && s->stb.blocks == blocks) return CS_OK;
+    CS_CUDA(cudaStreamSynchronize(s->stream));
+    free_stage_lists(s);
+    for (int h = 0; h < 2; ++h) {
+        CS_CUDA(cudaMalloc(&s->stb.list[h], need * sizeof(uint64_t)));
+        CS_CUDA(cudaMalloc(&s->stb.cnt[h], blocks * sizeof(uint32_t)));
+    }
+    s->stb.blocks = blocks;
+    s->stb.cap_entries = need;
+    return CS_OK;
+}
+
+/* One scan launch over a chunk, shaped by the table budget: everything at once when all
+ * tables fit; else scale by scale -- the one-kernel scan when the scale fits, the staged pipeline when not. */
+int launch_scan_chunk(cs_sketch* s, const float* xyz, uint64_t n, uint64_t index0, double sample_p) {
+    const PassParams full = pass_params(s, index0, sample_p);
+    ScanParams S;
+    fill_scan_params(s, &S);
+    const uint64_t row_bytes = s->w * sizeof(int32_t);
+    const uint64_t scale_bytes = row_bytes * s->d;
+    cudaError_t e = cudaSuccess;
+    if (scale_bytes * s->n_scales <= s->table_budget) {
+        e = launch_scan(full, S, xyz, n, s->sm_count, s->stream);
+        s->launches += 1;
+    } else {
+        for (int i = 0; i < s->n_scales && e == cudaSuccess; ++i) {
+            PassParams P = full;
+            P.n_scales = 1;
+            P.sc[0] = full.sc[i];
+            for (int j = 0; j < s->d; ++j) P.rows[j] = full.rows[i * s->d + j];
+            if (scale_bytes <= s->table_budget) {
+                ScanParams S1 = {};
+                S1.tg[0] = S.tg[i];
+                e = launch_scan(P, S1, xyz, n, s->sm_count, s->stream);
+                s->launches += 1;
+            } else {
+                int rc = ensure_stage_lists(s, n);
+                if (rc) return rc;
+                uint64_t fit = s->table_budget / row_bytes;
+                if (fit < 1) fit = 1;
+                e = launch_scan_staged(P, S.tg[i], s->stb, (int)(fit > 8 ? 8 : fit), xyz, n, s->stream, &s->launches);
+            }
+        }
+    }
+    if (e != cudaSuccess) return fail(CS_ERR_CUDA, "scan kernel: %s", cudaGetErrorString(e));
+    s->n_scan_launches += 1;
+    return CS_OK;
+}
+
 /* After a chunk: which scales must be compacted now (list past half the buffer, or doubled since last time). */
 bool wants_compaction(const cs_sketch* s, int i) {
     const uint32_t c = s->st_host[i].count;
@@ -332,14 +397,9 @@ int scan_device(cs_sketch* s, const float* xyz, uint64_t n, double sample_p) {
         for (;;) {
             uint32_t before[CS_MAX_SCALES];
             for (int i = 0; i < s->n_scales; ++i) before[i] = s->st_host[i].count;
-            ScanParams S;
-            fill_scan_params(s, &S);
-            PassParams P = pass_params(s, s->scan_index + done, sample_p);
-            cudaError_t e = launch_scan(P, S, xyz + 3 * done, chunk, s->sm_count, s->stream);
-            if (e != cudaSuccess) return fail(CS_ERR_CUDA, "scan kernel: %s", cudaGetErrorString(e));
-            s->launches += 1;
-            s->n_scan_launches += 1;
-            int rc = read_states(s);
+            int rc = launch_scan_chunk(s, xyz + 3 * done, chunk, s->scan_index + done, sample_p);
+            if (rc) return rc;
+            rc = read_states(s);
             if (rc) return rc;
             bool overflow = false;
             double r = 0.0;
@@ -551,6 +611,7 @@ int cs_destroy(cs_sketch* s) {
     if (s->stream || s->T[0]) cudaStreamSynchronize(s->stream);
     if (s->copy_stream) cudaStreamSynchronize(s->copy_stream);
     free_candidates(s);
+    free_stage_lists(s);
     for (int i = 0; i < CS_MAX_SCALES; ++i) if (s->T[i]) cudaFree(s->T[i]);
     if (s->st_dev) cudaFree(s->st_dev);
     if (s->st_host) cudaFreeHost(s->st_host);

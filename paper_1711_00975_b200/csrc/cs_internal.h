@@ -77,6 +77,16 @@ struct ScanParams {
 cudaError_t launch_update(const PassParams& P, const float* xyz, uint64_t n, int sm_count, cudaStream_t st);
 cudaError_t launch_scan(const PassParams& P, const ScanParams& S, const float* xyz, uint64_t n, int sm_count,
                         cudaStream_t st);
+/* row-partitioned scan of one scale (cs_scan_staged.cu) */
+struct StageBuffers {
+    uint64_t* list[2];     // survivor lists (ping-pong), cap_entries each
+    uint32_t* cnt[2];      // entries per segment, `blocks` words each
+    uint32_t blocks;       // grid size of every stage = number of segments
+    uint64_t cap_entries;
+};
+uint64_t staged_list_entries(uint64_t n, uint32_t blocks);
+cudaError_t launch_scan_staged(const PassParams& P, const ScanTarget& tg, const StageBuffers& B, int rows_per_stage,
+                               const float* xyz, uint64_t n, cudaStream_t st, uint64_t* launches);
 cudaError_t launch_scan_cells(const PassParams& P, const ScanParams& S, int scale, const uint64_t* cells,
                               uint64_t m, cudaStream_t st);
 cudaError_t launch_estimate(const PassParams& P, int scale, const uint64_t* cells, uint64_t m, int32_t* est,

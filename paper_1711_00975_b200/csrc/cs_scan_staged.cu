@@ -1,0 +1,241 @@
+/*
+ * cs_scan_staged.cu -- row-partitioned candidate re-scan for sketches larger than the L2-resident budget
+ * (DESIGN.md section 6).
+ *
+ * Random 4-byte gathers run at ~290 G/s while the rows they touch stay L2-resident and at ~130 G/s (112 MiB)
+ * to ~50 G/s (448 MiB) when they do not (measured, cs_probe_l2 mode 2).  The d rows of one scale are therefore
+ * split into groups that fit the budget and the scan becomes a pipeline of stages, one per group:
+ *   stage 0      positions -> cell id c, row values of group 0, fails = #{values < tau};
+ *                a cell is dropped once fails > (d-1)/2 (its median is then < tau);
+ *                survivors are written as (c | fails << 60) to a list
+ *   stage i      list -> rows of group i -> list
+ *   last stage   survivors have Estimate(c) >= tau: the full median over all d rows is recomputed for them
+ *                (they are few) and (c, est) is appended to the candidate list.
+ * Lists are segmented per block (block b of every stage owns segment b), so no global atomic is needed for the
+ * survivor lists and the result does not depend on scheduling (the candidate list is sorted afterwards).
+ */
+#include "cs_scan_common.cuh"
+
+namespace cs {
+
+constexpr uint64_t FAIL_SHIFT = 60;
+constexpr uint64_t CELL_MASK = (1ULL << FAIL_SHIFT) - 1;
+
+struct StageParams {
+    const uint64_t* in;      // survivor list of the previous stage (unused by stage 0)
+    uint64_t* out;           // survivor list of this stage (unused by the last stage)
+    const uint32_t* cnt_in;  // entries per segment
+    uint32_t* cnt_out;
+    uint32_t seg_cap;        // entries per segment
+    int32_t row0;            // first row of this stage's group
+    int32_t d_all;           // rows of the scale (for the final median)
+    int32_t pad;
+};
+
+/* Row values of rows [row0, row0 + R) of the (single) scale in P; returns the updated fail count. */
+template <int R, bool POW2, bool BIG>
+__device__ __forceinline__ int stage_rows(const PassParams& P, int row0, uint64_t c, int32_t tau, int fails,
+                                          int max_fail) {
+    const uint32_t c0 = (uint32_t)c, c1 = (uint32_t)(c >> 32);
+    const int32_t* T = P.sc[0].T;
+#pragma unroll
+    for (int j = 0; j < R; ++j) {
+        if (fails <= max_fail) {
+            int32_t v = row_value<BIG, POW2>(P, T, P.rows[row0 + j], row0 + j, c0, c1);
+            fails += (v < tau);
+        }
+    }
+    return fails;
+}
+
+template <bool POW2, bool BIG>
+__device__ __noinline__ int32_t estimate_all_rows(const PassParams& P, int d, uint64_t c) {
+    const uint32_t c0 = (uint32_t)c, c1 = (uint32_t)(c >> 32);
+    int32_t v[CS_MAX_ROWS];
+    for (int j = 0; j < d; ++j) v[j] = row_value<BIG, POW2>(P, P.sc[0].T, P.rows[j], j, c0, c1);
+    return median_rt(v, d);
+}
+
+/* One cell through one stage.  Must be reached by all 32 lanes (the appends are warp-aggregated). */
+template <int R, bool POW2, bool LAST>
+__device__ __forceinline__ void stage_cell(const PassParams& P, const StageParams& Q, const ScanTarget& tg,
+                                           int32_t tau, int max_fail, bool live, uint64_t c, int fails,
+                                           uint64_t* seg_out, uint32_t* s_cnt) {
+    if (live) {
+        fails = P.sc[0].big ? stage_rows<R, POW2, true>(P, Q.row0, c, tau, fails, max_fail)
+                            : stage_rows<R, POW2, false>(P, Q.row0, c, tau, fails, max_fail);
+        live = fails <= max_fail;
+    }
+    if (LAST) {
+        int32_t est = 0;
+        if (live) est = P.sc[0].big ? estimate_all_rows<POW2, true>(P, Q.d_all, c)
+                                    : estimate_all_rows<POW2, false>(P, Q.d_all, c);
+        append_candidate(tg, live, c, est);
+    } else {
+        const uint32_t mask = __ballot_sync(0xFFFFFFFFu, live);
+        if (mask) {
+            const uint32_t lane = threadIdx.x & 31u;
+            const int leader = __ffs(mask) - 1;
+            uint32_t base = 0;
+            if ((int)lane == leader) base = atomicAdd(s_cnt, (uint32_t)__popc(mask));
+            base = __shfl_sync(0xFFFFFFFFu, base, leader);
+            if (live) seg_out[base + __popc(mask & ((1u << lane) - 1u))] = c | ((uint64_t)fails << FAIL_SHIFT);
+        }
+    }
+}
+
+/* Stage 0: block b owns position groups [b*gpb, (b+1)*gpb); block 0 also takes the <= 6 edge particles. */
+template <int R, bool POW2, bool LAST>
+__global__ void __launch_bounds__(PASS_THREADS)
+k_stage_first(const __grid_constant__ PassParams P, const __grid_constant__ StageParams Q,
+              const __grid_constant__ ScanTarget tg, const float* __restrict__ xyz, uint64_t n, uint32_t head,
+              uint64_t groups, uint64_t gpb) {
+    __shared__ uint32_t s_cnt;
+    if (threadIdx.x == 0) s_cnt = 0;
+    __syncthreads();
+    const int32_t tau = tg.st->tau;
+    const int max_fail = (Q.d_all - 1) / 2;
+    uint64_t* seg = LAST ? nullptr : Q.out + (uint64_t)blockIdx.x * Q.seg_cap;
+    const float4* body = reinterpret_cast<const float4*>(xyz + 3 * (uint64_t)head);
+    const uint64_t g_lo = (uint64_t)blockIdx.x * gpb;
+    const uint64_t g_hi = g_lo + gpb < groups ? g_lo + gpb : groups;
+    const uint32_t lane = threadIdx.x & 31u;
+    for (uint64_t g0 = g_lo + (threadIdx.x - lane); g0 < g_hi; g0 += PASS_THREADS) {
+        const uint64_t g = g0 + lane;
+        const bool in = g < g_hi;
+        float4 q0 = make_float4(0.f, 0.f, 0.f, 0.f), q1 = q0, q2 = q0;
+        if (in) {
+            q0 = ld_stream16(body + 3 * g);
+            q1 = ld_stream16(body + 3 * g + 1);
+            q2 = ld_stream16(body + 3 * g + 2);
+        }
+        bool k0 = in, k1 = in, k2 = in, k3 = in;
+        if (P.sample && in) {
+            const uint64_t i0 = P.index0 + head + 4 * g;
+            k0 = keep_particle(P.K, i0 + 0, P.Tp);
+            k1 = keep_particle(P.K, i0 + 1, P.Tp);
+            k2 = keep_particle(P.K, i0 + 2, P.Tp);
+            k3 = keep_particle(P.K, i0 + 3, P.Tp);
+        }
+        stage_cell<R, POW2, LAST>(P, Q, tg, tau, max_fail, k0, cell_of(q0.x, q0.y, q0.z, P.sc[0]), 0, seg, &s_cnt);
+        stage_cell<R, POW2, LAST>(P, Q, tg, tau, max_fail, k1, cell_of(q0.w, q1.x, q1.y, P.sc[0]), 0, seg, &s_cnt);
+        stage_cell<R, POW2, LAST>(P, Q, tg, tau, max_fail, k2, cell_of(q1.z, q1.w, q2.x, P.sc[0]), 0, seg, &s_cnt);
+        stage_cell<R, POW2, LAST>(P, Q, tg, tau, max_fail, k3, cell_of(q2.y, q2.z, q2.w, P.sc[0]), 0, seg, &s_cnt);
+    }
+    if (blockIdx.x == 0 && threadIdx.x < 32) {
+        const uint64_t tail0 = (uint64_t)head + 4 * groups;
+        const uint64_t n_edge = (uint64_t)head + (n - tail0);
+        bool keep = false;
+        uint64_t c = 0;
+        if (threadIdx.x < n_edge) {
+            const uint64_t i = threadIdx.x < head ? threadIdx.x : tail0 + (threadIdx.x - head);
+            keep = !P.sample || keep_particle(P.K, P.index0 + i, P.Tp);
+            const float* p = xyz + 3 * i;
+            c = cell_of(ld_stream4(p), ld_stream4(p + 1), ld_stream4(p + 2), P.sc[0]);
+        }
+        stage_cell<R, POW2, LAST>(P, Q, tg, tau, max_fail, keep, c, 0, seg, &s_cnt);
+    }
+    if (!LAST) {
+        __syncthreads();
+        if (threadIdx.x == 0) Q.cnt_out[blockIdx.x] = s_cnt;
+    }
+}
+
+/* Stage i > 0: block b reads segment b of the previous stage. */
+template <int R, bool POW2, bool LAST>
+__global__ void __launch_bounds__(PASS_THREADS)
+k_stage_next(const __grid_constant__ PassParams P, const __grid_constant__ StageParams Q,
+             const __grid_constant__ ScanTarget tg) {
+    __shared__ uint32_t s_cnt;
+    if (threadIdx.x == 0) s_cnt = 0;
+    __syncthreads();
+    const int32_t tau = tg.st->tau;
+    const int max_fail = (Q.d_all - 1) / 2;
+    const uint64_t* seg_in = Q.in + (uint64_t)blockIdx.x * Q.seg_cap;
+    uint64_t* seg = LAST ? nullptr : Q.out + (uint64_t)blockIdx.x * Q.seg_cap;
+    const uint32_t cnt = Q.cnt_in[blockIdx.x];
+    for (uint32_t t0 = 0; t0 < cnt; t0 += PASS_THREADS) {
+        const uint32_t t = t0 + threadIdx.x;
+        const bool live = t < cnt;
+        const uint64_t e = live ? seg_in[t] : 0;
+        stage_cell<R, POW2, LAST>(P, Q, tg, tau, max_fail, live, e & CELL_MASK, (int)(e >> FAIL_SHIFT), seg, &s_cnt);
+    }
+    if (!LAST) {
+        __syncthreads();
+        if (threadIdx.x == 0) Q.cnt_out[blockIdx.x] = s_cnt;
+    }
+}
+
+/* ---- host side ------------------------------------------------------------------------------------------ */
+
+template <int R, bool POW2, bool LAST>
+static void launch_stage(bool first, int blocks, const PassParams& P, const StageParams& Q, const ScanTarget& tg,
+                         const float* xyz, uint64_t n, uint32_t head, uint64_t groups, uint64_t gpb, cudaStream_t st) {
+    if (first) k_stage_first<R, POW2, LAST><<<blocks, PASS_THREADS, 0, st>>>(P, Q, tg, xyz, n, head, groups, gpb);
+    else       k_stage_next<R, POW2, LAST><<<blocks, PASS_THREADS, 0, st>>>(P, Q, tg);
+}
+
+template <bool POW2, bool LAST>
+static void launch_stage_r(int R, bool first, int blocks, const PassParams& P, const StageParams& Q,
+                           const ScanTarget& tg, const float* xyz, uint64_t n, uint32_t head, uint64_t groups,
+                           uint64_t gpb, cudaStream_t st) {
+    switch (R) {
+        case 1: launch_stage<1, POW2, LAST>(first, blocks, P, Q, tg, xyz, n, head, groups, gpb, st); break;
+        case 2: launch_stage<2, POW2, LAST>(first, blocks, P, Q, tg, xyz, n, head, groups, gpb, st); break;
+        case 3: launch_stage<3, POW2, LAST>(first, blocks, P, Q, tg, xyz, n, head, groups, gpb, st); break;
+        case 4: launch_stage<4, POW2, LAST>(first, blocks, P, Q, tg, xyz, n, head, groups, gpb, st); break;
+        case 5: launch_stage<5, POW2, LAST>(first, blocks, P, Q, tg, xyz, n, head, groups, gpb, st); break;
+        case 6: launch_stage<6, POW2, LAST>(first, blocks, P, Q, tg, xyz, n, head, groups, gpb, st); break;
+        case 7: launch_stage<7, POW2, LAST>(first, blocks, P, Q, tg, xyz, n, head, groups, gpb, st); break;
+        default: launch_stage<8, POW2, LAST>(first, blocks, P, Q, tg, xyz, n, head, groups, gpb, st); break;
+    }
+}
+
+uint64_t staged_list_entries(uint64_t n, uint32_t blocks) {
+    const uint64_t groups = n / 4 + 1;
+    const uint64_t gpb = (groups + blocks - 1) / blocks;
+    return (uint64_t)blocks * (4 * gpb + 8);
+}
+
+/* P: PassParams of ONE scale (n_scales = 1, rows[0..d), d = all its rows).  rows_per_stage in [1, 8]. */
+cudaError_t launch_scan_staged(const PassParams& P, const ScanTarget& tg, const StageBuffers& B, int rows_per_stage,
+                               const float* xyz, uint64_t n, cudaStream_t st, uint64_t* launches) {
+    uint32_t head;
+    uint64_t groups;
+    split_aligned(xyz, n, &head, &groups);
+    const int blocks = (int)B.blocks;
+    const uint64_t gpb = (groups + blocks - 1) / blocks;
+    const uint32_t seg_cap = (uint32_t)(4 * gpb + 8);
+    if ((uint64_t)blocks * seg_cap > B.cap_entries) return cudaErrorInvalidValue;
+    const bool pow2 = (P.w & (P.w - 1)) == 0;
+    if (rows_per_stage > 8) rows_per_stage = 8;
+    if (rows_per_stage < 1) rows_per_stage = 1;
+    const int stages = (P.d + rows_per_stage - 1) / rows_per_stage;
+    const int each = (P.d + stages - 1) / stages;                 /* balanced groups */
+    int cur = 0;
+    for (int row0 = 0, i = 0; row0 < P.d; row0 += each, ++i) {
+        const int R = row0 + each <= P.d ? each : P.d - row0;
+        const bool last = row0 + R >= P.d;
+        StageParams Q;
+        Q.in = B.list[cur];
+        Q.cnt_in = B.cnt[cur];
+        Q.out = B.list[cur ^ 1];
+        Q.cnt_out = B.cnt[cur ^ 1];
+        Q.seg_cap = seg_cap;
+        Q.row0 = row0;
+        Q.d_all = P.d;
+        Q.pad = 0;
+        if (pow2) {
+            if (last) launch_stage_r<true, true>(R, i == 0, blocks, P, Q, tg, xyz, n, head, groups, gpb, st);
+            else      launch_stage_r<true, false>(R, i == 0, blocks, P, Q, tg, xyz, n, head, groups, gpb, st);
+        } else {
+            if (last) launch_stage_r<false, true>(R, i == 0, blocks, P, Q, tg, xyz, n, head, groups, gpb, st);
+            else      launch_stage_r<false, false>(R, i == 0, blocks, P, Q, tg, xyz, n, head, groups, gpb, st);
+        }
+        *launches += 1;
+        cur ^= 1;
+    }
+    return cudaGetLastError();
+}
+
+}  // namespace cs

@@ -36,12 +36,14 @@ def _ids(t):
     return t.cpu().numpy().view(np.uint64)
 
 
-def _check_all(cs, wl, xyz, sample_p=1.0, k=None, thresholds=(), probe_cells=4096, split=None, cap=None):
+def _check_all(cs, wl, xyz, sample_p=1.0, k=None, thresholds=(), probe_cells=4096, split=None, cap=None, budget=None):
     """Update + estimate + scan + top-k (+ excursion) on both sides; everything must be identical."""
     k = wl.k if k is None else k
     host = xyz.cpu().numpy()
     o = ora.OracleSketch(wl.d, wl.w, wl.G, wl.L, wl.seed)
     g = cs.CountSketch(wl.d, wl.w, list(wl.G), wl.L, wl.seed)
+    if budget:
+        g.set_table_budget(budget)
     n = host.shape[0]
     cuts = [0, n] if not split else [0] + sorted(split) + [n]
     for a, b in zip(cuts[:-1], cuts[1:]):
@@ -143,6 +145,31 @@ def test_cfg5_reduced_multiscale_sampled(cs):
     """4 nested grids in one pass, hash-Bernoulli sampling p = 0.1, thresholds and top-k per scale."""
     wl, xyz = _gen("cfg5", 1 << 22)
     _check_all(cs, wl, xyz, sample_p=wl.sample_p, k=1000, thresholds=(3, 4, 6), split=[1000001, 3000000])
+
+
+# ---- row-partitioned passes (table budget below the sketch size) ------------------------------------------------
+
+@pytest.mark.parametrize("rows_fit", [1, 2, 4, 6])
+def test_row_partitioned_update_and_staged_scan(cs, rows_fit):
+    """Budget of 1 / 2 / 4 / 6 rows of a d = 7 sketch: update in row groups, scan as a pipeline of stages."""
+    wl, xyz = _gen("cfg3", (1 << 21) + 5, w=1 << 16)
+    st = _check_all(cs, wl, xyz, k=2000, thresholds=(6,), budget=rows_fit * wl.w * 4)
+    assert st["scan_launches"] >= 1
+
+
+@pytest.mark.parametrize("budget_rows", [3, 5, 11])
+def test_budget_splits_scales(cs, budget_rows):
+    """4 scales x 5 rows: budget below one scale (staged per scale), one scale, two scales (scale groups)."""
+    wl, xyz = _gen("cfg5", 1 << 21, w=1 << 14)
+    _check_all(cs, wl, xyz, sample_p=0.25, k=500, thresholds=(4,), budget=budget_rows * wl.w * 4)
+
+
+def test_staged_scan_even_d_and_many_rows(cs):
+    from paper_1711_00975_b200 import synth
+    for d, fit in ((4, 1), (12, 5), (32, 3)):
+        wl = synth.Workload("st", N=60001, G=(700,), d=d, w=3001, k=300, H=32, f_bg=0.3, m_min=0, L=50.0, seed=d,
+                            gen_seed=d + 5)
+        _check_all(cs, wl, synth.generate(wl, device="cuda"), thresholds=(2,), probe_cells=256, budget=fit * wl.w * 4)
 
 
 # ---- randomised small configs and edge cases ------------------------------------------------------------------
