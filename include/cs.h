@@ -76,6 +76,13 @@ int cs_derive_coeffs(uint64_t seed, int d, uint64_t* out_4d, uint64_t* K_out);
 /* floor(sample_p * 2^64) as the sampler compares against (R13); 0 for p outside (0, 1). */
 uint64_t cs_sample_threshold(double sample_p);
 
+/* Host evaluation of the library's limb-split hash arithmetic -- the same inline functions the kernels compile
+ * (csrc/cs_hash.h) -- so that it can be checked against big-integer arithmetic without a GPU:
+ * *r_out = (a*c + b) mod (2^61-1), canonical, through the full-residue form; *low32_out = its low 32 bits through
+ * the short form the kernels use for power-of-two w and for the sign.  big = 0 selects the form compiled for
+ * meshes with G^3 <= 2^31 (needs c < 2^31), big = 1 the general one (c < 2^60).  1 <= a < p, b < p. */
+int cs_hash_cell(uint64_t a, uint64_t b, uint64_t c, int big, uint64_t* r_out, uint32_t* low32_out);
+
 /* ---- life cycle --------------------------------------------------------------------------------------- */
 
 /* cs_create: one sketch of d rows x w int32 counters over a G^3 mesh on a box of side L.

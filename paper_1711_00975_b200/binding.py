@@ -23,6 +23,7 @@ SIGNATURES = {
     "cs_last_error": (C.c_char_p, []),
     "cs_derive_coeffs": (ci, [u64, ci, vp, vp]),
     "cs_sample_threshold": (u64, [dbl]),
+    "cs_hash_cell": (ci, [u64, u64, u64, ci, vp, vp]),
     "cs_create": (ci, [vp, ci, u64, u32, dbl, u64]),
     "cs_create_multi": (ci, [vp, ci, ci, u64, vp, dbl, u64]),
     "cs_destroy": (ci, [vp]),
@@ -92,6 +93,13 @@ def derive_coeffs(seed: int, d: int):
     K = u64(0)
     _chk(lib().cs_derive_coeffs(seed, d, out.ctypes.data_as(vp), C.byref(K)), "cs_derive_coeffs")
     return out.reshape(d, 4), int(K.value)
+
+
+def hash_cell(a: int, b: int, c: int, big: bool = True):
+    """Host-only: ((a*c + b) mod (2^61-1), its low 32 bits) through the library's limb arithmetic (csrc/cs_hash.h)."""
+    r, lo = u64(0), u32(0)
+    _chk(lib().cs_hash_cell(a, b, c, int(big), C.byref(r), C.byref(lo)), "cs_hash_cell")
+    return int(r.value), int(lo.value)
 
 
 def sample_threshold(p: float) -> int:

@@ -19,7 +19,7 @@ CSRC = PKG / "csrc"
 OBJ = CSRC / "build"
 LIB = PKG / "libcs.so"
 SOURCES = ["cs_api.cu", "cs_kernels.cu", "cs_scan.cu", "cs_scan_staged.cu", "cs_select.cu", "cs_probe.cu"]
-HEADERS = ["cs_internal.h", "cs_device.cuh", "cs_launch.cuh", "cs_scan_common.cuh", "../../include/cs.h"]
+HEADERS = ["cs_internal.h", "cs_hash.h", "cs_device.cuh", "cs_launch.cuh", "cs_scan_common.cuh", "../../include/cs.h"]
 
 NVCC_FLAGS = [
     "-gencode", "arch=compute_100a,code=sm_100a",

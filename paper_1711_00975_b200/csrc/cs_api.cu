@@ -55,19 +55,6 @@ void derive_coeffs(uint64_t seed, int d, uint64_t* out_4d, uint64_t* K_out) {
     if (K_out) *K_out = stream_at(seed, 4 * (uint64_t)d + 1);
 }
 
-HashCoef split_coef(uint64_t a, uint64_t b) {
-    HashCoef k;
-    k.a0 = (uint32_t)(a & 0x7FFFFFFFu);
-    k.ah = (uint32_t)(a >> 31);
-    /* A = a * 2^32 mod p: a = x*2^29 + y (y < 2^29)  =>  a*2^32 = x*2^61 + y*2^32 == x + y*2^32 */
-    uint64_t A = (a >> 29) + ((a & 0x1FFFFFFFULL) << 32);
-    if (A >= P61) A -= P61;
-    k.A0 = (uint32_t)(A & 0x7FFFFFFFu);
-    k.Ah = (uint32_t)(A >> 31);
-    k.b = b;
-    return k;
-}
-
 uint64_t sample_threshold(double p) {
     if (!(p > 0.0) || !(p < 1.0)) return 0;
     return (uint64_t)std::floor(std::ldexp(p, 64));
@@ -542,6 +529,22 @@ int cs_derive_coeffs(uint64_t seed, int d, uint64_t* out_4d, uint64_t* K_out) {
 
 uint64_t cs_sample_threshold(double sample_p) { return sample_threshold(sample_p); }
 
+int cs_hash_cell(uint64_t a, uint64_t b, uint64_t c, int big, uint64_t* r_out, uint32_t* low32_out) {
+    if (!r_out || !low32_out) return fail(CS_ERR_ARG, "cs_hash_cell: null output");
+    if (a < 1 || a >= P61 || b >= P61) return fail(CS_ERR_ARG, "cs_hash_cell: a must be in [1, p-1], b in [0, p-1]");
+    if (c >= (1ull << 60) || (!big && c >= (1ull << 31)))
+        return fail(CS_ERR_ARG, "cs_hash_cell: c out of range for this form");
+    const HashCoef k = split_coef(a, b);
+    if (big) {
+        *r_out = affine_mod_p<true>(k, cell_c0(c), cell_c1(c));
+        *low32_out = affine_low32<true>(k, cell_c0(c), cell_c1(c));
+    } else {
+        *r_out = affine_mod_p<false>(k, cell_c0(c), 0);
+        *low32_out = affine_low32<false>(k, cell_c0(c), 0);
+    }
+    return CS_OK;
+}
+
 int cs_create_multi(cs_sketch** out, int n_scales, int d, uint64_t w, const uint32_t* G, double L, uint64_t seed) {
     if (!out) return fail(CS_ERR_ARG, "null output handle");
     *out = nullptr;
@@ -579,7 +582,7 @@ int cs_create_multi(cs_sketch** out, int n_scales, int d, uint64_t w, const uint
         P.sc[i].G = G[i];
         P.sc[i].qscale = (float)((double)G[i] / L);
         P.sc[i].top = (float)(G[i] - 1);
-        P.sc[i].big = cells > (1ull << 32) ? 1u : 0u;
+        P.sc[i].big = cells > (1ull << 31) ? 1u : 0u;
     }
     P.K = s->K;
 

@@ -1,6 +1,6 @@
 /*
  * cs_device.cuh -- device-side arithmetic of the Count-Sketch pass (sm_100a): quantise, sampling hash,
- * affine hashes mod 2^61-1 built from 32x32->64 multiplies, median of d.
+ * affine hashes mod 2^61-1 (cs_hash.h: 32x32->64 multiplies, word-aligned Mersenne folds), median of d.
  * Restates the arithmetic contract of include/cs.h; shares nothing with oracle/.
  */
 #ifndef CS_DEVICE_CUH_
@@ -42,24 +42,6 @@ __device__ __forceinline__ uint64_t mad_wide(uint32_t a, uint32_t b, uint64_t c)
     return (uint64_t)a * (uint64_t)b + c;     // IMAD.WIDE.U32
 }
 
-/* (a*c + b) mod (2^61-1), canonical residue, for c = c1*2^32 + c0 < 2^60.
- *   a*c + b == a*c0 + A*c1 + b (mod p)  with A = a*2^32 mod p,
- *   = hi*2^31 + lo,  lo = a0*c0 + A0*c1 + b < 2^64,  hi = ah*c0 + Ah*c1 < 2^63,
- *   hi*2^31 = (hi>>30)*2^61 + (hi & (2^30-1))*2^31 == (hi>>30) + (hi & (2^30-1))*2^31   (2^61 == 1). */
-template <bool BIG>
-__device__ __forceinline__ uint64_t affine_mod_p(const HashCoef& k, uint32_t c0, uint32_t c1) {
-    uint64_t lo = mad_wide(k.a0, c0, k.b);
-    uint64_t hi = (uint64_t)k.ah * (uint64_t)c0;
-    if (BIG) {
-        lo = mad_wide(k.A0, c1, lo);
-        hi = mad_wide(k.Ah, c1, hi);
-    }
-    uint64_t r = (hi >> 30) + ((hi & 0x3FFFFFFFULL) << 31) + (lo & P61) + (lo >> 61);   // < 2^62 + 2^34
-    r = (r & P61) + (r >> 61);                                                           // <= p + 2
-    r = (r + ((r + 1) >> 61)) & P61;                                                     // r >= p -> r - p
-    return r;
-}
-
 /* General form for any 64-bit c (used when a caller-supplied cell id is >= 2^60): 128-bit product through
  * __umul64hi, 2^64 == 8 (mod p). */
 __device__ __forceinline__ uint64_t affine_mod_p_wide(uint64_t a, uint64_t b, uint64_t c) {
@@ -71,16 +53,13 @@ __device__ __forceinline__ uint64_t affine_mod_p_wide(uint64_t a, uint64_t b, ui
     return r;
 }
 
-__device__ __forceinline__ uint64_t coef_a(const HashCoef& k) { return ((uint64_t)k.ah << 31) | k.a0; }
-
 /* Bucket index and sign of row `rc` for cell c. */
 template <bool BIG, bool POW2>
 __device__ __forceinline__ void bucket_sign(const RowCoef& rc, uint32_t c0, uint32_t c1, uint64_t w,
                                             uint32_t& bucket, int32_t& sign) {
-    uint64_t r = affine_mod_p<BIG>(rc.h, c0, c1);
-    bucket = POW2 ? ((uint32_t)r & (uint32_t)(w - 1)) : (uint32_t)(r % w);
-    uint64_t r2 = affine_mod_p<BIG>(rc.s, c0, c1);
-    sign = 1 - 2 * (int32_t)((uint32_t)r2 & 1u);
+    if (POW2) bucket = affine_low32<BIG>(rc.h, c0, c1) & (uint32_t)(w - 1);     // w <= 2^31
+    else      bucket = (uint32_t)(affine_mod_p<BIG>(rc.h, c0, c1) % w);
+    sign = 1 - 2 * (int32_t)(affine_low32<BIG>(rc.s, c0, c1) & 1u);
 }
 
 __device__ __forceinline__ int32_t mul_sign(int32_t t, int32_t sign) {

@@ -9,19 +9,11 @@
 #include <stdint.h>
 
 #include "../../include/cs.h"
+#include "cs_hash.h"
 
 namespace cs {
 
-constexpr uint64_t P61 = (1ULL << 61) - 1;            // Mersenne prime 2^61 - 1
 constexpr uint64_t GAMMA = 0x9E3779B97F4A7C15ULL;     // splitmix64 increment
-
-/* One affine hash x -> (a*x + b) mod p, pre-split on the host for 32-bit multiplies:
- * a = ah*2^31 + a0 (a0 < 2^31, ah < 2^30) multiplies the low 32 bits of the cell id;
- * A = (a * 2^32) mod p = Ah*2^31 + A0 multiplies the high bits (cell ids >= 2^32 only). */
-struct HashCoef {
-    uint32_t a0, ah, A0, Ah;
-    uint64_t b;
-};
 
 struct RowCoef {
     HashCoef h;   // bucket hash
@@ -33,7 +25,7 @@ struct ScaleParams {
     float qscale;      // (float)((double)G / L)
     float top;         // (float)(G - 1)
     uint32_t G;
-    uint32_t big;      // 1 if G^3 > 2^32 (cell ids need the high-word multiplies)
+    uint32_t big;      // 1 if G^3 > 2^31 (cell ids need the c1 multiplies, cs_hash.h)
 };
 
 /* Per-scale candidate collection state, in device memory, mirrored to pinned host memory after each chunk. */

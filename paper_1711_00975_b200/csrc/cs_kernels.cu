@@ -19,7 +19,7 @@ namespace cs {
 template <int D, bool POW2, bool BIG>
 __device__ __forceinline__ void add_rows(const PassParams& P, int s, uint64_t c) {
     const int d = D ? D : P.d;
-    const uint32_t c0 = (uint32_t)c, c1 = (uint32_t)(c >> 32);
+    const uint32_t c0 = cell_c0(c), c1 = cell_c1(c);
     int32_t* T = P.sc[s].T;
     const RowCoef* rows = &P.rows[s * d];
 #pragma unroll

@@ -32,7 +32,7 @@ template <int D, bool POW2, bool BIG>
 __device__ __forceinline__ bool estimate_ge(const PassParams& P, int s, uint64_t c, int32_t tau, int32_t& est) {
     const int d = D ? D : P.d;
     const int max_fail = (d - 1) / 2;            // est >= tau  <=>  at most (d-1)/2 row values are < tau
-    const uint32_t c0 = (uint32_t)c, c1 = (uint32_t)(c >> 32);
+    const uint32_t c0 = cell_c0(c), c1 = cell_c1(c);
     const int32_t* T = P.sc[s].T;
     const RowCoef* rows = &P.rows[s * d];
     int32_t v[D ? D : CS_MAX_ROWS];
@@ -84,14 +84,14 @@ __device__ __forceinline__ void append_candidate(const ScanTarget& tg, bool emit
 /* Estimate of an arbitrary caller-supplied 64-bit cell id (any value: ids >= 2^60 take the __umul64hi form). */
 template <int D, bool POW2>
 __device__ __forceinline__ int32_t estimate_any(const PassParams& P, int s, uint64_t c) {
-    if ((c >> 32) == 0) return estimate_full<D, POW2, false>(P, s, c);
+    if ((c >> 31) == 0) return estimate_full<D, POW2, false>(P, s, c);
     if ((c >> 60) == 0) return estimate_full<D, POW2, true>(P, s, c);
     const int d = D ? D : P.d;
     int32_t v[CS_MAX_ROWS];
     for (int j = 0; j < d; ++j) {
         const RowCoef& rc = P.rows[s * d + j];
-        uint64_t r = affine_mod_p_wide(coef_a(rc.h), rc.h.b, c);
-        uint64_t r2 = affine_mod_p_wide(coef_a(rc.s), rc.s.b, c);
+        uint64_t r = affine_mod_p_wide(coef_a(rc.h), coef_b(rc.h), c);
+        uint64_t r2 = affine_mod_p_wide(coef_a(rc.s), coef_b(rc.s), c);
         uint32_t b = POW2 ? ((uint32_t)r & (uint32_t)(P.w - 1)) : (uint32_t)(r % P.w);
         v[j] = mul_sign(ld_table(P.sc[s].T + (uint64_t)j * P.w + b), 1 - 2 * (int32_t)((uint32_t)r2 & 1u));
     }

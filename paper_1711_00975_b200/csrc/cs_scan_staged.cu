@@ -36,7 +36,7 @@ struct StageParams {
 template <int R, bool POW2, bool BIG>
 __device__ __forceinline__ int stage_rows(const PassParams& P, int row0, uint64_t c, int32_t tau, int fails,
                                           int max_fail) {
-    const uint32_t c0 = (uint32_t)c, c1 = (uint32_t)(c >> 32);
+    const uint32_t c0 = cell_c0(c), c1 = cell_c1(c);
     const int32_t* T = P.sc[0].T;
 #pragma unroll
     for (int j = 0; j < R; ++j) {
@@ -50,7 +50,7 @@ __device__ __forceinline__ int stage_rows(const PassParams& P, int row0, uint64_
 
 template <bool POW2, bool BIG>
 __device__ __noinline__ int32_t estimate_all_rows(const PassParams& P, int d, uint64_t c) {
-    const uint32_t c0 = (uint32_t)c, c1 = (uint32_t)(c >> 32);
+    const uint32_t c0 = cell_c0(c), c1 = cell_c1(c);
     int32_t v[CS_MAX_ROWS];
     for (int j = 0; j < d; ++j) v[j] = row_value<BIG, POW2>(P, P.sc[0].T, P.rows[j], j, c0, c1);
     return median_rt(v, d);

@@ -124,3 +124,44 @@ def test_binding_fails_loudly_without_library(monkeypatch, tmp_path):
     monkeypatch.setattr(binding, "LIB_PATH", tmp_path / "libcs.so")
     with pytest.raises(RuntimeError, match="no CPU fallback"):
         binding.lib()
+
+
+def test_limb_hash_arithmetic_against_big_integers(cslib, golden):
+    """csrc/cs_hash.h (the inline functions the kernels compile), evaluated on the host through cs_hash_cell,
+    against Python big integers: closed forms, residues that land on 0 / p-1 / the fold carries, random values."""
+    from paper_1711_00975_b200 import binding
+    rng = np.random.default_rng(20260)
+    cases = []
+    # closed forms of tests/golden (2^61 == 1): (a, c, b) -> r
+    for case in golden["mersenne"]["cases"]:
+        a, c, b, want = (int(eval(case[key], {"p": P61})) for key in ("a", "c", "b", "r"))
+        assert binding.hash_cell(a, b, c, big=True) == (want, want & 0xFFFFFFFF), case
+        cases.append((a, b, c))
+    edge_a = [1, 2, P61 - 1, P61 - 2, 2 ** 32 - 1, 2 ** 32, 2 ** 32 + 1, 2 ** 60, 2 ** 60 + 1, 2 ** 61 - 2 ** 32 - 1,
+              (2 ** 29 - 1) << 32 | 0xFFFFFFFE]
+    edge_b = [0, 1, P61 - 1, P61 - 5, 2 ** 32 - 1, 2 ** 32, 2 ** 60]
+    edge_c = [0, 1, 5, 2 ** 31 - 1, 2 ** 31, 2 ** 31 + 1, 2 ** 32 - 1, 2 ** 32, 2 ** 36 - 1, 2 ** 37, 2 ** 60 - 1,
+              4095 + 4096 * (4095 + 4096 * 4095), 4641 + 4642 * (4641 + 4642 * 4641)]
+    for a in edge_a:
+        for b in edge_b:
+            for c in edge_c:
+                cases.append((a, b, c))
+    # residues forced to 0, p-1, 1: choose b = (target - a*c) mod p
+    for _ in range(300):
+        a = int(rng.integers(1, P61)); c = int(rng.integers(0, 2 ** 60))
+        for target in (0, P61 - 1, 1, 2 ** 32 - 1, 2 ** 32):
+            cases.append((a, (target - a * c) % P61, c))
+    for _ in range(20000):
+        bits = int(rng.integers(1, 61))
+        cases.append((int(rng.integers(1, P61)), int(rng.integers(0, P61)), int(rng.integers(0, 2 ** bits))))
+    for a, b, c in cases:
+        want = (a * c + b) % P61
+        r, lo = binding.hash_cell(a, b, c, big=True)
+        assert r == want and lo == want & 0xFFFFFFFF, (a, b, c)
+        if c < 2 ** 31:
+            r, lo = binding.hash_cell(a, b, c, big=False)
+            assert r == want and lo == want & 0xFFFFFFFF, (a, b, c, "small form")
+    assert cslib.cs_hash_cell(0, 0, 0, 1, None, None) == binding.CS_ERR_ARG
+    r, lo = C.c_uint64(0), C.c_uint32(0)
+    assert cslib.cs_hash_cell(1, 0, 2 ** 31, 0, C.byref(r), C.byref(lo)) == binding.CS_ERR_ARG
+    assert cslib.cs_hash_cell(P61, 0, 1, 1, C.byref(r), C.byref(lo)) == binding.CS_ERR_ARG
