@@ -106,6 +106,14 @@ int cs_set_stream(cs_sketch* s, void* cuda_stream);
  * that the red.global.add traffic of each pass stays L2-resident.  The result does not depend on it. */
 int cs_set_table_budget(cs_sketch* s, uint64_t bytes);
 
+/* How cs_update applies the counter updates.  The result never depends on it.
+ *   mode 1 "direct": one red.global.add.s32 per (particle, row) into L2-resident row groups (table budget above).
+ *   mode 2 "binned": updates are first written as 2-byte records partitioned by table slice, then applied slice by
+ *           slice in shared memory (csrc/cs_update_binned.cu); needs w a power of two in [2^8, 2^25], else falls
+ *           back to direct.  rows_direct rows of every binned pass still take the direct route (0 = none).
+ *   mode 0 "auto" (default): binned for calls of at least 2^22 particles when the shape allows it. */
+int cs_set_update_mode(cs_sketch* s, int mode, int rows_direct);
+
 /* Running particle index of the update stream / of the current scan (sampling, R13, R17).
  * Setting it lets a stream shard (multi-GPU) reproduce the single-stream sampling decisions. */
 int cs_set_update_index(cs_sketch* s, uint64_t index);

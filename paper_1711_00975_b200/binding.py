@@ -30,6 +30,7 @@ SIGNATURES = {
     "cs_reset": (ci, [vp]),
     "cs_set_stream": (ci, [vp, vp]),
     "cs_set_table_budget": (ci, [vp, u64]),
+    "cs_set_update_mode": (ci, [vp, ci, ci]),
     "cs_set_update_index": (ci, [vp, u64]),
     "cs_set_scan_index": (ci, [vp, u64]),
     "cs_get_update_index": (ci, [vp, vp]),
@@ -153,6 +154,9 @@ class CountSketch:
 
     def set_table_budget(self, nbytes: int):
         _chk(lib().cs_set_table_budget(self._h, nbytes), "cs_set_table_budget")
+
+    def set_update_mode(self, mode: int, rows_direct: int = 0):
+        _chk(lib().cs_set_update_mode(self._h, mode, rows_direct), "cs_set_update_mode")
 
     def set_update_index(self, index: int):
         _chk(lib().cs_set_update_index(self._h, index), "cs_set_update_index")

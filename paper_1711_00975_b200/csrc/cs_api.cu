@@ -108,6 +108,13 @@ struct cs_sketch {
     int32_t* out_est = nullptr;
     uint64_t out_cap = 0;
 
+    /* binned update (cs_update_binned.cu) */
+    int update_mode = 0;               /* cs_set_update_mode: 0 auto, 1 direct red.global, 2 binned */
+    int bin_rows_direct = 0;           /* rows of each binned pass that still go through red.global */
+    uint16_t* bins = nullptr;          /* record regions */
+    uint64_t bins_records = 0;         /* capacity of `bins` in records */
+    uint32_t* cursor = nullptr;        /* BIN_MAX words */
+
     /* survivor lists of the row-partitioned scan */
     StageBuffers stb = {};
 
@@ -212,12 +219,94 @@ PassParams pass_params(const cs_sketch* s, uint64_t index0, double sample_p) {
 
 bool bad_p(double p) { return !(p > 0.0) || p > 1.0; }
 
+/* ---- binned update: plan + passes (kernels in cs_update_binned.cu) -------------------- */
+
+constexpr uint32_t BIN_MAX = 4096;                    /* bins per pass (words of `cursor`) */
+constexpr uint64_t BIN_CHUNK = 1ull << 27;            /* particles per scatter/apply pair */
+constexpr uint64_t BIN_MIN_N = 1ull << 22;            /* auto mode: below this the direct kernel is as fast */
+constexpr size_t BIN_SMEM = 200 * 1024;               /* shared memory of one scatter CTA */
+
+struct BinPlan {
+    uint32_t log2w, log2S, SL, C;
+    int rows_per_pass;
+};
+
+int ilog2(uint64_t v) { return bit_length(v) - 1; }
+
+/* false: this shape cannot be binned (w not a power of two, too small or too wide): use the direct kernel */
+bool bin_plan(const cs_sketch* s, BinPlan* pl) {
+    const uint64_t w = s->w;
+    if (w & (w - 1)) return false;
+    const int lw = ilog2(w);
+    if (lw < 8 || lw > 25) return false;
+    int lS = lw - 7;                                   /* 128 slices per row ... */
+    if (lS < 8) lS = 8;
+    if (lS > 15) lS = 15;                              /* ... of at most 2^15 counters (128 KB, 15-bit offsets) */
+    if (lS > lw) lS = lw;
+    const uint32_t SL = (uint32_t)(w >> lS);
+    const double lambda = 2048.0 / SL;                 /* records per bin, round and CTA (1024 threads x 2 particles) */
+    uint32_t C = (uint32_t)(32.0 + lambda + 6.0 * std::sqrt(lambda) + 8.0);
+    C = (C + 7u) & ~7u;
+    if (C > 256) C = 256;                              /* beyond: staging overflows go through red.global */
+    int rows = 0;
+    for (int r = 1; r <= 8 && r <= s->d; ++r)
+        if ((uint64_t)r * SL <= BIN_MAX && scatter_smem_bytes(r * SL, C) <= BIN_SMEM) rows = r;
+    if (!rows) return false;
+    pl->log2w = (uint32_t)lw; pl->log2S = (uint32_t)lS; pl->SL = SL; pl->C = C; pl->rows_per_pass = rows;
+    return true;
+}
+
+int update_binned(cs_sketch* s, const BinPlan& pl, const float* xyz, uint64_t n, uint64_t index0, double sample_p) {
+    const PassParams full = pass_params(s, index0, sample_p);
+    const int groups = (s->d + pl.rows_per_pass - 1) / pl.rows_per_pass;
+    const int each = (s->d + groups - 1) / groups;                       /* balanced row groups */
+    const uint64_t chunk_max = n < BIN_CHUNK ? n : BIN_CHUNK;
+    const double keep = sample_p < 1.0 ? sample_p : 1.0;
+    uint64_t cap = (uint64_t)((double)chunk_max * keep / pl.SL * 1.04) + 2048;
+    cap = (cap + 31) & ~(uint64_t)31;
+    const uint64_t need = cap * each * pl.SL;
+    if (!s->cursor) CS_CUDA(cudaMalloc(&s->cursor, BIN_MAX * sizeof(uint32_t)));
+    if (s->bins_records < need) {
+        CS_CUDA(cudaStreamSynchronize(s->stream));
+        if (s->bins) cudaFree(s->bins);
+        s->bins = nullptr; s->bins_records = 0;
+        CS_CUDA(cudaMalloc(&s->bins, need * sizeof(uint16_t)));
+        s->bins_records = need;
+    }
+    for (uint64_t off = 0; off < n; off += BIN_CHUNK) {
+        uint64_t m = n - off < BIN_CHUNK ? n - off : BIN_CHUNK;
+        for (int i = 0; i < s->n_scales; ++i)
+            for (int j0 = 0; j0 < s->d; j0 += each) {
+                const int nr = j0 + each <= s->d ? each : s->d - j0;
+                PassParams P = full;
+                P.index0 = index0 + off;
+                P.n_scales = 1;
+                P.d = nr;
+                P.sc[0] = full.sc[i];
+                P.sc[0].T = full.sc[i].T + (uint64_t)j0 * s->w;
+                for (int j = 0; j < nr; ++j) P.rows[j] = full.rows[i * s->d + j0 + j];
+                BinParams B;
+                B.bins = s->bins; B.cursor = s->cursor; B.cap = (uint32_t)cap;
+                B.nb = (uint32_t)nr * pl.SL; B.C = pl.C; B.log2S = pl.log2S; B.log2w = pl.log2w;
+                B.rows_direct = s->bin_rows_direct < nr ? s->bin_rows_direct : nr;
+                CS_CUDA(cudaMemsetAsync(s->cursor, 0, B.nb * sizeof(uint32_t), s->stream));
+                cudaError_t e = launch_update_binned(P, B, xyz + 3 * off, m, s->sm_count, s->stream);
+                if (e != cudaSuccess) return fail(CS_ERR_CUDA, "binned update kernels: %s", cudaGetErrorString(e));
+                s->launches += B.rows_direct < nr ? 2 : 1;
+            }
+    }
+    return CS_OK;
+}
+
 /* Row-partitioned update: red.global.add runs at its L2 rate only while the counters a
  * pass touches stay L2-resident (measured: ~194 G/s up to ~56 MiB, 107 G/s at 112 MiB, 25 G/s at 448 MiB), so
  * the d rows of each scale are split into groups of at most table_budget bytes and the positions are re-read
  * once per group (12 B/particle at HBM rate, far cheaper than DRAM-backed atomics).  Each group is the same
  * kernel with a PassParams that names only that group's rows and tables. */
 int update_passes(cs_sketch* s, const float* xyz, uint64_t n, uint64_t index0, double sample_p) {
+    BinPlan pl;
+    if (s->update_mode != 1 && (s->update_mode == 2 || n >= BIN_MIN_N) && bin_plan(s, &pl))
+        return update_binned(s, pl, xyz, n, index0, sample_p);
     const PassParams full = pass_params(s, index0, sample_p);
     const uint64_t row_bytes = s->w * sizeof(int32_t);
     const uint64_t all_bytes = row_bytes * s->d * s->n_scales;
@@ -615,6 +704,8 @@ int cs_destroy(cs_sketch* s) {
     if (s->copy_stream) cudaStreamSynchronize(s->copy_stream);
     free_candidates(s);
     free_stage_lists(s);
+    if (s->bins) cudaFree(s->bins);
+    if (s->cursor) cudaFree(s->cursor);
     for (int i = 0; i < CS_MAX_SCALES; ++i) if (s->T[i]) cudaFree(s->T[i]);
     if (s->st_dev) cudaFree(s->st_dev);
     if (s->st_host) cudaFreeHost(s->st_host);
@@ -653,6 +744,15 @@ int cs_set_table_budget(cs_sketch* s, uint64_t bytes) {
     if (!s) return fail(CS_ERR_ARG, "null handle");
     if (bytes < 4) return fail(CS_ERR_ARG, "budget must be at least one counter");
     s->table_budget = bytes;
+    return CS_OK;
+}
+
+int cs_set_update_mode(cs_sketch* s, int mode, int rows_direct) {
+    if (!s) return fail(CS_ERR_ARG, "null handle");
+    if (mode < 0 || mode > 2 || rows_direct < 0 || rows_direct > CS_MAX_ROWS)
+        return fail(CS_ERR_ARG, "mode must be 0 (auto), 1 (direct) or 2 (binned); rows_direct in [0, 32]");
+    s->update_mode = mode;
+    s->bin_rows_direct = rows_direct;
     return CS_OK;
 }
 

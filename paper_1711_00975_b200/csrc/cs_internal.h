@@ -65,6 +65,22 @@ struct ScanParams {
     ScanTarget tg[CS_MAX_SCALES];
 };
 
+/* Binned update (cs_update_binned.cu): the rows of one pass are cut into slices of 2^log2S counters; bin =
+ * (row, slice) = counter index >> log2S; a record is (offset in slice) << 1 | sign bit, 2 bytes. */
+struct BinParams {
+    uint16_t* bins;       // nb regions of `cap` records each
+    uint32_t* cursor;     // records reserved per bin (zeroed before each pass)
+    uint32_t cap;         // records per bin region, a multiple of 32
+    uint32_t nb;          // bins of this pass = rows << (log2w - log2S)
+    uint32_t C;           // records per shared-memory staging buffer, a multiple of 8
+    uint32_t log2S;       // <= 15
+    uint32_t log2w;
+    int32_t rows_direct;  // the first rows_direct rows of the pass use red.global instead of the bins
+};
+size_t scatter_smem_bytes(uint32_t nb, uint32_t C);
+cudaError_t launch_update_binned(const PassParams& P, const BinParams& B, const float* xyz, uint64_t n, int sm_count,
+                                 cudaStream_t st);
+
 /* kernel launchers (cs_kernels.cu) */
 cudaError_t launch_update(const PassParams& P, const float* xyz, uint64_t n, int sm_count, cudaStream_t st);
 cudaError_t launch_scan(const PassParams& P, const ScanParams& S, const float* xyz, uint64_t n, int sm_count,

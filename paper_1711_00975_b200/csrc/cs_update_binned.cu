@@ -1,0 +1,274 @@
+/*
+ * cs_update_binned.cu -- the Add pass (T[j][h_j(c)] += s_j(c)) without one L2 atomic per
+ * counter update.
+ *
+ * Why: red.global.add.s32 at random addresses is bounded by the L2 tag-lookup rate (measured ~194 G/s chip-wide,
+ * ncu: lts__t_tag_requests at ~78 % of peak, half of the requests cross the die fabric), i.e. ~39 ms for the
+ * 7.5e9 updates of cfg 3, while shared-memory atomics run at ~2250 G/s.  So the updates are first partitioned
+ * by table slice and then applied slice by slice in shared memory:
+ *
+ *   k_bin_scatter   positions -> quantise -> (sample) -> 2R hashes -> one 2-byte record per (particle, row):
+ *                   record = (offset within slice) << 1 | (sign bit);  bin = (row, slice).  Each CTA keeps a
+ *                   small staging buffer per bin in shared memory; a bin that has collected 32 records is
+ *                   written out as one 64-byte unit to the bin's region in HBM (space reserved with one global
+ *                   atomic per unit).  Records that do not fit (a staging buffer or a bin region is full:
+ *                   heavily duplicated streams) are applied directly with red.global -- int32 adds commute,
+ *                   so the table is the same whichever way a record travels.
+ *   k_bin_apply     one CTA per bin: zero a slice of counters in shared memory, stream the bin's records
+ *                   (16-byte loads, 8 records each), atomicAdd into shared memory, then T[slice] += it
+ *                   with plain coalesced loads/stores (the CTA owns the slice during this kernel).
+ *
+ * HBM traffic per particle and row: 2 B written + 2 B read, plus 12 B per particle per pass for the positions.
+ */
+#include "cs_device.cuh"
+#include "cs_launch.cuh"
+
+namespace cs {
+
+constexpr int BIN_THREADS = 1024;
+constexpr uint32_t UNIT = 32;            // records per flush unit (64 bytes)
+
+__device__ __forceinline__ float2 ld_stream8(const float2* p) {
+    float2 v;
+    asm volatile("ld.global.cs.v2.f32 {%0, %1}, [%2];" : "=f"(v.x), "=f"(v.y) : "l"(p));
+    return v;
+}
+__device__ __forceinline__ uint4 ld_stream16u(const uint4* p) {
+    uint4 v;
+    asm volatile("ld.global.cs.v4.u32 {%0, %1, %2, %3}, [%4];" : "=r"(v.x), "=r"(v.y), "=r"(v.z), "=r"(v.w) : "l"(p));
+    return v;
+}
+
+/* Shared-memory layout of k_bin_scatter (dynamic): cnt[NB] | qlen[2] | pad | queue[NB] (u16) | buf[NB*C] (u16) */
+struct ScatterSmem {
+    uint32_t* cnt;
+    uint32_t* qlen;
+    uint16_t* queue;
+    uint16_t* buf;
+};
+__host__ __device__ inline size_t smem_off_queue(uint32_t nb) { return (((size_t)nb + 2) * 4 + 15) & ~(size_t)15; }
+__host__ __device__ inline size_t smem_off_buf(uint32_t nb) { return (smem_off_queue(nb) + (size_t)nb * 2 + 15) & ~(size_t)15; }
+size_t scatter_smem_bytes(uint32_t nb, uint32_t C) { return smem_off_buf(nb) + (size_t)nb * C * 2; }
+
+/* Apply one record directly (fallback path and the partial buffers at the end of the kernel). */
+__device__ __forceinline__ void apply_direct(int32_t* T, uint32_t bin, uint32_t log2S, uint32_t rec) {
+    red_add(T + (((uint64_t)bin << log2S) | (rec >> 1)), 1 - 2 * (int32_t)(rec & 1u));
+}
+
+template <int R, bool BIG>
+__device__ __forceinline__ void bin_particle(const PassParams& P, const BinParams& B, const ScatterSmem& S,
+                                             uint32_t qsel, float x, float y, float z) {
+    const uint64_t c = cell_of(x, y, z, P.sc[0]);
+    const uint32_t c0 = cell_c0(c), c1 = cell_c1(c);
+    int32_t* T = P.sc[0].T;
+    const uint32_t wmask = (uint32_t)(P.w - 1);
+#pragma unroll
+    for (int j = 0; j < R; ++j) {
+        const uint32_t h = affine_low32<BIG>(P.rows[j].h, c0, c1) & wmask;
+        const uint32_t sb = affine_low32<BIG>(P.rows[j].s, c0, c1) & 1u;
+        const uint32_t key = ((uint32_t)j << B.log2w) | h;             // counter index within this pass's rows
+        if (j < B.rows_direct) {
+            red_add(T + key, 1 - 2 * (int32_t)sb);
+            continue;
+        }
+        const uint32_t bin = key >> B.log2S;
+        const uint32_t rec = ((key & ((1u << B.log2S) - 1u)) << 1) | sb;
+        const uint32_t slot = atomicAdd(&S.cnt[bin], 1u);
+        if (slot < B.C) {
+            S.buf[bin * B.C + slot] = (uint16_t)rec;
+            if (slot == UNIT - 1) S.queue[atomicAdd(&S.qlen[qsel], 1u)] = (uint16_t)bin;
+        } else {
+            red_add(T + key, 1 - 2 * (int32_t)sb);                     // staging buffer full: apply directly
+        }
+    }
+}
+
+/* Particles [head, head + 2*pairs) are read as pairs (3 x 8 B per thread, 8-byte aligned); the <= 1 particle
+ * before and the <= 1 after are applied directly by block 0. */
+template <int R, bool BIG>
+__global__ void __launch_bounds__(BIN_THREADS, 1)
+k_bin_scatter(const __grid_constant__ PassParams P, const __grid_constant__ BinParams B,
+              const float* __restrict__ xyz, uint64_t n, uint32_t head, uint64_t pairs) {
+    extern __shared__ __align__(16) unsigned char smem_raw[];
+    ScatterSmem S;
+    S.cnt = reinterpret_cast<uint32_t*>(smem_raw);
+    S.qlen = S.cnt + B.nb;
+    S.queue = reinterpret_cast<uint16_t*>(smem_raw + smem_off_queue(B.nb));
+    S.buf = reinterpret_cast<uint16_t*>(smem_raw + smem_off_buf(B.nb));
+    for (uint32_t i = threadIdx.x; i < B.nb + 2; i += BIN_THREADS) S.cnt[i] = 0;       // cnt and qlen[0..1]
+    __syncthreads();
+
+    const float2* body = reinterpret_cast<const float2*>(xyz + 3 * (uint64_t)head);
+    const uint64_t per_round = (uint64_t)gridDim.x * BIN_THREADS;
+    const uint64_t rounds = (pairs + per_round - 1) / per_round;
+    const uint32_t lane = threadIdx.x & 31u, warp = threadIdx.x >> 5;
+    const uint32_t grp = lane >> 2, l4 = lane & 3u;
+    const uint32_t gmask = 0xFu << (grp * 4);
+    int32_t* T = P.sc[0].T;
+
+    for (uint64_t r = 0; r < rounds; ++r) {
+        const uint32_t qsel = (uint32_t)(r & 1);
+        const uint64_t g = r * per_round + (uint64_t)blockIdx.x * BIN_THREADS + threadIdx.x;
+        if (g < pairs) {
+            const float2 q0 = ld_stream8(body + 3 * g);
+            const float2 q1 = ld_stream8(body + 3 * g + 1);
+            const float2 q2 = ld_stream8(body + 3 * g + 2);
+            const uint64_t i0 = P.index0 + head + 2 * g;
+            if (!P.sample || keep_particle(P.K, i0, P.Tp)) bin_particle<R, BIG>(P, B, S, qsel, q0.x, q0.y, q1.x);
+            if (!P.sample || keep_particle(P.K, i0 + 1, P.Tp)) bin_particle<R, BIG>(P, B, S, qsel, q1.y, q2.x, q2.y);
+        }
+        __syncthreads();
+        /* flush every bin that completed a unit in this round: groups of 4 lanes, one bin each */
+        const uint32_t nq = S.qlen[qsel];
+        if (threadIdx.x == 0) S.qlen[qsel ^ 1] = 0;                   // not in use until after the next barrier
+        for (uint32_t e0 = warp * 8; e0 < nq; e0 += (BIN_THREADS / 32) * 8) {
+            const uint32_t e = e0 + grp;
+            const bool on = e < nq;
+            uint32_t bin = 0, c = 0, units = 0, base = 0;
+            if (on) {
+                bin = S.queue[e];
+                c = min(S.cnt[bin], B.C);
+                units = c / UNIT;
+                if (l4 == 0) base = atomicAdd(&B.cursor[bin], units * UNIT);
+            }
+            base = __shfl_sync(0xFFFFFFFFu, base, grp * 4);
+            if (on) {
+                const uint16_t* src = S.buf + bin * B.C;
+                for (uint32_t u = 0; u < units; ++u) {
+                    const uint4 v = *reinterpret_cast<const uint4*>(src + u * UNIT + l4 * 8);
+                    const uint32_t at = base + u * UNIT;
+                    if (at + UNIT <= B.cap) {
+                        *reinterpret_cast<uint4*>(B.bins + (uint64_t)bin * B.cap + at + l4 * 8) = v;
+                    } else {                                           // bin region full: apply directly
+                        const uint32_t wds[4] = {v.x, v.y, v.z, v.w};
+#pragma unroll
+                        for (int k = 0; k < 4; ++k) {
+                            apply_direct(T, bin, B.log2S, wds[k] & 0xFFFFu);
+                            apply_direct(T, bin, B.log2S, wds[k] >> 16);
+                        }
+                    }
+                }
+                /* move the < 32 leftover records to the front (source and destination do not overlap) */
+                const uint32_t left = c - units * UNIT;
+                uint16_t tmp[8];
+#pragma unroll
+                for (int k = 0; k < 8; ++k) {
+                    const uint32_t i = l4 * 8 + k;
+                    tmp[k] = i < left ? src[units * UNIT + i] : (uint16_t)0;
+                }
+                __syncwarp(gmask);
+#pragma unroll
+                for (int k = 0; k < 8; ++k) {
+                    const uint32_t i = l4 * 8 + k;
+                    if (i < left) S.buf[bin * B.C + i] = tmp[k];
+                }
+                if (l4 == 0) S.cnt[bin] = left;
+            }
+        }
+        __syncthreads();
+    }
+    /* partial buffers (< 32 records per bin): applied directly */
+    for (uint32_t bin = threadIdx.x; bin < B.nb; bin += BIN_THREADS) {
+        const uint32_t c = min(S.cnt[bin], B.C);
+        for (uint32_t i = 0; i < c; ++i) apply_direct(T, bin, B.log2S, S.buf[bin * B.C + i]);
+    }
+    if (blockIdx.x == 0 && threadIdx.x < 2) {
+        const uint64_t tail0 = (uint64_t)head + 2 * pairs;
+        uint64_t i = ~0ull;
+        if (threadIdx.x == 0 && head) i = 0;
+        if (threadIdx.x == 1 && tail0 < n) i = tail0;
+        if (i != ~0ull && (!P.sample || keep_particle(P.K, P.index0 + i, P.Tp))) {
+            const float* p = xyz + 3 * i;
+            const uint64_t c = cell_of(ld_stream4(p), ld_stream4(p + 1), ld_stream4(p + 2), P.sc[0]);
+            const uint32_t c0 = cell_c0(c), c1 = cell_c1(c);
+            for (int j = 0; j < R; ++j) {
+                uint32_t b;
+                int32_t sg;
+                bucket_sign<BIG, true>(P.rows[j], c0, c1, P.w, b, sg);
+                red_add(T + (uint64_t)j * P.w + b, sg);
+            }
+        }
+    }
+}
+
+/* One CTA per bin. */
+__global__ void __launch_bounds__(BIN_THREADS, 1)
+k_bin_apply(int32_t* __restrict__ T, const uint16_t* __restrict__ bins, const uint32_t* __restrict__ cursor,
+            uint32_t cap, uint32_t log2S) {
+    extern __shared__ __align__(16) int32_t acc[];
+    const uint32_t S = 1u << log2S;
+    const uint32_t bin = blockIdx.x;
+    for (uint32_t i = threadIdx.x; i < S; i += BIN_THREADS) acc[i] = 0;
+    __syncthreads();
+    const uint32_t len = min(cursor[bin], cap);                        // a multiple of UNIT
+    const uint4* src = reinterpret_cast<const uint4*>(bins + (uint64_t)bin * cap);
+    const uint32_t nvec = len / 8;
+    for (uint32_t v = threadIdx.x; v < nvec; v += BIN_THREADS) {
+        const uint4 q = ld_stream16u(src + v);
+        const uint32_t wds[4] = {q.x, q.y, q.z, q.w};
+#pragma unroll
+        for (int k = 0; k < 4; ++k) {
+            const uint32_t lo = wds[k] & 0xFFFFu, hi = wds[k] >> 16;
+            atomicAdd(&acc[lo >> 1], 1 - 2 * (int32_t)(lo & 1u));
+            atomicAdd(&acc[hi >> 1], 1 - 2 * (int32_t)(hi & 1u));
+        }
+    }
+    __syncthreads();
+    int32_t* dst = T + ((uint64_t)bin << log2S);
+    for (uint32_t i = threadIdx.x; i < S; i += BIN_THREADS) {
+        const int32_t a = acc[i];
+        if (a) dst[i] = (int32_t)((uint32_t)dst[i] + (uint32_t)a);
+    }
+}
+
+/* ---- host side ------------------------------------------------------------------------------------------ */
+
+template <int R>
+static cudaError_t launch_scatter_r(const PassParams& P, const BinParams& B, const float* xyz, uint64_t n, int sm_count,
+                                    cudaStream_t st) {
+    uint32_t head = (reinterpret_cast<uintptr_t>(xyz) & 7u) ? 1u : 0u;   // 12 B per particle: skip one to reach 8-byte alignment
+    if (head > n) head = (uint32_t)n;
+    const uint64_t pairs = (n - head) / 2;
+    const size_t smem = scatter_smem_bytes(B.nb, B.C);
+    cudaError_t e;
+    if (P.sc[0].big) {
+        e = cudaFuncSetAttribute(k_bin_scatter<R, true>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
+        if (e != cudaSuccess) return e;
+        k_bin_scatter<R, true><<<sm_count, BIN_THREADS, smem, st>>>(P, B, xyz, n, head, pairs);
+    } else {
+        e = cudaFuncSetAttribute(k_bin_scatter<R, false>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
+        if (e != cudaSuccess) return e;
+        k_bin_scatter<R, false><<<sm_count, BIN_THREADS, smem, st>>>(P, B, xyz, n, head, pairs);
+    }
+    return cudaGetLastError();
+}
+
+/* P: PassParams of ONE scale restricted to the R = P.d rows of this pass (rows[0..R), sc[0].T = first row).
+ * The caller has zeroed B.cursor[0..nb) on the stream.  Launches scatter + apply. */
+cudaError_t launch_update_binned(const PassParams& P, const BinParams& B, const float* xyz, uint64_t n, int sm_count,
+                                 cudaStream_t st) {
+    cudaError_t e;
+    switch (P.d) {
+        case 1: e = launch_scatter_r<1>(P, B, xyz, n, sm_count, st); break;
+        case 2: e = launch_scatter_r<2>(P, B, xyz, n, sm_count, st); break;
+        case 3: e = launch_scatter_r<3>(P, B, xyz, n, sm_count, st); break;
+        case 4: e = launch_scatter_r<4>(P, B, xyz, n, sm_count, st); break;
+        case 5: e = launch_scatter_r<5>(P, B, xyz, n, sm_count, st); break;
+        case 6: e = launch_scatter_r<6>(P, B, xyz, n, sm_count, st); break;
+        case 7: e = launch_scatter_r<7>(P, B, xyz, n, sm_count, st); break;
+        case 8: e = launch_scatter_r<8>(P, B, xyz, n, sm_count, st); break;
+        default: return cudaErrorInvalidValue;
+    }
+    if (e != cudaSuccess) return e;
+    const uint32_t first = (uint32_t)B.rows_direct << (B.log2w - B.log2S);      // bins of direct rows stay empty
+    if (first >= B.nb) return cudaSuccess;
+    const size_t smem = (size_t)4 << B.log2S;
+    e = cudaFuncSetAttribute(k_bin_apply, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
+    if (e != cudaSuccess) return e;
+    k_bin_apply<<<B.nb - first, BIN_THREADS, smem, st>>>(P.sc[0].T + ((uint64_t)first << B.log2S),
+                                                         B.bins + (uint64_t)first * B.cap, B.cursor + first, B.cap,
+                                                         B.log2S);
+    return cudaGetLastError();
+}
+
+}  // namespace cs

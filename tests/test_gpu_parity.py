@@ -36,7 +36,8 @@ def _ids(t):
     return t.cpu().numpy().view(np.uint64)
 
 
-def _check_all(cs, wl, xyz, sample_p=1.0, k=None, thresholds=(), probe_cells=4096, split=None, cap=None, budget=None):
+def _check_all(cs, wl, xyz, sample_p=1.0, k=None, thresholds=(), probe_cells=4096, split=None, cap=None, budget=None,
+               mode=None):
     """Update + estimate + scan + top-k (+ excursion) on both sides; everything must be identical."""
     k = wl.k if k is None else k
     host = xyz.cpu().numpy()
@@ -44,6 +45,8 @@ def _check_all(cs, wl, xyz, sample_p=1.0, k=None, thresholds=(), probe_cells=409
     g = cs.CountSketch(wl.d, wl.w, list(wl.G), wl.L, wl.seed)
     if budget:
         g.set_table_budget(budget)
+    if mode is not None:
+        g.set_update_mode(*mode)
     n = host.shape[0]
     cuts = [0, n] if not split else [0] + sorted(split) + [n]
     for a, b in zip(cuts[:-1], cuts[1:]):
@@ -170,6 +173,53 @@ def test_staged_scan_even_d_and_many_rows(cs):
         wl = synth.Workload("st", N=60001, G=(700,), d=d, w=3001, k=300, H=32, f_bg=0.3, m_min=0, L=50.0, seed=d,
                             gen_seed=d + 5)
         _check_all(cs, wl, synth.generate(wl, device="cuda"), thresholds=(2,), probe_cells=256, budget=fit * wl.w * 4)
+
+
+# ---- binned update (csrc/cs_update_binned.cu): records partitioned by table slice, applied in shared memory ----
+
+@pytest.mark.parametrize("rows_direct", [0, 3])
+def test_binned_update_cfg3_shape(cs, rows_direct):
+    """d = 7, w = 2^22 (128 slices of 2^15 counters per row), cell ids >= 2^31; odd n; hybrid with 3 direct rows."""
+    wl, xyz = _gen("cfg3", (1 << 22) + 3)
+    _check_all(cs, wl, xyz, k=3000, mode=(2, rows_direct), split=[1234567])
+
+
+def test_binned_update_cfg1_full_heavy_cells(cs):
+    """cfg 1: cells with ~80 particles, w = 2^16 (slices of 512 counters)."""
+    wl, xyz = _gen("cfg1")
+    _check_all(cs, wl, xyz, thresholds=(40,), mode=(2, 0))
+
+
+def test_binned_update_cfg2_and_cfg4_shapes(cs):
+    wl, xyz = _gen("cfg2", 1 << 22)
+    _check_all(cs, wl, xyz, mode=(2, 0))
+    wl, xyz = _gen("cfg4", (1 << 21) + 1)          # w = 2^24: 512 slices per row, several row groups per pass
+    _check_all(cs, wl, xyz, k=3000, mode=(2, 1))
+
+
+def test_binned_update_multiscale_sampled(cs):
+    wl, xyz = _gen("cfg5", 1 << 22)
+    _check_all(cs, wl, xyz, sample_p=wl.sample_p, k=1000, thresholds=(3,), split=[1000001, 3000000], mode=(2, 0))
+
+
+@pytest.mark.parametrize("w", [1 << 8, 1 << 10, 1 << 13, 1000])
+def test_binned_update_small_tables_and_fallbacks(cs, w):
+    """Few slices per row: the staging buffers overflow and records take the direct route; w = 1000 is not a power
+    of two and must fall back to the direct kernel."""
+    from paper_1711_00975_b200 import synth
+    wl = synth.Workload("sm", N=200003, G=(300,), d=5, w=w, k=100, H=16, f_bg=0.3, m_min=0, L=100.0, seed=w, gen_seed=w + 1)
+    xyz = synth.generate(wl, device="cuda")
+    buf = torch.empty(3 * wl.N + 1, dtype=torch.float32, device="cuda")
+    buf[1:] = xyz.reshape(-1)                     # 4-byte aligned only: the pair loads start one particle in
+    _check_all(cs, wl, buf[1:].view(-1, 3), sample_p=0.6, thresholds=(1,), probe_cells=512, mode=(2, 0))
+
+
+def test_binned_update_single_cell_overflows_bin_region(cs):
+    """All particles in one cell: one bin per row receives every record, staging buffers and the bin region overflow."""
+    from paper_1711_00975_b200 import synth
+    pos = np.full((2000001, 3), 3.3, dtype=np.float32)
+    wl = synth.Workload("one", N=len(pos), G=(32,), d=7, w=1 << 16, k=10, H=1, f_bg=0.0, m_min=0, L=10.0)
+    _check_all(cs, wl, torch.from_numpy(pos).cuda(), k=10, cap=4096, mode=(2, 0))
 
 
 # ---- randomised small configs and edge cases ------------------------------------------------------------------
