@@ -110,7 +110,8 @@ int cs_set_table_budget(cs_sketch* s, uint64_t bytes);
  *   mode 1 "direct": one red.global.add.s32 per (particle, row) into L2-resident row groups (table budget above).
  *   mode 2 "binned": updates are first written as 2-byte records partitioned by table slice, then applied slice by
  *           slice in shared memory (csrc/cs_update_binned.cu); needs w a power of two in [2^8, 2^25], else falls
- *           back to direct.  rows_direct rows of every binned pass still take the direct route (0 = none).
+ *           back to direct.  rows_direct rows of every binned pass still take the direct route, concurrently
+ *           (0 = none, -1 = automatic, the default: about 4/7 of the rows while they fit the table budget).
  *   mode 0 "auto" (default): binned for calls of at least 2^22 particles when the shape allows it. */
 int cs_set_update_mode(cs_sketch* s, int mode, int rows_direct);
 

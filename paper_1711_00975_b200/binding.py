@@ -155,7 +155,7 @@ class CountSketch:
     def set_table_budget(self, nbytes: int):
         _chk(lib().cs_set_table_budget(self._h, nbytes), "cs_set_table_budget")
 
-    def set_update_mode(self, mode: int, rows_direct: int = 0):
+    def set_update_mode(self, mode: int, rows_direct: int = -1):
         _chk(lib().cs_set_update_mode(self._h, mode, rows_direct), "cs_set_update_mode")
 
     def set_update_index(self, index: int):

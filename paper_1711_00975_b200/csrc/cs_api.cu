@@ -110,7 +110,7 @@ struct cs_sketch {
 
     /* binned update (cs_update_binned.cu) */
     int update_mode = 0;               /* cs_set_update_mode: 0 auto, 1 direct red.global, 2 binned */
-    int bin_rows_direct = 0;           /* rows of each binned pass that still go through red.global */
+    int bin_rows_direct = -1;          /* rows of each binned pass that still go through red.global; -1 = auto */
     uint16_t* bins = nullptr;          /* record regions */
     uint64_t bins_records = 0;         /* capacity of `bins` in records */
     uint32_t* cursor = nullptr;        /* BIN_MAX words */
@@ -288,7 +288,15 @@ int update_binned(cs_sketch* s, const BinPlan& pl, const float* xyz, uint64_t n,
                 BinParams B;
                 B.bins = s->bins; B.cursor = s->cursor; B.cap = (uint32_t)cap;
                 B.nb = (uint32_t)nr * pl.SL; B.C = pl.C; B.log2S = pl.log2S; B.log2w = pl.log2w;
-                B.rows_direct = s->bin_rows_direct < nr ? s->bin_rows_direct : nr;
+                /* hybrid: the scatter kernel is bound by the integer pipes, the direct rows by the L2 tag rate, so
+                 * both run together; auto = 4/7 of the rows (measured best at d = 7), as long as they stay L2-resident */
+                int rd = s->bin_rows_direct;
+                if (rd < 0) {
+                    rd = (4 * nr + 3) / 7;
+                    const uint64_t fit = s->table_budget / (s->w * sizeof(int32_t));
+                    if ((uint64_t)rd > fit) rd = (int)fit;
+                }
+                B.rows_direct = rd < nr ? rd : nr;
                 CS_CUDA(cudaMemsetAsync(s->cursor, 0, B.nb * sizeof(uint32_t), s->stream));
                 cudaError_t e = launch_update_binned(P, B, xyz + 3 * off, m, s->sm_count, s->stream);
                 if (e != cudaSuccess) return fail(CS_ERR_CUDA, "binned update kernels: %s", cudaGetErrorString(e));
@@ -749,8 +757,8 @@ int cs_set_table_budget(cs_sketch* s, uint64_t bytes) {
 
 int cs_set_update_mode(cs_sketch* s, int mode, int rows_direct) {
     if (!s) return fail(CS_ERR_ARG, "null handle");
-    if (mode < 0 || mode > 2 || rows_direct < 0 || rows_direct > CS_MAX_ROWS)
-        return fail(CS_ERR_ARG, "mode must be 0 (auto), 1 (direct) or 2 (binned); rows_direct in [0, 32]");
+    if (mode < 0 || mode > 2 || rows_direct < -1 || rows_direct > CS_MAX_ROWS)
+        return fail(CS_ERR_ARG, "mode must be 0 (auto), 1 (direct) or 2 (binned); rows_direct in [-1, 32]");
     s->update_mode = mode;
     s->bin_rows_direct = rows_direct;
     return CS_OK;

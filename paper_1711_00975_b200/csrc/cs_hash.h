@@ -8,13 +8,14 @@
  *   a = ah*2^32 + al            al < 2^32, ah < 2^29
  *   A = a*2^31 mod p = Ah*2^32 + Al
  *   b = bh*2^32 + bl            bh < 2^29
- *   a*c + b == lo + m*2^32 (mod p)
- *     lo = al*c0 + bl + Al*c1   < 2^63 + 2^32 + 2^61            (fits 64 bits; two IMAD.WIDE)
- *     m  = ah*c0 + bh + Ah*c1   < 2^60 + 2^29 + 2^58 < 2^61     (two IMAD.WIDE)
+ *   a*c + b == lo + m*2^32 + b (mod p)
+ *     lo = al*c0 + Al*c1        < 2^63 + 2^61                   (fits 64 bits; two IMAD.WIDE)
+ *     m  = ah*c0 + Ah*c1        < 2^60 + 2^58 < 2^61            (two IMAD.WIDE)
  *   m*2^32 = (m >> 29)*2^61 + (m & (2^29-1))*2^32 == mh + ml*2^32      (word-aligned: no 64-bit shifts)
  *   lo     = (lo >> 61)*2^61 + (lo & p)           == lh + ll
- *   s = ll + ml*2^32 + mh + lh  < 2^62 + 2^32 + 8
- *   with sh = s >> 61 (0..2):  q = floor(s / p) = (s + sh + 1) >> 61,   r = s - q*p = (s + q) mod 2^61
+ *   s = ll + ml*2^32 + mh + lh + b  < 3*2^61 + 2^32 + 8 < 2^63
+ *   with sh = s >> 61 (0..3):  q = floor(s / p) = (s + sh + 1) >> 61,   r = s - q*p = (s + q) mod 2^61
+ *   (s = sh*p + (sh + sl) with sl = s mod 2^61, and sh + sl < p + 4 < 2p, so q = sh + [sh + sl >= p])
  * so the low 32 bits of the canonical residue are low32(s) + q: the bucket (w a power of two <= 2^31) and the
  * sign bit need nothing else.
  */
@@ -57,20 +58,32 @@ inline HashCoef split_coef(uint64_t a, uint64_t b) {
 CS_HD uint32_t cell_c0(uint64_t c) { return (uint32_t)c & 0x7FFFFFFFu; }
 CS_HD uint32_t cell_c1(uint64_t c) { return (uint32_t)(c >> 31); }
 
+/* 32 x 32 + 64 -> 64.  On the device this is spelled as the PTX mad.wide.u32 (one IMAD.WIDE): written as C, NVVM
+ * widens the operands to 64 bits and ptxas no longer sees that their high words are zero. */
+CS_HD uint64_t mad_wide_u32(uint32_t a, uint32_t b, uint64_t c) {
+#if defined(__CUDA_ARCH__)
+    uint64_t d;
+    asm("mad.wide.u32 %0, %1, %2, %3;" : "=l"(d) : "r"(a), "r"(b), "l"(c));
+    return d;
+#else
+    return (uint64_t)a * b + c;
+#endif
+}
+
 /* s of the header comment; BIG = false when c < 2^31 (c1 == 0). */
 template <bool BIG>
 CS_HD uint64_t affine_partial(const HashCoef& k, uint32_t c0, uint32_t c1) {
-    uint64_t lo = (uint64_t)k.al * c0 + k.bl;
-    uint64_t m = (uint64_t)k.ah * c0 + k.bh;
+    uint64_t lo = mad_wide_u32(k.al, c0, 0);
+    uint64_t m = mad_wide_u32(k.ah, c0, 0);
     if (BIG) {
-        lo += (uint64_t)k.Al * c1;
-        m += (uint64_t)k.Ah * c1;
+        lo = mad_wide_u32(k.Al, c1, lo);
+        m = mad_wide_u32(k.Ah, c1, m);
     }
     const uint32_t mh = (uint32_t)(m >> 29);
     const uint32_t ml = (uint32_t)m & 0x1FFFFFFFu;
     const uint32_t lo_h = (uint32_t)(lo >> 32);
-    const uint32_t hi = (lo_h & 0x1FFFFFFFu) + ml;                 // < 2^30
-    return (((uint64_t)hi << 32) | (uint32_t)lo) + (uint64_t)mh + (lo_h >> 29);
+    const uint32_t hi = (lo_h & 0x1FFFFFFFu) + ml + k.bh;          // < 3 * 2^29: b rides in free 3-input adder slots
+    return (((uint64_t)hi << 32) | (uint32_t)lo) + (uint64_t)mh + (uint64_t)(lo_h >> 29) + (uint64_t)k.bl;
 }
 
 /* low 32 bits of the canonical residue (a*c + b) mod p */

@@ -39,64 +39,79 @@ __device__ __forceinline__ uint4 ld_stream16u(const uint4* p) {
     return v;
 }
 
-/* Shared-memory layout of k_bin_scatter (dynamic): cnt[NB] | qlen[2] | pad | queue[NB] (u16) | buf[NB*C] (u16) */
-struct ScatterSmem {
-    uint32_t* cnt;
-    uint32_t* qlen;
-    uint16_t* queue;
-    uint16_t* buf;
-};
+/* Shared-memory layout of k_bin_scatter (dynamic): cnt[NB] | qlen | pad | queue[NB] (u16) | buf[NB*C] (u16).
+ * All accesses of the hot loop use 32-bit shared-space addresses (no generic-to-shared conversion per access). */
 __host__ __device__ inline size_t smem_off_queue(uint32_t nb) { return (((size_t)nb + 2) * 4 + 15) & ~(size_t)15; }
 __host__ __device__ inline size_t smem_off_buf(uint32_t nb) { return (smem_off_queue(nb) + (size_t)nb * 2 + 15) & ~(size_t)15; }
 size_t scatter_smem_bytes(uint32_t nb, uint32_t C) { return smem_off_buf(nb) + (size_t)nb * C * 2; }
+
+__device__ __forceinline__ uint32_t atoms_inc(uint32_t addr) {
+    uint32_t old;
+    asm volatile("atom.shared.add.u32 %0, [%1], 1;" : "=r"(old) : "r"(addr) : "memory");
+    return old;
+}
+__device__ __forceinline__ void sts_u16(uint32_t addr, uint32_t v) {
+    asm volatile("st.shared.u16 [%0], %1;" :: "r"(addr), "h"((unsigned short)v) : "memory");
+}
 
 /* Apply one record directly (fallback path and the partial buffers at the end of the kernel). */
 __device__ __forceinline__ void apply_direct(int32_t* T, uint32_t bin, uint32_t log2S, uint32_t rec) {
     red_add(T + (((uint64_t)bin << log2S) | (rec >> 1)), 1 - 2 * (int32_t)(rec & 1u));
 }
 
+/* Loop-invariant values of the insert path, kept in registers. */
+struct InsertCtx {
+    uint32_t cnt_addr;     // shared address of cnt[0]
+    uint32_t buf_addr;     // shared address of buf[0]
+    uint32_t C, C2;        // staging capacity in records / bytes
+    uint32_t log2S, smask; // slice shift, (1 << log2S) - 1
+    uint32_t log2w, wmask;
+    int32_t rows_direct;
+};
+
 template <int R, bool BIG>
-__device__ __forceinline__ void bin_particle(const PassParams& P, const BinParams& B, const ScatterSmem& S,
-                                             uint32_t qsel, float x, float y, float z) {
+__device__ __forceinline__ void bin_particle(const PassParams& P, const InsertCtx& X, float x, float y, float z) {
     const uint64_t c = cell_of(x, y, z, P.sc[0]);
     const uint32_t c0 = cell_c0(c), c1 = cell_c1(c);
     int32_t* T = P.sc[0].T;
-    const uint32_t wmask = (uint32_t)(P.w - 1);
 #pragma unroll
     for (int j = 0; j < R; ++j) {
-        const uint32_t h = affine_low32<BIG>(P.rows[j].h, c0, c1) & wmask;
+        const uint32_t h = affine_low32<BIG>(P.rows[j].h, c0, c1) & X.wmask;
         const uint32_t sb = affine_low32<BIG>(P.rows[j].s, c0, c1) & 1u;
-        const uint32_t key = ((uint32_t)j << B.log2w) | h;             // counter index within this pass's rows
-        if (j < B.rows_direct) {
+        const uint32_t key = ((uint32_t)j << X.log2w) | h;             // counter index within this pass's rows
+        if (j < X.rows_direct) {
             red_add(T + key, 1 - 2 * (int32_t)sb);
             continue;
         }
-        const uint32_t bin = key >> B.log2S;
-        const uint32_t rec = ((key & ((1u << B.log2S) - 1u)) << 1) | sb;
-        const uint32_t slot = atomicAdd(&S.cnt[bin], 1u);
-        if (slot < B.C) {
-            S.buf[bin * B.C + slot] = (uint16_t)rec;
-            if (slot == UNIT - 1) S.queue[atomicAdd(&S.qlen[qsel], 1u)] = (uint16_t)bin;
-        } else {
-            red_add(T + key, 1 - 2 * (int32_t)sb);                     // staging buffer full: apply directly
-        }
+        const uint32_t bin = key >> X.log2S;
+        const uint32_t slot = atoms_inc(X.cnt_addr + bin * 4u);
+        if (slot < X.C) sts_u16(X.buf_addr + bin * X.C2 + slot * 2u, ((key & X.smask) << 1) + sb);
+        else            red_add(T + key, 1 - 2 * (int32_t)sb);         // staging buffer full: apply directly
     }
 }
 
 /* Particles [head, head + 2*pairs) are read as pairs (3 x 8 B per thread, 8-byte aligned); the <= 1 particle
- * before and the <= 1 after are applied directly by block 0. */
+ * before and the <= 1 after are applied directly by block 0.
+ * One round = every thread bins one pair; then the bins holding >= 32 records are queued and flushed. */
 template <int R, bool BIG>
 __global__ void __launch_bounds__(BIN_THREADS, 1)
 k_bin_scatter(const __grid_constant__ PassParams P, const __grid_constant__ BinParams B,
               const float* __restrict__ xyz, uint64_t n, uint32_t head, uint64_t pairs) {
     extern __shared__ __align__(16) unsigned char smem_raw[];
-    ScatterSmem S;
-    S.cnt = reinterpret_cast<uint32_t*>(smem_raw);
-    S.qlen = S.cnt + B.nb;
-    S.queue = reinterpret_cast<uint16_t*>(smem_raw + smem_off_queue(B.nb));
-    S.buf = reinterpret_cast<uint16_t*>(smem_raw + smem_off_buf(B.nb));
-    for (uint32_t i = threadIdx.x; i < B.nb + 2; i += BIN_THREADS) S.cnt[i] = 0;       // cnt and qlen[0..1]
+    uint32_t* cnt = reinterpret_cast<uint32_t*>(smem_raw);
+    uint32_t* qlen = cnt + B.nb;
+    uint16_t* queue = reinterpret_cast<uint16_t*>(smem_raw + smem_off_queue(B.nb));
+    uint16_t* buf = reinterpret_cast<uint16_t*>(smem_raw + smem_off_buf(B.nb));
+    for (uint32_t i = threadIdx.x; i < B.nb + 1; i += BIN_THREADS) cnt[i] = 0;          // cnt and qlen
     __syncthreads();
+
+    InsertCtx X;
+    X.cnt_addr = (uint32_t)__cvta_generic_to_shared(cnt);
+    X.buf_addr = (uint32_t)__cvta_generic_to_shared(buf);
+    X.C = B.C; X.C2 = B.C * 2u;
+    X.log2S = B.log2S; X.smask = (1u << B.log2S) - 1u;
+    X.log2w = B.log2w; X.wmask = (uint32_t)(P.w - 1);
+    X.rows_direct = B.rows_direct;
 
     const float2* body = reinterpret_cast<const float2*>(xyz + 3 * (uint64_t)head);
     const uint64_t per_round = (uint64_t)gridDim.x * BIN_THREADS;
@@ -107,33 +122,45 @@ k_bin_scatter(const __grid_constant__ PassParams P, const __grid_constant__ BinP
     int32_t* T = P.sc[0].T;
 
     for (uint64_t r = 0; r < rounds; ++r) {
-        const uint32_t qsel = (uint32_t)(r & 1);
+        if (threadIdx.x == 0) *qlen = 0;                               // last read before the previous barrier
         const uint64_t g = r * per_round + (uint64_t)blockIdx.x * BIN_THREADS + threadIdx.x;
         if (g < pairs) {
             const float2 q0 = ld_stream8(body + 3 * g);
             const float2 q1 = ld_stream8(body + 3 * g + 1);
             const float2 q2 = ld_stream8(body + 3 * g + 2);
             const uint64_t i0 = P.index0 + head + 2 * g;
-            if (!P.sample || keep_particle(P.K, i0, P.Tp)) bin_particle<R, BIG>(P, B, S, qsel, q0.x, q0.y, q1.x);
-            if (!P.sample || keep_particle(P.K, i0 + 1, P.Tp)) bin_particle<R, BIG>(P, B, S, qsel, q1.y, q2.x, q2.y);
+            if (!P.sample || keep_particle(P.K, i0, P.Tp)) bin_particle<R, BIG>(P, X, q0.x, q0.y, q1.x);
+            if (!P.sample || keep_particle(P.K, i0 + 1, P.Tp)) bin_particle<R, BIG>(P, X, q1.y, q2.x, q2.y);
         }
         __syncthreads();
-        /* flush every bin that completed a unit in this round: groups of 4 lanes, one bin each */
-        const uint32_t nq = S.qlen[qsel];
-        if (threadIdx.x == 0) S.qlen[qsel ^ 1] = 0;                   // not in use until after the next barrier
+        /* queue the bins that hold at least one full unit */
+        for (uint32_t b0 = warp * 32; b0 < B.nb; b0 += BIN_THREADS) {
+            const uint32_t bin = b0 + lane;
+            const bool full = bin < B.nb && cnt[bin] >= UNIT;
+            const uint32_t m = __ballot_sync(0xFFFFFFFFu, full);
+            if (m) {
+                uint32_t at = 0;
+                if (lane == 0) at = atomicAdd(qlen, (uint32_t)__popc(m));
+                at = __shfl_sync(0xFFFFFFFFu, at, 0);
+                if (full) queue[at + __popc(m & ((1u << lane) - 1u))] = (uint16_t)bin;
+            }
+        }
+        __syncthreads();
+        /* flush: groups of 4 lanes, one queued bin each */
+        const uint32_t nq = *qlen;
         for (uint32_t e0 = warp * 8; e0 < nq; e0 += (BIN_THREADS / 32) * 8) {
             const uint32_t e = e0 + grp;
             const bool on = e < nq;
             uint32_t bin = 0, c = 0, units = 0, base = 0;
             if (on) {
-                bin = S.queue[e];
-                c = min(S.cnt[bin], B.C);
+                bin = queue[e];
+                c = min(cnt[bin], B.C);
                 units = c / UNIT;
                 if (l4 == 0) base = atomicAdd(&B.cursor[bin], units * UNIT);
             }
             base = __shfl_sync(0xFFFFFFFFu, base, grp * 4);
             if (on) {
-                const uint16_t* src = S.buf + bin * B.C;
+                const uint16_t* src = buf + bin * B.C;
                 for (uint32_t u = 0; u < units; ++u) {
                     const uint4 v = *reinterpret_cast<const uint4*>(src + u * UNIT + l4 * 8);
                     const uint32_t at = base + u * UNIT;
@@ -160,17 +187,17 @@ k_bin_scatter(const __grid_constant__ PassParams P, const __grid_constant__ BinP
 #pragma unroll
                 for (int k = 0; k < 8; ++k) {
                     const uint32_t i = l4 * 8 + k;
-                    if (i < left) S.buf[bin * B.C + i] = tmp[k];
+                    if (i < left) buf[bin * B.C + i] = tmp[k];
                 }
-                if (l4 == 0) S.cnt[bin] = left;
+                if (l4 == 0) cnt[bin] = left;
             }
         }
         __syncthreads();
     }
     /* partial buffers (< 32 records per bin): applied directly */
     for (uint32_t bin = threadIdx.x; bin < B.nb; bin += BIN_THREADS) {
-        const uint32_t c = min(S.cnt[bin], B.C);
-        for (uint32_t i = 0; i < c; ++i) apply_direct(T, bin, B.log2S, S.buf[bin * B.C + i]);
+        const uint32_t c = min(cnt[bin], B.C);
+        for (uint32_t i = 0; i < c; ++i) apply_direct(T, bin, B.log2S, buf[bin * B.C + i]);
     }
     if (blockIdx.x == 0 && threadIdx.x < 2) {
         const uint64_t tail0 = (uint64_t)head + 2 * pairs;
