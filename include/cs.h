@@ -80,7 +80,8 @@ uint64_t cs_sample_threshold(double sample_p);
  * (csrc/cs_hash.h) -- so that it can be checked against big-integer arithmetic without a GPU:
  * *r_out = (a*c + b) mod (2^61-1), canonical, through the full-residue form; *low32_out = its low 32 bits through
  * the short form the kernels use for power-of-two w and for the sign.  big = 0 selects the form compiled for
- * meshes with G^3 <= 2^31 (needs c < 2^31), big = 1 the general one (c < 2^60).  1 <= a < p, b < p. */
+ * meshes with G^3 <= 2^31 (needs c < 2^31), big = 1 the general one (c < 2^60), big = 2 the table form used when
+ * the high limb of every cell id is < 64 (needs c < 2^37).  1 <= a < p, b < p. */
 int cs_hash_cell(uint64_t a, uint64_t b, uint64_t c, int big, uint64_t* r_out, uint32_t* low32_out);
 
 /* ---- life cycle --------------------------------------------------------------------------------------- */

@@ -96,7 +96,7 @@ def derive_coeffs(seed: int, d: int):
     return out.reshape(d, 4), int(K.value)
 
 
-def hash_cell(a: int, b: int, c: int, big: bool = True):
+def hash_cell(a: int, b: int, c: int, big=True):
     """Host-only: ((a*c + b) mod (2^61-1), its low 32 bits) through the library's limb arithmetic (csrc/cs_hash.h)."""
     r, lo = u64(0), u32(0)
     _chk(lib().cs_hash_cell(a, b, c, int(big), C.byref(r), C.byref(lo)), "cs_hash_cell")

@@ -629,10 +629,14 @@ uint64_t cs_sample_threshold(double sample_p) { return sample_threshold(sample_p
 int cs_hash_cell(uint64_t a, uint64_t b, uint64_t c, int big, uint64_t* r_out, uint32_t* low32_out) {
     if (!r_out || !low32_out) return fail(CS_ERR_ARG, "cs_hash_cell: null output");
     if (a < 1 || a >= P61 || b >= P61) return fail(CS_ERR_ARG, "cs_hash_cell: a must be in [1, p-1], b in [0, p-1]");
-    if (c >= (1ull << 60) || (!big && c >= (1ull << 31)))
+    if (c >= (1ull << 60) || (!big && c >= (1ull << 31)) || (big == 2 && (c >> 31) >= HASH_TB))
         return fail(CS_ERR_ARG, "cs_hash_cell: c out of range for this form");
     const HashCoef k = split_coef(a, b);
-    if (big) {
+    if (big == 2) {
+        const uint64_t tb = affine_mod_p<true>(k, 0u, cell_c1(c));      /* the table entry the kernels look up */
+        *low32_out = affine_low32_tb(k, cell_c0(c), tb + 1);
+        *r_out = (affine_partial_tb(k, cell_c0(c), tb) + 0) % P61;      /* s mod p, for the comparison only */
+    } else if (big) {
         *r_out = affine_mod_p<true>(k, cell_c0(c), cell_c1(c));
         *low32_out = affine_low32<true>(k, cell_c0(c), cell_c1(c));
     } else {

@@ -86,6 +86,57 @@ CS_HD uint64_t affine_partial(const HashCoef& k, uint32_t c0, uint32_t c1) {
     return (((uint64_t)hi << 32) | (uint32_t)lo) + (uint64_t)mh + (uint64_t)(lo_h >> 29) + (uint64_t)k.bl;
 }
 
+/* Table form for cell ids with a small high limb (c1 < 64, i.e. G^3 <= 2^37): tb = (A*c1 + b) mod p is looked up
+ * (kernels keep tb[c1][hash] in shared memory), so that only the two c0 products remain:
+ *   s = ll + ml*2^32 + mh + lh + tb,  same bounds as above with tb < 2^61 in the place of b. */
+CS_HD uint64_t affine_partial_tb(const HashCoef& k, uint32_t c0, uint64_t tb) {
+    const uint64_t lo = mad_wide_u32(k.al, c0, 0);
+    const uint64_t m = mad_wide_u32(k.ah, c0, 0);
+    const uint32_t mh = (uint32_t)(m >> 29);
+    const uint32_t ml = (uint32_t)m & 0x1FFFFFFFu;
+    const uint32_t lo_h = (uint32_t)(lo >> 32);
+    const uint32_t hi = (lo_h & 0x1FFFFFFFu) + ml + (uint32_t)(tb >> 32);
+    return (((uint64_t)hi << 32) | (uint32_t)lo) + (uint64_t)mh + (uint64_t)(lo_h >> 29) + (uint64_t)(uint32_t)tb;
+}
+
+/* low 32 bits of the canonical residue from s (see the header comment) */
+CS_HD uint32_t fold_low32(uint64_t s) {
+    const uint32_t sh = (uint32_t)(s >> 61);
+    const uint32_t q = (uint32_t)((s + (uint64_t)(sh + 1u)) >> 61);
+    return (uint32_t)s + q;
+}
+
+/* The same value as fold_low32(affine_partial_tb(k, c0, tb1 - 1)) for tb1 = tb + 1 (the kernels' tables hold
+ * tb + 1).  On the device the 64-bit adds, the shifts by 29 and the 29-bit masks are spelled as multiply-adds
+ * (x*8 as a 32x32->64 product yields x >> 29 in its high word; x - (x >> 29)*2^29 is x & (2^29-1)), because the
+ * kernels are bound by the integer ALU pipe while the multiply-add pipe idles:
+ *   lo = al*c0 + tb1 = lh*2^61 + ll,   s1 = ll + lh + mh + ml*2^32 = s + 1  (< 2^62 + 2^33),
+ *   q = floor(s / p) = (s1 + (s1 >> 61)) >> 61   (holds also when s1 is a multiple of 2^61),  low32(r) = low32(s1) + q - 1. */
+CS_HD uint32_t affine_low32_tb(const HashCoef& k, uint32_t c0, uint64_t tb1) {
+#if defined(__CUDA_ARCH__)
+    const uint64_t m = mad_wide_u32(k.ah, c0, 0);
+    const uint32_t m_l = (uint32_t)m, m_h = (uint32_t)(m >> 32);
+    const uint32_t t_h = (uint32_t)(mad_wide_u32(m_l, 8u, 0) >> 32);            // m_l >> 29
+    const uint32_t mh = m_h * 8u + t_h;                                          // m >> 29
+    const uint32_t ml = m_l & 0x1FFFFFFFu;
+    const uint64_t lo = mad_wide_u32(k.al, c0, tb1);
+    const uint32_t lo_l = (uint32_t)lo, lo_h = (uint32_t)(lo >> 32);
+    const uint32_t lh = (uint32_t)(mad_wide_u32(lo_h, 8u, 0) >> 32);            // lo >> 61
+    const uint32_t hi = (lo_h & 0x1FFFFFFFu) + ml;
+    uint64_t s1 = ((uint64_t)hi << 32) | lo_l;
+    s1 = mad_wide_u32(mh, 1u, s1);
+    s1 = mad_wide_u32(lh, 1u, s1);
+    const uint32_t sh = (uint32_t)(mad_wide_u32((uint32_t)(s1 >> 32), 8u, 0) >> 32);
+    const uint64_t w = mad_wide_u32(sh, 1u, s1);
+    const uint32_t q = (uint32_t)(mad_wide_u32((uint32_t)(w >> 32), 8u, 0) >> 32);
+    return (uint32_t)s1 + q - 1u;
+#else
+    return fold_low32(affine_partial_tb(k, c0, tb1 - 1));
+#endif
+}
+
+constexpr uint32_t HASH_TB = 64;     /* table entries per hash: c1 = 0 .. 63 */
+
 /* low 32 bits of the canonical residue (a*c + b) mod p */
 template <bool BIG>
 CS_HD uint32_t affine_low32(const HashCoef& k, uint32_t c0, uint32_t c1) {

@@ -161,6 +161,9 @@ def test_limb_hash_arithmetic_against_big_integers(cslib, golden):
         if c < 2 ** 31:
             r, lo = binding.hash_cell(a, b, c, big=False)
             assert r == want and lo == want & 0xFFFFFFFF, (a, b, c, "small form")
+        if c < 2 ** 37:
+            r, lo = binding.hash_cell(a, b, c, big=2)
+            assert r == want and lo == want & 0xFFFFFFFF, (a, b, c, "table form")
     assert cslib.cs_hash_cell(0, 0, 0, 1, None, None) == binding.CS_ERR_ARG
     r, lo = C.c_uint64(0), C.c_uint32(0)
     assert cslib.cs_hash_cell(1, 0, 2 ** 31, 0, C.byref(r), C.byref(lo)) == binding.CS_ERR_ARG
