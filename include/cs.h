@@ -116,6 +116,14 @@ int cs_set_table_budget(cs_sketch* s, uint64_t bytes);
  *   mode 0 "auto" (default): binned for calls of at least 2^22 particles when the shape allows it. */
 int cs_set_update_mode(cs_sketch* s, int mode, int rows_direct);
 
+/* How cs_scan evaluates cells.  The result never depends on it.
+ *   mode 1 "plain": every cell gets the early-exit estimate from the int32 tables.
+ *   mode 2 "bitmap": once the collection threshold tau is >= 1 (and w is a power of two), a 1-bit-per-counter
+ *           bitmap |T| >= tau is built and every cell is first tested against it with the bucket hashes alone
+ *           (csrc/cs_scan_bitmap.cu); survivors get the exact estimate.
+ *   mode 0 "auto" (default): the faster of the two as measured on the BASELINE shapes (currently plain). */
+int cs_set_scan_mode(cs_sketch* s, int mode);
+
 /* Running particle index of the update stream / of the current scan (sampling, R13, R17).
  * Setting it lets a stream shard (multi-GPU) reproduce the single-stream sampling decisions. */
 int cs_set_update_index(cs_sketch* s, uint64_t index);

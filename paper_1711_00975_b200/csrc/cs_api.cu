@@ -68,7 +68,7 @@ int bit_length(uint64_t v) {
 
 constexpr int STAGE_SLOTS = 3;
 constexpr uint64_t STAGE_PARTICLES = 1ull << 24;      /* 192 MiB per staging slot */
-constexpr uint64_t MAX_CHUNK = 1ull << 25;            /* particles per scan launch */
+constexpr uint64_t MAX_CHUNK = 1ull << 27;            /* particles per scan launch */
 constexpr uint32_t MIN_CAP = 1u << 22;                /* candidate entries per scale */
 
 }  // namespace
@@ -114,6 +114,12 @@ struct cs_sketch {
     uint16_t* bins = nullptr;          /* record regions */
     uint64_t bins_records = 0;         /* capacity of `bins` in records */
     uint32_t* cursor = nullptr;        /* BIN_MAX words */
+
+    /* bitmap prefilter of the scan (cs_scan_bitmap.cu): B[j][b] = |T[j][b]| >= tau_bm, per scale */
+    int scan_mode = 0;                 /* cs_set_scan_mode: 0 auto, 1 plain, 2 bitmap once tau >= 1 */
+    uint32_t* bm[CS_MAX_SCALES] = {};
+    int32_t tau_bm[CS_MAX_SCALES] = {};
+    bool bm_valid[CS_MAX_SCALES] = {};
 
     /* survivor lists of the row-partitioned scan */
     StageBuffers stb = {};
@@ -227,11 +233,31 @@ constexpr uint64_t BIN_MIN_N = 1ull << 22;            /* auto mode: below this t
 constexpr size_t BIN_SMEM = 200 * 1024;               /* shared memory of one scatter CTA */
 
 struct BinPlan {
-    uint32_t log2w, log2S, SL, C;
-    int rows_per_pass;
+    uint32_t log2w, log2S, SL, C, threads;
+    int rows_per_pass, rows_direct;       /* rows of one pass, and how many of them take the direct route */
 };
 
 int ilog2(uint64_t v) { return bit_length(v) - 1; }
+
+uint32_t staging_capacity(uint32_t threads, uint32_t SL) {
+    const double lambda = 2.0 * threads / SL;          /* records per bin, round and CTA (2 particles per thread) */
+    uint32_t C = (uint32_t)(32.0 + lambda + 6.0 * std::sqrt(lambda) + 8.0);
+    C = (C + 7u) & ~7u;
+    return C > 256 ? 256 : C;                          /* beyond: staging overflows go through red.global */
+}
+
+/* Rows of a pass of r rows that take the direct route.  Hybrid: the scatter kernel is bound by the integer pipes,
+ * the direct rows by the L2 tag rate, so both run together; auto = 3/7 of the rows (measured best at d = 7) as long
+ * as they stay L2-resident. */
+int direct_rows(const cs_sketch* s, int r) {
+    int rd = s->bin_rows_direct;
+    if (rd < 0) {
+        rd = (3 * r + 3) / 7;
+        const uint64_t fit = s->table_budget / (s->w * sizeof(int32_t));
+        if ((uint64_t)rd > fit) rd = (int)fit;
+    }
+    return rd < r ? rd : r;
+}
 
 /* false: this shape cannot be binned (w not a power of two, too small or too wide): use the direct kernel */
 bool bin_plan(const cs_sketch* s, BinPlan* pl) {
@@ -242,24 +268,28 @@ bool bin_plan(const cs_sketch* s, BinPlan* pl) {
     int lS = lw - 7;                                   /* 128 slices per row ... */
     if (lS < 8) lS = 8;
     if (lS > 15) lS = 15;                              /* ... of at most 2^15 counters (128 KB, 15-bit offsets) */
-    if (lS > lw) lS = lw;
     const uint32_t SL = (uint32_t)(w >> lS);
-    const double lambda = 2048.0 / SL;                 /* records per bin, round and CTA (1024 threads x 2 particles) */
-    uint32_t C = (uint32_t)(32.0 + lambda + 6.0 * std::sqrt(lambda) + 8.0);
-    C = (C + 7u) & ~7u;
-    if (C > 256) C = 256;                              /* beyond: staging overflows go through red.global */
     int rows = 0;
-    for (int r = 1; r <= 8 && r <= s->d; ++r)
-        if ((uint64_t)r * SL <= BIN_MAX && scatter_smem_bytes(r * SL, C) <= BIN_SMEM) rows = r;
+    for (int r = 1; r <= 8 && r <= s->d; ++r) {
+        const uint32_t nb = (uint32_t)(r - direct_rows(s, r)) * SL;
+        if (nb <= BIN_MAX && scatter_smem_bytes(nb, staging_capacity(1024, SL)) <= BIN_SMEM) rows = r;
+    }
     if (!rows) return false;
-    pl->log2w = (uint32_t)lw; pl->log2S = (uint32_t)lS; pl->SL = SL; pl->C = C; pl->rows_per_pass = rows;
+    const int groups = (s->d + rows - 1) / rows;
+    rows = (s->d + groups - 1) / groups;               /* balanced row groups */
+    pl->log2w = (uint32_t)lw; pl->log2S = (uint32_t)lS; pl->SL = SL;
+    pl->rows_per_pass = rows;
+    pl->rows_direct = direct_rows(s, rows);
+    /* two CTAs of 512 threads per SM when their staging buffers fit: one CTA's flush phase overlaps the other's hashing */
+    const uint32_t nb = (uint32_t)(rows - pl->rows_direct) * SL;
+    pl->threads = scatter_smem_bytes(nb, staging_capacity(512, SL)) <= 110 * 1024 ? 512 : 1024;
+    pl->C = staging_capacity(pl->threads, SL);
     return true;
 }
 
 int update_binned(cs_sketch* s, const BinPlan& pl, const float* xyz, uint64_t n, uint64_t index0, double sample_p) {
     const PassParams full = pass_params(s, index0, sample_p);
-    const int groups = (s->d + pl.rows_per_pass - 1) / pl.rows_per_pass;
-    const int each = (s->d + groups - 1) / groups;                       /* balanced row groups */
+    const int each = pl.rows_per_pass;
     const uint64_t chunk_max = n < BIN_CHUNK ? n : BIN_CHUNK;
     const double keep = sample_p < 1.0 ? sample_p : 1.0;
     uint64_t cap = (uint64_t)((double)chunk_max * keep / pl.SL * 1.04) + 2048;
@@ -287,20 +317,13 @@ int update_binned(cs_sketch* s, const BinPlan& pl, const float* xyz, uint64_t n,
                 for (int j = 0; j < nr; ++j) P.rows[j] = full.rows[i * s->d + j0 + j];
                 BinParams B;
                 B.bins = s->bins; B.cursor = s->cursor; B.cap = (uint32_t)cap;
-                B.nb = (uint32_t)nr * pl.SL; B.C = pl.C; B.log2S = pl.log2S; B.log2w = pl.log2w;
-                /* hybrid: the scatter kernel is bound by the integer pipes, the direct rows by the L2 tag rate, so
-                 * both run together; auto = 4/7 of the rows (measured best at d = 7), as long as they stay L2-resident */
-                int rd = s->bin_rows_direct;
-                if (rd < 0) {
-                    rd = (4 * nr + 3) / 7;
-                    const uint64_t fit = s->table_budget / (s->w * sizeof(int32_t));
-                    if ((uint64_t)rd > fit) rd = (int)fit;
-                }
-                B.rows_direct = rd < nr ? rd : nr;
-                CS_CUDA(cudaMemsetAsync(s->cursor, 0, B.nb * sizeof(uint32_t), s->stream));
+                B.rows_direct = pl.rows_direct < nr ? pl.rows_direct : nr;
+                B.nb = (uint32_t)(nr - B.rows_direct) * pl.SL;
+                B.threads = pl.threads; B.C = pl.C; B.log2S = pl.log2S; B.log2w = pl.log2w;
+                if (B.nb) CS_CUDA(cudaMemsetAsync(s->cursor, 0, B.nb * sizeof(uint32_t), s->stream));
                 cudaError_t e = launch_update_binned(P, B, xyz + 3 * off, m, s->sm_count, s->stream);
                 if (e != cudaSuccess) return fail(CS_ERR_CUDA, "binned update kernels: %s", cudaGetErrorString(e));
-                s->launches += B.rows_direct < nr ? 2 : 1;
+                s->launches += B.nb ? 2 : 1;
             }
     }
     return CS_OK;
@@ -397,6 +420,28 @@ int launch_scan_chunk(cs_sketch* s, const float* xyz, uint64_t n, uint64_t index
     const PassParams full = pass_params(s, index0, sample_p);
     ScanParams S;
     fill_scan_params(s, &S);
+    /* bitmap prefilter: valid once every scale collects against a tau >= 1 (|T| >= tau is then necessary for a row
+     * to pass); rebuilt (d*w/8 bytes, microseconds) whenever a compaction has raised tau */
+    bool use_bm = s->scan_mode == 2 && (s->w & (s->w - 1)) == 0;
+    for (int i = 0; i < s->n_scales && use_bm; ++i) use_bm = s->st_host[i].tau >= 1;
+    if (use_bm) {
+        const uint64_t counters = (uint64_t)s->d * s->w;
+        for (int i = 0; i < s->n_scales; ++i) {
+            if (!s->bm[i]) CS_CUDA(cudaMalloc(&s->bm[i], ((counters + 31) / 32) * sizeof(uint32_t)));
+            if (!s->bm_valid[i] || s->tau_bm[i] != s->st_host[i].tau) {
+                cudaError_t eb = launch_build_bitmap(s->T[i], counters, s->st_host[i].tau, s->bm[i], s->stream);
+                if (eb != cudaSuccess) return fail(CS_ERR_CUDA, "bitmap kernel: %s", cudaGetErrorString(eb));
+                s->launches += 1;
+                s->tau_bm[i] = s->st_host[i].tau;
+                s->bm_valid[i] = true;
+            }
+        }
+        cudaError_t eb = launch_scan_bitmap(full, S, s->bm, xyz, n, s->sm_count, s->stream);
+        if (eb != cudaSuccess) return fail(CS_ERR_CUDA, "bitmap scan kernel: %s", cudaGetErrorString(eb));
+        s->launches += 1;
+        s->n_scan_launches += 1;
+        return CS_OK;
+    }
     const uint64_t row_bytes = s->w * sizeof(int32_t);
     const uint64_t scale_bytes = row_bytes * s->d;
     cudaError_t e = cudaSuccess;
@@ -718,6 +763,7 @@ int cs_destroy(cs_sketch* s) {
     free_stage_lists(s);
     if (s->bins) cudaFree(s->bins);
     if (s->cursor) cudaFree(s->cursor);
+    for (int i = 0; i < CS_MAX_SCALES; ++i) if (s->bm[i]) cudaFree(s->bm[i]);
     for (int i = 0; i < CS_MAX_SCALES; ++i) if (s->T[i]) cudaFree(s->T[i]);
     if (s->st_dev) cudaFree(s->st_dev);
     if (s->st_host) cudaFreeHost(s->st_host);
@@ -765,6 +811,13 @@ int cs_set_update_mode(cs_sketch* s, int mode, int rows_direct) {
         return fail(CS_ERR_ARG, "mode must be 0 (auto), 1 (direct) or 2 (binned); rows_direct in [-1, 32]");
     s->update_mode = mode;
     s->bin_rows_direct = rows_direct;
+    return CS_OK;
+}
+
+int cs_set_scan_mode(cs_sketch* s, int mode) {
+    if (!s) return fail(CS_ERR_ARG, "null handle");
+    if (mode < 0 || mode > 2) return fail(CS_ERR_ARG, "mode must be 0 (auto), 1 (plain) or 2 (bitmap)");
+    s->scan_mode = mode;
     return CS_OK;
 }
 
@@ -844,6 +897,7 @@ int cs_scan_begin(cs_sketch* s, uint64_t k_max, int32_t thr_min) {
     }
     s->k_max = k_max; s->thr_min = thr_min;
     s->scan_index = 0; s->rate = 1.0; s->first_chunk = true; s->n_scan_launches = 0;
+    for (int i = 0; i < CS_MAX_SCALES; ++i) s->bm_valid[i] = false;    /* the tables may have changed */
     for (int i = 0; i < s->n_scales; ++i) {
         s->st_host[i].count = 0;
         s->st_host[i].tau = k_max ? INT32_MIN : thr_min;

@@ -71,7 +71,8 @@ struct BinParams {
     uint16_t* bins;       // nb regions of `cap` records each
     uint32_t* cursor;     // records reserved per bin (zeroed before each pass)
     uint32_t cap;         // records per bin region, a multiple of 32
-    uint32_t nb;          // bins of this pass = rows << (log2w - log2S)
+    uint32_t nb;          // bins of this pass = binned rows << (log2w - log2S)
+    uint32_t threads;     // CTA size of the scatter kernel (512 or 1024)
     uint32_t C;           // records per shared-memory staging buffer, a multiple of 8
     uint32_t log2S;       // <= 15
     uint32_t log2w;
@@ -85,6 +86,10 @@ cudaError_t launch_update_binned(const PassParams& P, const BinParams& B, const 
 cudaError_t launch_update(const PassParams& P, const float* xyz, uint64_t n, int sm_count, cudaStream_t st);
 cudaError_t launch_scan(const PassParams& P, const ScanParams& S, const float* xyz, uint64_t n, int sm_count,
                         cudaStream_t st);
+/* bitmap-prefiltered scan (cs_scan_bitmap.cu) */
+cudaError_t launch_build_bitmap(const int32_t* T, uint64_t n_counters, int32_t tau, uint32_t* bm, cudaStream_t st);
+cudaError_t launch_scan_bitmap(const PassParams& P, const ScanParams& S, const uint32_t* const* bm, const float* xyz,
+                               uint64_t n, int sm_count, cudaStream_t st);
 /* row-partitioned scan of one scale (cs_scan_staged.cu) */
 struct StageBuffers {
     uint64_t* list[2];     // survivor lists (ping-pong), cap_entries each

@@ -114,11 +114,12 @@ __device__ __forceinline__ void bin_particle(const PassParams& P, const InsertCt
     for (int j = 0; j < R; ++j) {
         uint32_t h, sb;
         row_hashes<HM>(P.rows[j], c0, c1, tb_addr + j * 16, h, sb);
-        const uint32_t key = ((uint32_t)j << X.log2w) | (h & X.wmask);  // counter index within this pass's rows
         if (j < X.rows_direct) {
-            red_add(T + key, 1 - 2 * (int32_t)sb);
+            red_add(T + (((uint32_t)j << X.log2w) | (h & X.wmask)), 1 - 2 * (int32_t)sb);
             continue;
         }
+        /* counter index within the binned rows of this pass (bins cover rows rows_direct .. R-1 only) */
+        const uint32_t key = ((uint32_t)(j - X.rows_direct) << X.log2w) | (h & X.wmask);
         const uint32_t bin = key >> X.log2S;
         const uint32_t slot = atoms_inc(X.cnt_addr + bin * 4u);
         if (slot < X.C) sts_u16(X.buf_addr + bin * X.C2 + slot * 2u, ((key & X.smask) << 1) + sb);
@@ -135,15 +136,16 @@ __global__ void __launch_bounds__(BIN_THREADS, 1)
 k_bin_scatter(const __grid_constant__ PassParams P, const __grid_constant__ BinParams B,
               const float* __restrict__ xyz, uint64_t n, uint32_t head, uint64_t pairs) {
     extern __shared__ __align__(16) unsigned char smem_raw[];
+    const uint32_t NT = blockDim.x;                                  // 512 or 1024
     uint32_t* cnt = reinterpret_cast<uint32_t*>(smem_raw);
     uint32_t* qlen = cnt + B.nb;
     uint16_t* queue = reinterpret_cast<uint16_t*>(smem_raw + smem_off_queue(B.nb));
     uint16_t* buf = reinterpret_cast<uint16_t*>(smem_raw + smem_off_buf(B.nb));
     uint64_t* tb = reinterpret_cast<uint64_t*>(smem_raw + smem_off_tb(B.nb, B.C));
-    for (uint32_t i = threadIdx.x; i < B.nb + 1; i += BIN_THREADS) cnt[i] = 0;          // cnt and qlen
+    for (uint32_t i = threadIdx.x; i < B.nb + 1; i += NT) cnt[i] = 0;          // cnt and qlen
     if (HM == 1) {
         /* tb[c1][2j + {0,1}] = 1 + (A*c1 + b) mod p = 1 + (a*(c1*2^31) + b) mod p for the bucket / sign hash of row j */
-        for (uint32_t i = threadIdx.x; i < HASH_TB * 2 * R; i += BIN_THREADS) {
+        for (uint32_t i = threadIdx.x; i < HASH_TB * 2 * R; i += NT) {
             const uint32_t c1 = i / (2 * R), hs = i % (2 * R);
             const RowCoef& rc = P.rows[hs >> 1];
             tb[i] = affine_mod_p<true>((hs & 1) ? rc.s : rc.h, 0u, c1) + 1;          // tb + 1, see affine_low32_tb
@@ -161,15 +163,15 @@ k_bin_scatter(const __grid_constant__ PassParams P, const __grid_constant__ BinP
     X.rows_direct = B.rows_direct;
 
     const float2* body = reinterpret_cast<const float2*>(xyz + 3 * (uint64_t)head);
-    const uint64_t per_round = (uint64_t)gridDim.x * BIN_THREADS;
+    const uint64_t per_round = (uint64_t)gridDim.x * NT;
     const uint64_t rounds = (pairs + per_round - 1) / per_round;
     const uint32_t lane = threadIdx.x & 31u, warp = threadIdx.x >> 5;
     const uint32_t grp = lane >> 2, l4 = lane & 3u;
-    int32_t* T = P.sc[0].T;
+    int32_t* T = P.sc[0].T + ((uint64_t)B.rows_direct << B.log2w);      // first binned row: bin << log2S indexes from here
 
     for (uint64_t r = 0; r < rounds; ++r) {
         if (threadIdx.x == 0) *qlen = 0;                               // last read before the previous barrier
-        const uint64_t g = r * per_round + (uint64_t)blockIdx.x * BIN_THREADS + threadIdx.x;
+        const uint64_t g = r * per_round + (uint64_t)blockIdx.x * NT + threadIdx.x;
         if (g < pairs) {
             const float2 q0 = ld_stream8(body + 3 * g);
             const float2 q1 = ld_stream8(body + 3 * g + 1);
@@ -180,7 +182,7 @@ k_bin_scatter(const __grid_constant__ PassParams P, const __grid_constant__ BinP
         }
         __syncthreads();
         /* queue the bins that hold at least one full unit */
-        for (uint32_t b0 = warp * 32; b0 < B.nb; b0 += BIN_THREADS) {
+        for (uint32_t b0 = warp * 32; b0 < B.nb; b0 += NT) {
             const uint32_t bin = b0 + lane;
             const bool full = bin < B.nb && cnt[bin] >= UNIT;
             const uint32_t m = __ballot_sync(0xFFFFFFFFu, full);
@@ -194,7 +196,7 @@ k_bin_scatter(const __grid_constant__ PassParams P, const __grid_constant__ BinP
         __syncthreads();
         /* flush: groups of 4 lanes, one queued bin each */
         const uint32_t nq = *qlen;
-        for (uint32_t e0 = warp * 8; e0 < nq; e0 += (BIN_THREADS / 32) * 8) {
+        for (uint32_t e0 = warp * 8; e0 < nq; e0 += (NT / 32) * 8) {
             const uint32_t e = e0 + grp;
             const bool on = e < nq;
             uint32_t bin = 0, c = 0, units = 0, base = 0;
@@ -232,7 +234,7 @@ k_bin_scatter(const __grid_constant__ PassParams P, const __grid_constant__ BinP
         __syncthreads();
     }
     /* partial buffers (< 32 records per bin): applied directly */
-    for (uint32_t bin = threadIdx.x; bin < B.nb; bin += BIN_THREADS) {
+    for (uint32_t bin = threadIdx.x; bin < B.nb; bin += NT) {
         const uint32_t c = min(cnt[bin], B.C);
         for (uint32_t i = 0; i < c; ++i) apply_direct(T, bin, B.log2S, buf[bin * B.C + i]);
     }
@@ -294,7 +296,10 @@ static cudaError_t launch_scatter_r(const PassParams& P, const BinParams& B, con
 #define CS_SCATTER(HM)                                                                                          \
     e = cudaFuncSetAttribute(k_bin_scatter<R, HM>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);     \
     if (e != cudaSuccess) return e;                                                                             \
-    k_bin_scatter<R, HM><<<sm_count, BIN_THREADS, smem, st>>>(P, B, xyz, n, head, pairs);
+    { int per_sm = 0;                                                                                         \
+      cudaOccupancyMaxActiveBlocksPerMultiprocessor(&per_sm, k_bin_scatter<R, HM>, (int)B.threads, smem);       \
+      if (per_sm < 1) per_sm = 1;                                                                               \
+      k_bin_scatter<R, HM><<<sm_count * per_sm, B.threads, smem, st>>>(P, B, xyz, n, head, pairs); }
     if (hm == 0) { CS_SCATTER(0) } else if (hm == 1) { CS_SCATTER(1) } else { CS_SCATTER(2) }
 #undef CS_SCATTER
     return cudaGetLastError();
@@ -317,14 +322,12 @@ cudaError_t launch_update_binned(const PassParams& P, const BinParams& B, const 
         default: return cudaErrorInvalidValue;
     }
     if (e != cudaSuccess) return e;
-    const uint32_t first = (uint32_t)B.rows_direct << (B.log2w - B.log2S);      // bins of direct rows stay empty
-    if (first >= B.nb) return cudaSuccess;
+    if (B.nb == 0) return cudaSuccess;                                       // every row of the pass is direct
     const size_t smem = (size_t)4 << B.log2S;
     e = cudaFuncSetAttribute(k_bin_apply, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
     if (e != cudaSuccess) return e;
-    k_bin_apply<<<B.nb - first, BIN_THREADS, smem, st>>>(P.sc[0].T + ((uint64_t)first << B.log2S),
-                                                         B.bins + (uint64_t)first * B.cap, B.cursor + first, B.cap,
-                                                         B.log2S);
+    k_bin_apply<<<B.nb, BIN_THREADS, smem, st>>>(P.sc[0].T + ((uint64_t)B.rows_direct << B.log2w), B.bins, B.cursor, B.cap,
+                                                 B.log2S);
     return cudaGetLastError();
 }
 

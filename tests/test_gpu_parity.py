@@ -37,7 +37,7 @@ def _ids(t):
 
 
 def _check_all(cs, wl, xyz, sample_p=1.0, k=None, thresholds=(), probe_cells=4096, split=None, cap=None, budget=None,
-               mode=None):
+               mode=None, scan_mode=None):
     """Update + estimate + scan + top-k (+ excursion) on both sides; everything must be identical."""
     k = wl.k if k is None else k
     host = xyz.cpu().numpy()
@@ -47,6 +47,8 @@ def _check_all(cs, wl, xyz, sample_p=1.0, k=None, thresholds=(), probe_cells=409
         g.set_table_budget(budget)
     if mode is not None:
         g.set_update_mode(*mode)
+    if scan_mode is not None:
+        g.set_scan_mode(scan_mode)
     n = host.shape[0]
     cuts = [0, n] if not split else [0] + sorted(split) + [n]
     for a, b in zip(cuts[:-1], cuts[1:]):
@@ -154,9 +156,10 @@ def test_cfg5_reduced_multiscale_sampled(cs):
 
 @pytest.mark.parametrize("rows_fit", [1, 2, 4, 6])
 def test_row_partitioned_update_and_staged_scan(cs, rows_fit):
-    """Budget of 1 / 2 / 4 / 6 rows of a d = 7 sketch: update in row groups, scan as a pipeline of stages."""
+    """Budget of 1 / 2 / 4 / 6 rows of a d = 7 sketch: update in row groups, scan as a pipeline of stages
+    (plain scan mode: the bitmap prefilter would take over as soon as tau >= 1)."""
     wl, xyz = _gen("cfg3", (1 << 21) + 5, w=1 << 16)
-    st = _check_all(cs, wl, xyz, k=2000, thresholds=(6,), budget=rows_fit * wl.w * 4)
+    st = _check_all(cs, wl, xyz, k=2000, thresholds=(6,), budget=rows_fit * wl.w * 4, mode=(1, 0), scan_mode=1)
     assert st["scan_launches"] >= 1
 
 
@@ -164,7 +167,7 @@ def test_row_partitioned_update_and_staged_scan(cs, rows_fit):
 def test_budget_splits_scales(cs, budget_rows):
     """4 scales x 5 rows: budget below one scale (staged per scale), one scale, two scales (scale groups)."""
     wl, xyz = _gen("cfg5", 1 << 21, w=1 << 14)
-    _check_all(cs, wl, xyz, sample_p=0.25, k=500, thresholds=(4,), budget=budget_rows * wl.w * 4)
+    _check_all(cs, wl, xyz, sample_p=0.25, k=500, thresholds=(4,), budget=budget_rows * wl.w * 4, scan_mode=1)
 
 
 def test_staged_scan_even_d_and_many_rows(cs):
@@ -220,6 +223,31 @@ def test_binned_update_single_cell_overflows_bin_region(cs):
     pos = np.full((2000001, 3), 3.3, dtype=np.float32)
     wl = synth.Workload("one", N=len(pos), G=(32,), d=7, w=1 << 16, k=10, H=1, f_bg=0.0, m_min=0, L=10.0)
     _check_all(cs, wl, torch.from_numpy(pos).cuda(), k=10, cap=4096, mode=(2, 0))
+
+
+# ---- bitmap-prefiltered scan (csrc/cs_scan_bitmap.cu) against the plain scan paths ---------------------------------
+
+@pytest.mark.parametrize("scan_mode", [2, 1])
+def test_scan_modes_cfg3_shape(cs, scan_mode):
+    """Same stream through the bitmap prefilter (auto) and through the plain early-exit estimate."""
+    wl, xyz = _gen("cfg3", (1 << 22) + 3)
+    st = _check_all(cs, wl, xyz, k=3000, thresholds=(12, 20), scan_mode=scan_mode, split=[777777])
+    assert st["tau"] >= 1
+
+
+def test_bitmap_scan_excursion_only_and_low_thresholds(cs):
+    """k_max = 0 with thr_min >= 1: the bitmap is used from the first particle; thr_min <= 0: never (all cells pass)."""
+    wl, xyz = _gen("cfg1", 1 << 19)
+    _check_all(cs, wl, xyz, k=0, thresholds=(3, 30), scan_mode=2)
+    _check_all(cs, wl, xyz, k=0, thresholds=(0, 5), scan_mode=2)
+    _check_all(cs, wl, xyz, k=0, thresholds=(-4,), cap=1 << 20, scan_mode=2)
+
+
+def test_bitmap_scan_even_d_many_rows_and_wide_tables(cs):
+    from paper_1711_00975_b200 import synth
+    for d, w, G in ((4, 1 << 12, 700), (12, 1 << 10, 90), (32, 1 << 9, 5000), (6, 1 << 18, 1 << 20)):
+        wl = synth.Workload("bm", N=150001, G=(G,), d=d, w=w, k=300, H=32, f_bg=0.3, m_min=0, L=50.0, seed=d, gen_seed=d + 5)
+        st = _check_all(cs, wl, synth.generate(wl, device="cuda"), thresholds=(2,), probe_cells=256, scan_mode=2)
 
 
 # ---- randomised small configs and edge cases ------------------------------------------------------------------
