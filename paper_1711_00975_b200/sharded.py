@@ -52,10 +52,11 @@ def merge_topk(engine, k: int, dist, world: int):
 
 
 def sharded_pass(engine, xyz_shard, index0: int, sample_p: float, k: int, thr_min: int, dist=None, world: int = 1,
-                 update=None, scan=None):
+                 update=None, scan=None, topk_device=None):
     """reset -> update(shard) -> [all-reduce tables] -> re-scan(shard) -> [merge top-k]; returns per-scale (ids, est).
 
-    `update` / `scan` override the engine methods used for the two passes (the host-streamed variants)."""
+    `update` / `scan` override the engine methods used for the two passes (the host-streamed variants);
+    `topk_device` ("cpu") makes the single-rank result land in host memory."""
     engine.reset()
     engine.set_update_index(index0)
     (update or engine.update)(xyz_shard, sample_p)
@@ -66,4 +67,6 @@ def sharded_pass(engine, xyz_shard, index0: int, sample_p: float, k: int, thr_mi
     (scan or engine.scan)(xyz_shard, sample_p)
     if world > 1:
         return merge_topk(engine, k, dist, world)
+    if topk_device is not None:
+        return [engine.topk(k, s, device=topk_device) for s in range(engine.n_scales)]
     return [engine.topk(k, s) for s in range(engine.n_scales)]
