@@ -33,7 +33,7 @@ CPU_BASELINE_SAMPLE = 1 << 23  # particles of the cpu_baseline leg (about 10-30 
 
 # dram__bytes_read.sum + dram__bytes_write.sum of one k_update launch from the committed `ncu --set full`
 # capture (profiles/), keyed by workload; None until a capture exists for that workload.
-NCU_TRAFFIC_BYTES = {}
+NCU_TRAFFIC_BYTES = {"cfg3": 39.7e9}     # profiles/r1_kernels_cfg3.md: 8 x (scatter + apply) launches per step
 
 
 def _peaks():

@@ -100,6 +100,7 @@ struct cs_sketch {
     uint64_t n_scan_launches = 0;
     double rate = 1.0;
     bool first_chunk = true;
+    uint64_t scanned = 0;              /* particles scanned since cs_scan_begin */
     ScanState* st_dev = nullptr;      /* CS_MAX_SCALES entries */
     ScanState* st_host = nullptr;     /* pinned mirror */
     uint32_t* word_dev = nullptr;     /* 1 scratch word */
@@ -478,8 +479,9 @@ bool wants_compaction(const cs_sketch* s, int i) {
     const uint32_t c = s->st_host[i].count;
     uint64_t base = s->last_compact[i];
     if (base < s->k_max) base = s->k_max;
-    if (base < 65536) base = 65536;
-    return s->dirty[i] && (c > s->cap / 2 || c >= 2 * base);
+    if (base < 8192) base = 8192;
+    /* compacting raises tau (the k_max-th estimate seen so far), which sharpens every later chunk's filter */
+    return s->dirty[i] && (c > s->cap / 2 || 2 * (uint64_t)c >= 3 * base);
 }
 
 /* Replay n device-resident particles against the tables, collecting candidates.
@@ -518,6 +520,8 @@ int scan_device(cs_sketch* s, const float* xyz, uint64_t n, double sample_p) {
         if (s->first_chunk && s->k_max) {                /* a small first chunk fixes a first tau cheaply */
             uint64_t c0 = 8 * s->k_max > (1u << 18) ? 8 * s->k_max : (1u << 18);
             if (chunk > c0) chunk = c0;
+        } else if (s->k_max && chunk > 4 * s->scanned) {  /* tau still rises fast: grow geometrically, not at once */
+            chunk = 4 * s->scanned;
         }
         if (chunk > n - done) chunk = n - done;
         if (chunk < n - done) chunk &= ~(uint64_t)3;     /* keep the 16-byte phase of the remaining stream */
@@ -566,6 +570,7 @@ int scan_device(cs_sketch* s, const float* xyz, uint64_t n, double sample_p) {
             if (chunk > free_min) chunk = free_min & ~3u;
         }
         done += chunk;
+        s->scanned += chunk;
         s->first_chunk = false;
         bool any = false;
         for (int i = 0; i < s->n_scales; ++i)
@@ -896,7 +901,7 @@ int cs_scan_begin(cs_sketch* s, uint64_t k_max, int32_t thr_min) {
         if (rc) return rc;
     }
     s->k_max = k_max; s->thr_min = thr_min;
-    s->scan_index = 0; s->rate = 1.0; s->first_chunk = true; s->n_scan_launches = 0;
+    s->scan_index = 0; s->rate = 1.0; s->first_chunk = true; s->n_scan_launches = 0; s->scanned = 0;
     for (int i = 0; i < CS_MAX_SCALES; ++i) s->bm_valid[i] = false;    /* the tables may have changed */
     for (int i = 0; i < s->n_scales; ++i) {
         s->st_host[i].count = 0;
