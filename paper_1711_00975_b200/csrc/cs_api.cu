@@ -122,6 +122,10 @@ struct cs_sketch {
     int32_t tau_bm[CS_MAX_SCALES] = {};
     bool bm_valid[CS_MAX_SCALES] = {};
 
+    /* dense buffer of kept particles for strongly sampled streams (k_compact_kept) */
+    float* kept = nullptr;
+    uint64_t kept_cap = 0;             /* particles */
+
     /* survivor lists of the row-partitioned scan */
     StageBuffers stb = {};
 
@@ -335,7 +339,7 @@ int update_binned(cs_sketch* s, const BinPlan& pl, const float* xyz, uint64_t n,
  * the d rows of each scale are split into groups of at most table_budget bytes and the positions are re-read
  * once per group (12 B/particle at HBM rate, far cheaper than DRAM-backed atomics).  Each group is the same
  * kernel with a PassParams that names only that group's rows and tables. */
-int update_passes(cs_sketch* s, const float* xyz, uint64_t n, uint64_t index0, double sample_p) {
+int update_passes_raw(cs_sketch* s, const float* xyz, uint64_t n, uint64_t index0, double sample_p) {
     BinPlan pl;
     if (s->update_mode != 1 && (s->update_mode == 2 || n >= BIN_MIN_N) && bin_plan(s, &pl))
         return update_binned(s, pl, xyz, n, index0, sample_p);
@@ -487,7 +491,7 @@ bool wants_compaction(const cs_sketch* s, int i) {
 /* Replay n device-resident particles against the tables, collecting candidates.
  * Invariant that makes overflow impossible on a retry: a chunk of at most `free` particles cannot append more
  * than `free` entries to any scale. */
-int scan_device(cs_sketch* s, const float* xyz, uint64_t n, double sample_p) {
+int scan_device_raw(cs_sketch* s, const float* xyz, uint64_t n, double sample_p) {
     uint64_t done = 0;
     while (done < n) {
         uint32_t free_min = s->cap;
@@ -587,6 +591,70 @@ int scan_device(cs_sketch* s, const float* xyz, uint64_t n, double sample_p) {
         }
     }
     s->scan_index += n;
+    return CS_OK;
+}
+
+/* ---- strongly sampled streams: compact the kept particles once, then run every pass on them ------------------ */
+
+constexpr double COMPACT_BELOW_P = 0.5;               /* sample_p below which compaction pays */
+constexpr uint64_t COMPACT_MIN_N = 1ull << 20;
+constexpr uint64_t COMPACT_CHUNK = 1ull << 28;
+
+/* Kept particles of xyz[0..m) (running index index0) -> s->kept; *cnt = their number, or UINT64_MAX if they did not
+ * fit (the caller then takes the sampling-in-kernel path for this chunk). */
+int compact_chunk(cs_sketch* s, const float* xyz, uint64_t m, uint64_t index0, double sample_p, uint64_t* cnt) {
+    const uint64_t want = (uint64_t)((double)(m < COMPACT_CHUNK ? m : COMPACT_CHUNK) * sample_p * 1.05) + 65536;
+    if (s->kept_cap < want) {
+        CS_CUDA(cudaStreamSynchronize(s->stream));
+        if (s->kept) cudaFree(s->kept);
+        s->kept = nullptr; s->kept_cap = 0;
+        CS_CUDA(cudaMalloc(&s->kept, want * 12));
+        s->kept_cap = want;
+    }
+    CS_CUDA(cudaMemsetAsync(s->word_dev, 0, 4, s->stream));
+    cudaError_t e = launch_compact_kept(xyz, m, index0, s->K, sample_threshold(sample_p), s->kept, s->word_dev,
+                                        (uint32_t)(s->kept_cap < 0xFFFFFFFFull ? s->kept_cap : 0xFFFFFFFFull), s->sm_count,
+                                        s->stream);
+    if (e != cudaSuccess) return fail(CS_ERR_CUDA, "compaction kernel: %s", cudaGetErrorString(e));
+    s->launches += 1;
+    CS_CUDA(cudaMemcpyAsync(s->word_host, s->word_dev, 4, cudaMemcpyDeviceToHost, s->stream));
+    CS_CUDA(cudaStreamSynchronize(s->stream));
+    *cnt = *s->word_host <= s->kept_cap ? *s->word_host : UINT64_MAX;
+    return CS_OK;
+}
+
+bool wants_compaction_of_stream(uint64_t n, double sample_p) { return sample_p < COMPACT_BELOW_P && n >= COMPACT_MIN_N; }
+
+int update_passes(cs_sketch* s, const float* xyz, uint64_t n, uint64_t index0, double sample_p) {
+    if (!wants_compaction_of_stream(n, sample_p)) return update_passes_raw(s, xyz, n, index0, sample_p);
+    for (uint64_t off = 0; off < n; off += COMPACT_CHUNK) {
+        const uint64_t m = n - off < COMPACT_CHUNK ? n - off : COMPACT_CHUNK;
+        uint64_t cnt = 0;
+        int rc = compact_chunk(s, xyz + 3 * off, m, index0 + off, sample_p, &cnt);
+        if (rc) return rc;
+        if (cnt == UINT64_MAX) rc = update_passes_raw(s, xyz + 3 * off, m, index0 + off, sample_p);
+        else if (cnt)          rc = update_passes_raw(s, s->kept, cnt, 0, 1.0);
+        if (rc) return rc;
+    }
+    return CS_OK;
+}
+
+int scan_device(cs_sketch* s, const float* xyz, uint64_t n, double sample_p) {
+    if (!wants_compaction_of_stream(n, sample_p)) return scan_device_raw(s, xyz, n, sample_p);
+    for (uint64_t off = 0; off < n; off += COMPACT_CHUNK) {
+        const uint64_t m = n - off < COMPACT_CHUNK ? n - off : COMPACT_CHUNK;
+        uint64_t cnt = 0;
+        int rc = compact_chunk(s, xyz + 3 * off, m, s->scan_index, sample_p, &cnt);
+        if (rc) return rc;
+        if (cnt == UINT64_MAX) {
+            rc = scan_device_raw(s, xyz + 3 * off, m, sample_p);       /* advances scan_index by m itself */
+        } else {
+            const uint64_t next = s->scan_index + m;
+            if (cnt) rc = scan_device_raw(s, s->kept, cnt, 1.0);       /* p = 1: the index is not used */
+            s->scan_index = next;
+        }
+        if (rc) return rc;
+    }
     return CS_OK;
 }
 
@@ -768,6 +836,7 @@ int cs_destroy(cs_sketch* s) {
     free_stage_lists(s);
     if (s->bins) cudaFree(s->bins);
     if (s->cursor) cudaFree(s->cursor);
+    if (s->kept) cudaFree(s->kept);
     for (int i = 0; i < CS_MAX_SCALES; ++i) if (s->bm[i]) cudaFree(s->bm[i]);
     for (int i = 0; i < CS_MAX_SCALES; ++i) if (s->T[i]) cudaFree(s->T[i]);
     if (s->st_dev) cudaFree(s->st_dev);

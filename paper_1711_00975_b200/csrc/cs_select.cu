@@ -45,28 +45,50 @@ k_hist(const uint64_t* __restrict__ id, const uint32_t* __restrict__ ek, uint32_
     counts[threadIdx.x * nblocks + blockIdx.x] = h[threadIdx.x];
 }
 
-/* In-place exclusive prefix sum of a[0..len) by one block of 1024 threads; *total_out (optional) = sum. */
+/* In-place exclusive prefix sum of a[0..len) by one block of 1024 threads; *total_out (optional) = sum.
+ * Tiles of 4096 words: coalesced 4-word loads per thread, warp-shuffle scans, a running carry between tiles. */
 __global__ void __launch_bounds__(1024) k_exscan(uint32_t* __restrict__ a, uint32_t len, uint32_t* total_out) {
-    __shared__ uint32_t part[1024];
-    const uint32_t per = (len + 1023u) / 1024u;
-    const uint32_t lo = min(threadIdx.x * per, len), hi = min(lo + per, len);
-    uint32_t s = 0;
-    for (uint32_t i = lo; i < hi; ++i) s += a[i];
-    part[threadIdx.x] = s;
+    __shared__ uint32_t wsum[32];
+    __shared__ uint32_t s_carry;
+    const uint32_t lane = threadIdx.x & 31u, warp = threadIdx.x >> 5;
+    if (threadIdx.x == 0) s_carry = 0;
     __syncthreads();
-    for (int off = 1; off < 1024; off <<= 1) {               // Hillis-Steele inclusive scan
-        uint32_t v = threadIdx.x >= off ? part[threadIdx.x - off] : 0;
+    for (uint32_t t0 = 0; t0 < len; t0 += 4096) {
+        const uint32_t i = t0 + threadIdx.x * 4;
+        uint32_t v[4];
+#pragma unroll
+        for (int k = 0; k < 4; ++k) v[k] = i + k < len ? a[i + k] : 0;
+        const uint32_t mine = v[0] + v[1] + v[2] + v[3];
+        uint32_t incl = mine;
+#pragma unroll
+        for (int off = 1; off < 32; off <<= 1) {
+            const uint32_t u = __shfl_up_sync(0xFFFFFFFFu, incl, off);
+            if (lane >= off) incl += u;
+        }
+        if (lane == 31) wsum[warp] = incl;
         __syncthreads();
-        part[threadIdx.x] += v;
+        if (warp == 0) {
+            uint32_t w = wsum[lane], wi = w;
+#pragma unroll
+            for (int off = 1; off < 32; off <<= 1) {
+                const uint32_t u = __shfl_up_sync(0xFFFFFFFFu, wi, off);
+                if (lane >= off) wi += u;
+            }
+            wsum[lane] = wi - w;                                   // exclusive prefix of the warp totals
+        }
+        __syncthreads();
+        const uint32_t carry = s_carry;
+        uint32_t run = carry + wsum[warp] + incl - mine;
+#pragma unroll
+        for (int k = 0; k < 4; ++k) {
+            if (i + k < len) a[i + k] = run;
+            run += v[k];
+        }
+        __syncthreads();
+        if (threadIdx.x == 1023) s_carry = run;                    // total up to the end of this tile
         __syncthreads();
     }
-    uint32_t run = threadIdx.x ? part[threadIdx.x - 1] : 0;
-    for (uint32_t i = lo; i < hi; ++i) {
-        uint32_t v = a[i];
-        a[i] = run;
-        run += v;
-    }
-    if (total_out && threadIdx.x == 1023) *total_out = part[1023];
+    if (total_out && threadIdx.x == 0) *total_out = s_carry;
 }
 
 /* Stable scatter of one radix pass.  Warp wq owns entries [t0 + wq*SORT_SEG, +SORT_SEG) in order; within a
