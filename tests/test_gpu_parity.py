@@ -395,3 +395,54 @@ def test_call_order_and_argument_errors(cs):
     assert len(ids) == 5
     assert g.launch_count() > 0
     g.close()
+
+
+# ---- BASELINE.json full size (cfg 3: 2^30 particles), in the launch configuration bench.py times ------------------
+
+def test_cfg3_full_size_properties(cs):
+    """The oracle cannot replay 2^30 particles in test time, so this checks what holds at any size: row parity
+    and mass invariants of the table, linearity (two half-stream handles sum to the whole-stream table,
+    PAPER.md:578), update-mode independence on a 2^27 prefix (direct vs binned kernels), and that the top-k is
+    sorted by (estimate desc, id asc), duplicate-free, consistent with cs_estimate and closed under the cut:
+    no sampled occupied cell outside the list beats its last entry."""
+    free, _total = torch.cuda.mem_get_info()
+    if free < 48 << 30:
+        pytest.skip("needs ~40 GB of free device memory")
+    wl, xyz = _gen("cfg3")
+    n = wl.N
+    g = cs.CountSketch(wl.d, wl.w, list(wl.G), wl.L, wl.seed)
+    g.update(xyz)
+    T = g.sketch()
+    assert bool(((T.sum(dim=1) - n) % 2 == 0).all()), "row sums must have the parity of n"
+    assert bool((T.abs().to(torch.int64).sum(dim=1) <= n).all())
+    # linearity: halves through separate handles (second half through the host-visible merge call)
+    a = cs.CountSketch(wl.d, wl.w, list(wl.G), wl.L, wl.seed)
+    a.update(xyz[: n // 2 + 1])
+    b = cs.CountSketch(wl.d, wl.w, list(wl.G), wl.L, wl.seed)
+    b.update(xyz[n // 2 + 1:])
+    a.sketch_add(b.sketch())
+    assert torch.equal(a.sketch(), T), "sketch(A ++ B) != sketch(A) + sketch(B)"
+    b.close()
+    # the two update routes give the same table on a prefix
+    a.reset(); a.set_update_mode(1, 0); a.update(xyz[: 1 << 27]); Td = a.sketch()
+    a.reset(); a.set_update_mode(2, 0); a.update(xyz[: 1 << 27])
+    assert torch.equal(a.sketch(), Td), "direct and binned updates differ"
+    a.close()
+    del Td
+    g.scan_begin(wl.k)
+    g.scan(xyz)
+    ids, est = g.topk(wl.k)
+    assert ids.numel() == wl.k
+    assert torch.equal(g.estimate(ids), est), "top-k estimates differ from cs_estimate"
+    e64, i64 = est.to(torch.int64), ids
+    ok = (e64[:-1] > e64[1:]) | ((e64[:-1] == e64[1:]) & (i64[:-1] < i64[1:]))
+    assert bool(ok.all()), "top-k not in (estimate desc, id asc) order or has duplicates"
+    # closure: cells of a 2^22-particle sample that are not in the list must rank after its last entry
+    host = xyz[: 1 << 22].cpu().numpy()
+    cells = torch.from_numpy(np.unique(ora.quantise(host, wl.G[0], wl.L)).view(np.int64)).cuda()
+    ce = g.estimate(cells).to(torch.int64)
+    inlist = torch.isin(cells, ids)
+    last_e, last_i = int(est[-1]), int(ids[-1])
+    beats = (ce > last_e) | ((ce == last_e) & (cells < last_i))
+    assert not bool((beats & ~inlist).any()), "an occupied cell outside the top-k beats its last entry"
+    g.close()
