@@ -385,7 +385,7 @@ def main():
     ap.add_argument("--e2e-steps", type=int, default=2)
     ap.add_argument("--no-e2e", action="store_true")
     ap.add_argument("--no-cpu-baseline", action="store_true")
-    ap.add_argument("--scan-mode", type=int, default=0, help="cs_set_scan_mode: 0 auto (bitmap prefilter), 1 plain")
+    ap.add_argument("--scan-mode", type=int, default=0, help="cs_set_scan_mode: 0 auto, 1 plain, 2 bitmap, 3 bitmap stages")
     ap.add_argument("--update-mode", type=int, default=0, help="cs_set_update_mode: 0 auto, 1 direct, 2 binned")
     ap.add_argument("--rows-direct", type=int, default=-1, help="rows of each binned pass that use red.global")
     args = ap.parse_args()

@@ -121,7 +121,10 @@ int cs_set_update_mode(cs_sketch* s, int mode, int rows_direct);
  *   mode 2 "bitmap": once the collection threshold tau is >= 1 (and w is a power of two), a 1-bit-per-counter
  *           bitmap |T| >= tau is built and every cell is first tested against it with the bucket hashes alone
  *           (csrc/cs_scan_bitmap.cu); survivors get the exact estimate.
- *   mode 0 "auto" (default): the faster of the two as measured on the BASELINE shapes (currently plain). */
+ *   mode 3 "bitmap stages": the same bitmap plus a coarse copy of its first (d-1)/2 + 1 rows in shared memory decide
+ *           the first rows; survivors run the remaining rows on dense warps (csrc/cs_scan_staged.cu).  Single-scale
+ *           handles, 2 <= d <= 10, w a power of two >= 4096; else as mode 2.
+ *   mode 0 "auto" (default): mode 3 where it applies, else mode 1. */
 int cs_set_scan_mode(cs_sketch* s, int mode);
 
 /* Running particle index of the update stream / of the current scan (sampling, R13, R17).

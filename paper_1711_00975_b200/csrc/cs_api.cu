@@ -117,10 +117,11 @@ struct cs_sketch {
     uint32_t* cursor = nullptr;        /* BIN_MAX words */
 
     /* bitmap prefilter of the scan (cs_scan_bitmap.cu): B[j][b] = |T[j][b]| >= tau_bm, per scale */
-    int scan_mode = 0;                 /* cs_set_scan_mode: 0 auto, 1 plain, 2 bitmap once tau >= 1 */
+    int scan_mode = 0;                 /* cs_set_scan_mode: 0 auto, 1 plain, 2 bitmap, 3 bitmap first stage */
     uint32_t* bm[CS_MAX_SCALES] = {};
     int32_t tau_bm[CS_MAX_SCALES] = {};
     bool bm_valid[CS_MAX_SCALES] = {};
+    uint32_t* coarse = nullptr;        /* coarse bitmap of scale 0 (bitmap first stage, single-scale handles) */
 
     /* dense buffer of kept particles for strongly sampled streams (k_compact_kept) */
     float* kept = nullptr;
@@ -427,10 +428,13 @@ int launch_scan_chunk(cs_sketch* s, const float* xyz, uint64_t n, uint64_t index
     fill_scan_params(s, &S);
     /* bitmap prefilter: valid once every scale collects against a tau >= 1 (|T| >= tau is then necessary for a row
      * to pass); rebuilt (d*w/8 bytes, microseconds) whenever a compaction has raised tau */
-    bool use_bm = s->scan_mode == 2 && (s->w & (s->w - 1)) == 0;
+    uint32_t cg0 = 0, crw0 = 0;
+    const bool staged_bm = s->n_scales == 1 && coarse_shape(s->d, s->w, &cg0, &crw0);
+    bool use_bm = (s->scan_mode == 2 || s->scan_mode == 3 || (s->scan_mode == 0 && staged_bm)) && (s->w & (s->w - 1)) == 0;
     for (int i = 0; i < s->n_scales && use_bm; ++i) use_bm = s->st_host[i].tau >= 1;
     if (use_bm) {
         const uint64_t counters = (uint64_t)s->d * s->w;
+        bool rebuilt = false;
         for (int i = 0; i < s->n_scales; ++i) {
             if (!s->bm[i]) CS_CUDA(cudaMalloc(&s->bm[i], ((counters + 31) / 32) * sizeof(uint32_t)));
             if (!s->bm_valid[i] || s->tau_bm[i] != s->st_host[i].tau) {
@@ -439,7 +443,23 @@ int launch_scan_chunk(cs_sketch* s, const float* xyz, uint64_t n, uint64_t index
                 s->launches += 1;
                 s->tau_bm[i] = s->st_host[i].tau;
                 s->bm_valid[i] = true;
+                rebuilt = true;
             }
+        }
+        uint32_t cg = 0, crw = 0;
+        if (s->scan_mode != 2 && s->n_scales == 1 && coarse_shape(s->d, s->w, &cg, &crw)) {
+            /* bitmap first stage (coarse bitmap in shared memory) + the remaining rows on dense warps */
+            int rc = ensure_stage_lists(s, n);
+            if (rc) return rc;
+            if (!s->coarse) {
+                CS_CUDA(cudaMalloc(&s->coarse, (size_t)((s->d - 1) / 2 + 1) * crw * sizeof(uint32_t)));
+                rebuilt = true;
+            }
+            cudaError_t ec = launch_scan_staged_cb(full, S.tg[0], s->stb, s->bm[0], s->coarse, cg, crw, rebuilt, xyz, n,
+                                                   s->sm_count, s->stream, &s->launches);
+            if (ec != cudaSuccess) return fail(CS_ERR_CUDA, "bitmap stage kernels: %s", cudaGetErrorString(ec));
+            s->n_scan_launches += 1;
+            return CS_OK;
         }
         cudaError_t eb = launch_scan_bitmap(full, S, s->bm, xyz, n, s->sm_count, s->stream);
         if (eb != cudaSuccess) return fail(CS_ERR_CUDA, "bitmap scan kernel: %s", cudaGetErrorString(eb));
@@ -838,6 +858,7 @@ int cs_destroy(cs_sketch* s) {
     if (s->cursor) cudaFree(s->cursor);
     if (s->kept) cudaFree(s->kept);
     for (int i = 0; i < CS_MAX_SCALES; ++i) if (s->bm[i]) cudaFree(s->bm[i]);
+    if (s->coarse) cudaFree(s->coarse);
     for (int i = 0; i < CS_MAX_SCALES; ++i) if (s->T[i]) cudaFree(s->T[i]);
     if (s->st_dev) cudaFree(s->st_dev);
     if (s->st_host) cudaFreeHost(s->st_host);
@@ -890,7 +911,7 @@ int cs_set_update_mode(cs_sketch* s, int mode, int rows_direct) {
 
 int cs_set_scan_mode(cs_sketch* s, int mode) {
     if (!s) return fail(CS_ERR_ARG, "null handle");
-    if (mode < 0 || mode > 2) return fail(CS_ERR_ARG, "mode must be 0 (auto), 1 (plain) or 2 (bitmap)");
+    if (mode < 0 || mode > 3) return fail(CS_ERR_ARG, "mode must be 0 (auto), 1 (plain), 2 (bitmap) or 3 (bitmap stages)");
     s->scan_mode = mode;
     return CS_OK;
 }

@@ -102,6 +102,10 @@ struct StageBuffers {
 uint64_t staged_list_entries(uint64_t n, uint32_t blocks);
 cudaError_t launch_scan_staged(const PassParams& P, const ScanTarget& tg, const StageBuffers& B, int rows_per_stage,
                                const float* xyz, uint64_t n, cudaStream_t st, uint64_t* launches);
+bool coarse_shape(int d, uint64_t w, uint32_t* g_out, uint32_t* row_words_out);
+cudaError_t launch_scan_staged_cb(const PassParams& P, const ScanTarget& tg, const StageBuffers& B, const uint32_t* fine,
+                                  uint32_t* coarse, uint32_t g, uint32_t row_words, bool rebuild_coarse, const float* xyz,
+                                  uint64_t n, int sm_count, cudaStream_t st, uint64_t* launches);
 cudaError_t launch_scan_cells(const PassParams& P, const ScanParams& S, int scale, const uint64_t* cells,
                               uint64_t m, cudaStream_t st);
 cudaError_t launch_estimate(const PassParams& P, int scale, const uint64_t* cells, uint64_t m, int32_t* est,

@@ -19,17 +19,6 @@
 
 namespace cs {
 
-__device__ __forceinline__ uint32_t ld_bits(const uint32_t* p) {
-    uint32_t v;
-    asm volatile("ld.global.relaxed.gpu.u32 %0, [%1];" : "=r"(v) : "l"(p));
-    return v;
-}
-__device__ __forceinline__ uint64_t lds_u64s(uint32_t addr) {
-    uint64_t v;
-    asm volatile("ld.shared.u64 %0, [%1];" : "=l"(v) : "r"(addr));
-    return v;
-}
-
 /* One thread = one 32-bit word of the bitmap = 32 consecutive counters (n = d*w counters, any multiple or not). */
 __global__ void __launch_bounds__(256)
 k_build_bitmap(const int32_t* __restrict__ T, uint64_t n, int32_t tau, uint32_t* __restrict__ bm) {
@@ -58,13 +47,6 @@ k_build_bitmap(const int32_t* __restrict__ T, uint64_t n, int32_t tau, uint32_t*
         }
         bm[wd] = bits;
     }
-}
-
-/* bucket hash of row rc under hash mode HM (0: c < 2^31; 1: table in shared memory; 2: general two-limb form) */
-template <int HM>
-__device__ __forceinline__ uint32_t bucket_of(const RowCoef& rc, uint32_t c0, uint32_t c1, uint32_t tb_addr, uint32_t wmask) {
-    if (HM == 1) return affine_low32_tb(rc.h, c0, lds_u64s(tb_addr)) & wmask;
-    return affine_low32<HM == 2>(rc.h, c0, c1) & wmask;
 }
 
 /* true iff at most (d-1)/2 rows of cell c are clear in the bitmap of scale s */

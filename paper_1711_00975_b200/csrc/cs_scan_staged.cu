@@ -70,7 +70,8 @@ __device__ __forceinline__ void stage_cell(const PassParams& P, const StageParam
         int32_t est = 0;
         if (live) est = P.sc[0].big ? estimate_all_rows<POW2, true>(P, Q.d_all, c)
                                     : estimate_all_rows<POW2, false>(P, Q.d_all, c);
-        append_candidate(tg, live, c, est);
+        /* with exact fail counts live already implies est >= tau; a bitmap first stage counts conservatively */
+        append_candidate(tg, live && est >= tau, c, est);
     } else {
         const uint32_t mask = __ballot_sync(0xFFFFFFFFu, live);
         if (mask) {
@@ -166,6 +167,159 @@ k_stage_next(const __grid_constant__ PassParams P, const __grid_constant__ Stage
     }
 }
 
+/* ------------------------------------------------------------------------------------------------------------
+ * Bitmap first stage.  Once tau >= 1, a row can only pass if |T[j][h_j(c)]| >= tau.  The first FIRST = (d-1)/2 + 1
+ * rows (which cannot reject on their own) are tested against
+ *   - a coarse bitmap in shared memory: bit i of row j = OR over counters [i*2^g, (i+1)*2^g) of (|T| >= tau); a
+ *     clear bit certifies the row as failed without any L2 request (about 40 % of the rows at cfg 3, g = 4);
+ *   - else the fine bitmap (1 bit per counter, d*w/8 bytes, L2-resident whatever the sketch size), 4-byte gathers.
+ * Only bucket hashes are needed (no sign hashes).  All four particles of a thread are taken through the phases
+ * together, so that up to 4*FIRST gathers per thread are in flight.  Fail counts are conservative (a set bit may
+ * still fail on the sign or the exact value); survivors go to the per-segment lists in the format of k_stage_first
+ * and the remaining rows run in k_stage_next<.., LAST> on dense warps, which re-checks Estimate >= tau exactly.
+ * One CTA of 512 threads per SM walks the segments blockIdx.x, blockIdx.x + gridDim.x, ...
+ * ------------------------------------------------------------------------------------------------------------ */
+
+constexpr int CB_THREADS = 1024;
+
+struct CoarseParams {
+    const uint32_t* fine;      // fine bitmap: bit (j*w + b)
+    const uint32_t* coarse;    // rows 0 .. FIRST-1, row_words words each
+    uint32_t g;                // log2 counters per coarse bit
+    uint32_t row_words;        // (w >> g) / 32
+    uint32_t hm;               // hash mode (0 one limb, 1 table, 2 general)
+    uint32_t nseg;             // segments = grid size of the following stages
+};
+
+template <int FIRST, int HM>
+__device__ __forceinline__ void cb_hashes(const PassParams& P, uint32_t tb_base, uint32_t wmask, const uint64_t* c,
+                                          uint32_t (&h)[2][FIRST]) {
+#pragma unroll
+    for (int q = 0; q < 2; ++q) {
+        const uint32_t c0 = cell_c0(c[q]), c1 = cell_c1(c[q]);
+        const uint32_t tb_addr = tb_base + c1 * (uint32_t)(P.d * 8);                  // tb[c1][j], j < d
+#pragma unroll
+        for (int j = 0; j < FIRST; ++j) h[q][j] = bucket_of<HM>(P.rows[j], c0, c1, tb_addr + j * 8, wmask);
+    }
+}
+
+template <int FIRST>
+__global__ void __launch_bounds__(CB_THREADS, 1)
+k_stage_first_cb(const __grid_constant__ PassParams P, const __grid_constant__ StageParams Q,
+                 const __grid_constant__ CoarseParams C, const float* __restrict__ xyz, uint64_t n, uint32_t head,
+                 uint64_t groups, uint64_t gpb) {
+    extern __shared__ __align__(16) uint32_t cb_smem[];
+    __shared__ uint32_t s_cnt;
+    const uint32_t cwords = (uint32_t)FIRST * C.row_words;                            // a multiple of 4
+    {
+        const uint4* src = reinterpret_cast<const uint4*>(C.coarse);
+        uint4* dst = reinterpret_cast<uint4*>(cb_smem);
+        for (uint32_t i = threadIdx.x; i < cwords / 4; i += CB_THREADS) dst[i] = src[i];
+    }
+    uint64_t* tb = reinterpret_cast<uint64_t*>(cb_smem + cwords);
+    for (uint32_t i = threadIdx.x; i < (uint32_t)(HASH_TB * P.d); i += CB_THREADS)
+        tb[i] = C.hm == 1 ? affine_mod_p<true>(P.rows[i % P.d].h, 0u, i / P.d) + 1 : 0;
+    __syncthreads();
+    const uint32_t cs_addr = (uint32_t)__cvta_generic_to_shared(cb_smem);
+    const uint32_t tb_base = (uint32_t)__cvta_generic_to_shared(tb);
+    const uint32_t wmask = (uint32_t)(P.w - 1);
+    const float4* body = reinterpret_cast<const float4*>(xyz + 3 * (uint64_t)head);
+    const uint32_t lane = threadIdx.x & 31u;
+    const uint32_t below = (1u << lane) - 1u;
+
+    for (uint32_t seg = blockIdx.x; seg < C.nseg; seg += gridDim.x) {
+        if (threadIdx.x == 0) s_cnt = 0;
+        __syncthreads();
+        uint64_t* out = Q.out + (uint64_t)seg * Q.seg_cap;
+        const uint64_t g_lo = (uint64_t)seg * gpb;
+        const uint64_t g_hi = g_lo + gpb < groups ? g_lo + gpb : groups;
+        for (uint64_t g0 = g_lo + (threadIdx.x - lane); g0 < g_hi; g0 += CB_THREADS) {
+            const uint64_t g = g0 + lane;
+            const bool in = g < g_hi;
+            float4 q0 = make_float4(0.f, 0.f, 0.f, 0.f), q1 = q0, q2 = q0;
+            if (in) {
+                q0 = ld_stream16(body + 3 * g);
+                q1 = ld_stream16(body + 3 * g + 1);
+                q2 = ld_stream16(body + 3 * g + 2);
+            }
+            bool keep[4] = {in, in, in, in};
+            if (P.sample && in) {
+                const uint64_t i0 = P.index0 + head + 4 * g;
+#pragma unroll
+                for (int q = 0; q < 4; ++q) keep[q] = keep_particle(P.K, i0 + q, P.Tp);
+            }
+            uint64_t c[4];
+            c[0] = cell_of(q0.x, q0.y, q0.z, P.sc[0]);
+            c[1] = cell_of(q0.w, q1.x, q1.y, P.sc[0]);
+            c[2] = cell_of(q1.z, q1.w, q2.x, P.sc[0]);
+            c[3] = cell_of(q2.y, q2.z, q2.w, P.sc[0]);
+            /* two particles at a time (64 registers per thread at 1024 threads): hashes, coarse bits from shared
+             * memory, then the fine words of the undecided rows, all in flight together */
+#pragma unroll
+            for (int half = 0; half < 2; ++half) {
+                uint32_t h[2][FIRST];
+                if (C.hm == 0)      cb_hashes<FIRST, 0>(P, tb_base, wmask, c + 2 * half, h);
+                else if (C.hm == 1) cb_hashes<FIRST, 1>(P, tb_base, wmask, c + 2 * half, h);
+                else                cb_hashes<FIRST, 2>(P, tb_base, wmask, c + 2 * half, h);
+                uint32_t wd[2][FIRST];
+#pragma unroll
+                for (int q = 0; q < 2; ++q)
+#pragma unroll
+                    for (int j = 0; j < FIRST; ++j) {
+                        const uint32_t i = h[q][j] >> C.g;
+                        wd[q][j] = (lds_u32s(cs_addr + ((uint32_t)j * C.row_words + (i >> 5)) * 4u) >> (i & 31u)) & 1u;
+                    }
+#pragma unroll
+                for (int q = 0; q < 2; ++q)
+#pragma unroll
+                    for (int j = 0; j < FIRST; ++j) {
+                        uint32_t w = 0;
+                        if (keep[2 * half + q] && wd[q][j]) w = ld_bits(C.fine + (((uint64_t)j * P.w + h[q][j]) >> 5));
+                        wd[q][j] = w;
+                    }
+#pragma unroll
+                for (int q = 0; q < 2; ++q) {
+                    uint32_t fails = 0;
+#pragma unroll
+                    for (int j = 0; j < FIRST; ++j) fails += 1u - ((wd[q][j] >> (h[q][j] & 31u)) & 1u);
+                    const bool live = keep[2 * half + q] && fails < (uint32_t)FIRST;  // FIRST fails = more than (d-1)/2
+                    const uint32_t mask = __ballot_sync(0xFFFFFFFFu, live);
+                    if (mask) {
+                        const int leader = __ffs(mask) - 1;
+                        uint32_t base = 0;
+                        if ((int)lane == leader) base = atomicAdd(&s_cnt, (uint32_t)__popc(mask));
+                        base = __shfl_sync(0xFFFFFFFFu, base, leader);
+                        if (live) out[base + __popc(mask & below)] = c[2 * half + q] | ((uint64_t)fails << FAIL_SHIFT);
+                    }
+                }
+            }
+        }
+        if (seg == 0 && threadIdx.x < 32) {           // the <= 6 edge particles: passed on undecided (fails = 0)
+            const uint64_t tail0 = (uint64_t)head + 4 * groups;
+            const uint64_t n_edge = (uint64_t)head + (n - tail0);
+            bool keep = false;
+            uint64_t c = 0;
+            if (threadIdx.x < n_edge) {
+                const uint64_t i = threadIdx.x < head ? threadIdx.x : tail0 + (threadIdx.x - head);
+                keep = !P.sample || keep_particle(P.K, P.index0 + i, P.Tp);
+                const float* p = xyz + 3 * i;
+                c = cell_of(ld_stream4(p), ld_stream4(p + 1), ld_stream4(p + 2), P.sc[0]);
+            }
+            const uint32_t mask = __ballot_sync(0xFFFFFFFFu, keep);
+            if (mask) {
+                const int leader = __ffs(mask) - 1;
+                uint32_t base = 0;
+                if ((int)lane == leader) base = atomicAdd(&s_cnt, (uint32_t)__popc(mask));
+                base = __shfl_sync(0xFFFFFFFFu, base, leader);
+                if (keep) out[base + __popc(mask & below)] = c;
+            }
+        }
+        __syncthreads();
+        if (threadIdx.x == 0) Q.cnt_out[seg] = s_cnt;
+        __syncthreads();
+    }
+}
+
 /* ---- host side ------------------------------------------------------------------------------------------ */
 
 template <int R, bool POW2, bool LAST>
@@ -235,6 +389,90 @@ cudaError_t launch_scan_staged(const PassParams& P, const ScanTarget& tg, const 
         *launches += 1;
         cur ^= 1;
     }
+    return cudaGetLastError();
+}
+
+/* coarse word cw: bit b = OR of the fine bits [(cw*32 + b) << g, +2^g) */
+__global__ void __launch_bounds__(256)
+k_build_coarse(const uint32_t* __restrict__ fine, uint64_t n_coarse_words, int g, uint32_t* __restrict__ coarse) {
+    const uint64_t stride = (uint64_t)gridDim.x * blockDim.x;
+    for (uint64_t cw = (uint64_t)blockIdx.x * blockDim.x + threadIdx.x; cw < n_coarse_words; cw += stride) {
+        uint32_t bits = 0;
+        for (int b = 0; b < 32; ++b) {
+            const uint64_t start = (cw * 32 + b) << g;
+            uint32_t any = 0;
+            if (g >= 5) {
+                for (uint64_t k = 0; k < (1ull << (g - 5)); ++k) any |= fine[(start >> 5) + k];
+            } else {
+                any = (fine[start >> 5] >> (start & 31u)) & (g == 0 ? 1u : ((1u << (1u << g)) - 1u));
+            }
+            bits |= (uint32_t)(any != 0) << b;
+        }
+        coarse[cw] = bits;
+    }
+}
+
+/* Group size 2^g of the coarse bitmap: the smallest whose FIRST rows fit the shared-memory budget.
+ * false: shape not supported by the bitmap first stage (the caller uses the plain stages). */
+bool coarse_shape(int d, uint64_t w, uint32_t* g_out, uint32_t* row_words_out) {
+    const int first = (d - 1) / 2 + 1, rest = d - first;
+    if (first > 5 || rest < 1 || rest > 8 || (w & (w - 1)) || w < 4096) return false;
+    for (uint32_t g = 0; g <= 8; ++g) {
+        if ((w >> g) < 128) break;
+        if ((uint64_t)first * ((w >> g) / 8) <= 190 * 1024) {
+            *g_out = g;
+            *row_words_out = (uint32_t)((w >> g) / 32);
+            return true;
+        }
+    }
+    return false;
+}
+
+/* fine: bitmap of the scale (bit j*w + b), already built for the current tau; coarse: scratch of FIRST*row_words words */
+cudaError_t launch_scan_staged_cb(const PassParams& P, const ScanTarget& tg, const StageBuffers& B, const uint32_t* fine,
+                                  uint32_t* coarse, uint32_t g, uint32_t row_words, bool rebuild_coarse, const float* xyz,
+                                  uint64_t n, int sm_count, cudaStream_t st, uint64_t* launches) {
+    const int first = (P.d - 1) / 2 + 1, rest = P.d - first;
+    if (rebuild_coarse) {
+        const uint64_t words = (uint64_t)first * row_words;
+        uint64_t blocks = (words + 255) / 256;
+        if (blocks > 148 * 8) blocks = 148 * 8;
+        k_build_coarse<<<(int)blocks, 256, 0, st>>>(fine, words, (int)g, coarse);
+        *launches += 1;
+    }
+    uint32_t head;
+    uint64_t groups;
+    split_aligned(xyz, n, &head, &groups);
+    const int blocks = (int)B.blocks;
+    const uint64_t gpb = (groups + blocks - 1) / blocks;
+    const uint32_t seg_cap = (uint32_t)(4 * gpb + 8);
+    if ((uint64_t)blocks * seg_cap > B.cap_entries) return cudaErrorInvalidValue;
+    StageParams Q;
+    Q.in = nullptr; Q.cnt_in = nullptr;
+    Q.out = B.list[0]; Q.cnt_out = B.cnt[0];
+    Q.seg_cap = seg_cap; Q.row0 = 0; Q.d_all = P.d; Q.pad = 0;
+    CoarseParams C;
+    C.fine = fine; C.coarse = coarse; C.g = g; C.row_words = row_words; C.nseg = (uint32_t)blocks;
+    const uint64_t cells = (uint64_t)P.sc[0].G * P.sc[0].G * P.sc[0].G;
+    C.hm = !P.sc[0].big ? 0 : (((cells - 1) >> 31) < HASH_TB ? 1 : 2);
+    const size_t smem = (size_t)first * row_words * 4 + (size_t)HASH_TB * P.d * sizeof(uint64_t);
+    cudaError_t e = cudaSuccess;
+#define CS_CB(F)                                                                                              \
+    case F:                                                                                                   \
+        e = cudaFuncSetAttribute(k_stage_first_cb<F>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem); \
+        if (e != cudaSuccess) return e;                                                                       \
+        k_stage_first_cb<F><<<sm_count < blocks ? sm_count : blocks, CB_THREADS, smem, st>>>(P, Q, C, xyz, n, head,   \
+                                                                                               groups, gpb);  \
+        break;
+    switch (first) { CS_CB(1) CS_CB(2) CS_CB(3) CS_CB(4) CS_CB(5) default: return cudaErrorInvalidValue; }
+#undef CS_CB
+    *launches += 1;
+    StageParams Q2 = Q;
+    Q2.in = B.list[0]; Q2.cnt_in = B.cnt[0];
+    Q2.out = B.list[1]; Q2.cnt_out = B.cnt[1];
+    Q2.row0 = first;
+    launch_stage_r<true, true>(rest, false, blocks, P, Q2, tg, xyz, n, head, groups, gpb, st);
+    *launches += 1;
     return cudaGetLastError();
 }
 

@@ -227,7 +227,7 @@ def test_binned_update_single_cell_overflows_bin_region(cs):
 
 # ---- bitmap-prefiltered scan (csrc/cs_scan_bitmap.cu) against the plain scan paths ---------------------------------
 
-@pytest.mark.parametrize("scan_mode", [2, 1])
+@pytest.mark.parametrize("scan_mode", [3, 2, 1])
 def test_scan_modes_cfg3_shape(cs, scan_mode):
     """Same stream through the bitmap prefilter (auto) and through the plain early-exit estimate."""
     wl, xyz = _gen("cfg3", (1 << 22) + 3)
@@ -235,19 +235,33 @@ def test_scan_modes_cfg3_shape(cs, scan_mode):
     assert st["tau"] >= 1
 
 
-def test_bitmap_scan_excursion_only_and_low_thresholds(cs):
+@pytest.mark.parametrize("scan_mode", [2, 3])
+def test_bitmap_scan_excursion_only_and_low_thresholds(cs, scan_mode):
     """k_max = 0 with thr_min >= 1: the bitmap is used from the first particle; thr_min <= 0: never (all cells pass)."""
     wl, xyz = _gen("cfg1", 1 << 19)
-    _check_all(cs, wl, xyz, k=0, thresholds=(3, 30), scan_mode=2)
-    _check_all(cs, wl, xyz, k=0, thresholds=(0, 5), scan_mode=2)
-    _check_all(cs, wl, xyz, k=0, thresholds=(-4,), cap=1 << 20, scan_mode=2)
+    _check_all(cs, wl, xyz, k=0, thresholds=(3, 30), scan_mode=scan_mode)
+    _check_all(cs, wl, xyz, k=0, thresholds=(0, 5), scan_mode=scan_mode)
+    _check_all(cs, wl, xyz, k=0, thresholds=(-4,), cap=1 << 20, scan_mode=scan_mode)
 
 
-def test_bitmap_scan_even_d_many_rows_and_wide_tables(cs):
+@pytest.mark.parametrize("scan_mode", [2, 3])
+def test_bitmap_scan_even_d_many_rows_and_wide_tables(cs, scan_mode):
     from paper_1711_00975_b200 import synth
-    for d, w, G in ((4, 1 << 12, 700), (12, 1 << 10, 90), (32, 1 << 9, 5000), (6, 1 << 18, 1 << 20)):
+    for d, w, G in ((4, 1 << 12, 700), (12, 1 << 10, 90), (32, 1 << 9, 5000), (6, 1 << 18, 1 << 20), (2, 1 << 13, 64),
+                    (9, 1 << 15, 3000), (10, 1 << 20, 4642)):
         wl = synth.Workload("bm", N=150001, G=(G,), d=d, w=w, k=300, H=32, f_bg=0.3, m_min=0, L=50.0, seed=d, gen_seed=d + 5)
-        st = _check_all(cs, wl, synth.generate(wl, device="cuda"), thresholds=(2,), probe_cells=256, scan_mode=2)
+        st = _check_all(cs, wl, synth.generate(wl, device="cuda"), thresholds=(2,), probe_cells=256, scan_mode=scan_mode)
+
+
+def test_bitmap_stages_cfg1_cfg2_cfg4_shapes_sampled_and_unaligned(cs):
+    wl, xyz = _gen("cfg1")
+    _check_all(cs, wl, xyz, thresholds=(40,), scan_mode=3)
+    wl, xyz = _gen("cfg2", (1 << 22) + 1)
+    _check_all(cs, wl, xyz, sample_p=0.7, scan_mode=3, split=[333333])
+    wl, xyz = _gen("cfg4", (1 << 21) + 2)
+    buf = torch.empty(3 * wl.N + 1, dtype=torch.float32, device="cuda")
+    buf[1:] = xyz.reshape(-1)
+    _check_all(cs, wl, buf[1:].view(-1, 3), k=3000, scan_mode=3)
 
 
 # ---- randomised small configs and edge cases ------------------------------------------------------------------
