@@ -170,6 +170,11 @@ int cs_scan_host(cs_sketch* s, const float* xyz_host, uint64_t n, double sample_
  * scanned ones).  Used to merge the candidate lists of several stream shards. */
 int cs_scan_cells(cs_sketch* s, int scale, const uint64_t* cells_dev, uint64_t m);
 
+/* Full-dictionary search (Alg. 1 l.7-13; the paper's "GPU without heap" query, :304-306): every cell
+ * id 0 .. G^3 - 1 of `scale` becomes a candidate, no positions needed.  Cost grows with G^3 (d gathers per cell until
+ * tau rejects early): meant for small meshes and as a cross-check of the re-scan; combine with cs_topk / cs_excursion. */
+int cs_scan_all(cs_sketch* s, int scale);
+
 /* Top-k (made deterministic, R9): the first min(k, #candidates)
  * candidates in (estimate descending, cell id ascending) order.  ids_out / est_out: any pointer, room for k
  * entries; *n_out (host) = number written.  k <= k_max. */

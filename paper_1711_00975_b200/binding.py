@@ -43,6 +43,7 @@ SIGNATURES = {
     "cs_scan": (ci, [vp, vp, u64, dbl]),
     "cs_scan_host": (ci, [vp, vp, u64, dbl]),
     "cs_scan_cells": (ci, [vp, ci, vp, u64]),
+    "cs_scan_all": (ci, [vp, ci]),
     "cs_topk": (ci, [vp, ci, u64, vp, vp, vp]),
     "cs_excursion": (ci, [vp, ci, i32, u64, vp, vp, vp]),
     "cs_scan_stats": (ci, [vp, ci, vp]),
@@ -208,6 +209,9 @@ class CountSketch:
         if not cells.is_cuda or cells.dtype not in (torch.int64, torch.uint64) or not cells.is_contiguous():
             raise ValueError("cells must be a contiguous CUDA int64/uint64 tensor")
         _chk(lib().cs_scan_cells(self._h, scale, vp(cells.data_ptr()), cells.numel()), "cs_scan_cells")
+
+    def scan_all(self, scale: int = 0):
+        _chk(lib().cs_scan_all(self._h, scale), "cs_scan_all")
 
     def topk(self, k: int, scale: int = 0, device=None):
         """(ids int64 tensor holding the uint64 cell ids, est int32 tensor), on `device` (default: the GPU)."""

@@ -1084,6 +1084,60 @@ int cs_scan_cells(cs_sketch* s, int scale, const uint64_t* cells_dev, uint64_t m
     return CS_OK;
 }
 
+int cs_scan_all(cs_sketch* s, int scale) {
+    if (!s) return fail(CS_ERR_ARG, "null handle");
+    if (scale < 0 || scale >= s->n_scales) return fail(CS_ERR_ARG, "scale out of range");
+    if (!s->scanning) return fail(CS_ERR_STATE, "cs_scan_all before cs_scan_begin");
+    const uint64_t m = (uint64_t)s->G[scale] * s->G[scale] * s->G[scale];
+    uint64_t done = 0;
+    while (done < m) {
+        uint32_t held = s->st_host[scale].count;
+        uint32_t fr = held < s->cap ? s->cap - held : 0;
+        if (fr < s->cap / 2) {                                   /* make room: compact (raises tau), else grow */
+            if (s->dirty[scale]) {
+                int rc = finalize_scale(s, scale);
+                if (rc) return rc;
+                continue;
+            }
+            int rc = grow_candidates(s);
+            if (rc) return rc;
+            continue;
+        }
+        /* optimistic chunk: few cells pass tau once the list is full; an overflow is detected, compacted and re-run */
+        uint64_t chunk = s->st_host[scale].tau > INT32_MIN ? (uint64_t)fr * 64 : fr;
+        if (chunk > m - done) chunk = m - done;
+        for (;;) {
+            ScanParams S;
+            fill_scan_params(s, &S);
+            PassParams P = pass_params(s, 0, 1.0);
+            cudaError_t e = launch_scan_range(P, S, scale, done, chunk, s->stream);
+            if (e != cudaSuccess) return fail(CS_ERR_CUDA, "scan_range kernel: %s", cudaGetErrorString(e));
+            s->launches += 1;
+            int rc = read_states(s);
+            if (rc) return rc;
+            if (s->st_host[scale].count != held) s->dirty[scale] = true;
+            if (s->st_host[scale].count <= s->cap) break;
+            rc = compact_scale(s, scale);                        /* entries past the capacity were dropped */
+            if (rc) return rc;
+            rc = read_states(s);
+            if (rc) return rc;
+            s->last_compact[scale] = s->st_host[scale].count;
+            held = s->st_host[scale].count;
+            while (s->cap - held < s->cap / 2) {
+                rc = grow_candidates(s);
+                if (rc) return rc;
+            }
+            if (chunk > s->cap - held) chunk = s->cap - held;    /* cannot overflow: one entry per cell at most */
+        }
+        done += chunk;
+        if (wants_compaction(s, scale)) {
+            int rc = finalize_scale(s, scale);
+            if (rc) return rc;
+        }
+    }
+    return CS_OK;
+}
+
 int cs_topk(cs_sketch* s, int scale, uint64_t k, uint64_t* ids_out, int32_t* est_out, uint64_t* n_out) {
     if (!s || !n_out) return fail(CS_ERR_ARG, "null argument");
     if (scale < 0 || scale >= s->n_scales) return fail(CS_ERR_ARG, "scale out of range");

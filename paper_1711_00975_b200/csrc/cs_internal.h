@@ -108,6 +108,8 @@ cudaError_t launch_scan_staged_cb(const PassParams& P, const ScanTarget& tg, con
                                   uint64_t n, int sm_count, cudaStream_t st, uint64_t* launches);
 cudaError_t launch_scan_cells(const PassParams& P, const ScanParams& S, int scale, const uint64_t* cells,
                               uint64_t m, cudaStream_t st);
+cudaError_t launch_scan_range(const PassParams& P, const ScanParams& S, int scale, uint64_t first, uint64_t m,
+                              cudaStream_t st);
 cudaError_t launch_estimate(const PassParams& P, int scale, const uint64_t* cells, uint64_t m, int32_t* est,
                             cudaStream_t st);
 cudaError_t launch_table_add(int32_t* T, const int32_t* in, uint64_t n, cudaStream_t st);

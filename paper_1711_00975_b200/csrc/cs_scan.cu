@@ -113,6 +113,25 @@ k_scan_cells(const __grid_constant__ PassParams P, const __grid_constant__ ScanP
     }
 }
 
+/* Full-dictionary search (Alg. 1 l.7-13: "for all j in [n]: Estimate(M, j)", the paper's "GPU without
+ * heap" query, :304-306): cells first .. first + m - 1 of scale s, no positions needed. */
+template <int D, bool POW2>
+__global__ void __launch_bounds__(PASS_THREADS)
+k_scan_range(const __grid_constant__ PassParams P, const __grid_constant__ ScanParams S, int s, uint64_t first,
+             uint64_t m) {
+    const int32_t tau = S.tg[s].st->tau;
+    const uint64_t stride = (uint64_t)gridDim.x * PASS_THREADS;
+    const uint32_t lane = threadIdx.x & 31u;
+    for (uint64_t i0 = (uint64_t)blockIdx.x * PASS_THREADS + (threadIdx.x - lane); i0 < m; i0 += stride) {
+        const uint64_t i = i0 + lane;
+        const uint64_t c = first + i;
+        int32_t e = 0;
+        bool emit = false;
+        if (i < m) emit = P.sc[s].big ? estimate_ge<D, POW2, true>(P, s, c, tau, e) : estimate_ge<D, POW2, false>(P, s, c, tau, e);
+        append_candidate(S.tg[s], emit, c, e);
+    }
+}
+
 /* ---- dispatch on (d, w power of two) ------------------------------------------------------------------ */
 
 template <bool POW2>
@@ -170,6 +189,22 @@ cudaError_t launch_scan_cells(const PassParams& P, const ScanParams& S, int scal
     const bool pow2 = (P.w & (P.w - 1)) == 0;
     return pow2 ? launch_scan_cells_p<true>(P, S, scale, cells, m, st)
                 : launch_scan_cells_p<false>(P, S, scale, cells, m, st);
+}
+
+template <bool POW2>
+static cudaError_t launch_scan_range_p(const PassParams& P, const ScanParams& S, int scale, uint64_t first, uint64_t m,
+                                       cudaStream_t st) {
+#define CS_CALL(DD) k_scan_range<DD, POW2><<<blocks_1d(m), PASS_THREADS, 0, st>>>(P, S, scale, first, m)
+    CS_DISPATCH_D(CS_CALL)
+#undef CS_CALL
+    return cudaGetLastError();
+}
+
+cudaError_t launch_scan_range(const PassParams& P, const ScanParams& S, int scale, uint64_t first, uint64_t m,
+                              cudaStream_t st) {
+    if (!m) return cudaSuccess;
+    const bool pow2 = (P.w & (P.w - 1)) == 0;
+    return pow2 ? launch_scan_range_p<true>(P, S, scale, first, m, st) : launch_scan_range_p<false>(P, S, scale, first, m, st);
 }
 
 }  // namespace cs

@@ -411,6 +411,35 @@ def test_call_order_and_argument_errors(cs):
     g.close()
 
 
+# ---- full-dictionary search (Alg. 1 l.7-13) ------------------------------------------------------
+
+@pytest.mark.parametrize("G,d,w,k", [(64, 5, 1 << 12, 200), (100, 4, 3001, 50), (128, 7, 1 << 16, 5000)])
+def test_full_dictionary_search(cs, G, d, w, k):
+    """cs_scan_all against the oracle's CSFS query (Estimate every j in [n], keep the top k): unoccupied cells are
+    candidates too, so this differs from the re-scan on purpose."""
+    from paper_1711_00975_b200 import synth
+    wl = synth.Workload("fs", N=200000, G=(G,), d=d, w=w, k=k, H=16, f_bg=0.3, m_min=0, L=100.0, seed=G + d, gen_seed=G)
+    xyz = synth.generate(wl, device="cuda")
+    o = ora.OracleSketch(d, w, (G,), wl.L, wl.seed)
+    o.update(xyz.cpu().numpy())
+    g = cs.CountSketch(d, w, [G], wl.L, wl.seed)
+    g.update(xyz)
+    g.set_candidate_capacity(1 << 14)                 # forces compactions, overflow re-runs and growth
+    g.scan_begin(k, 3)
+    g.scan_all()
+    gi, gv = g.topk(k)
+    oi, ov = o.full_search_topk(k)
+    assert np.array_equal(_ids(gi), oi) and np.array_equal(gv.cpu().numpy(), ov)
+    xi, xv, xt = g.excursion(3)
+    cells = np.arange(G ** 3, dtype=np.uint64)
+    est = o.estimate(cells)
+    keep = est >= 3
+    order = np.lexsort((cells[keep], -est[keep].astype(np.int64)))
+    assert xt == int(keep.sum())
+    assert np.array_equal(_ids(xi), cells[keep][order]) and np.array_equal(xv.cpu().numpy(), est[keep][order])
+    g.close(); o.close()
+
+
 # ---- BASELINE.json full size (cfg 3: 2^30 particles), in the launch configuration bench.py times ------------------
 
 def test_cfg3_full_size_properties(cs):
