@@ -175,6 +175,12 @@ int cs_scan_cells(cs_sketch* s, int scale, const uint64_t* cells_dev, uint64_t m
  * tau rejects early): meant for small meshes and as a cross-check of the re-scan; combine with cs_topk / cs_excursion. */
 int cs_scan_all(cs_sketch* s, int scale);
 
+/* Hierarchical, positions-free query (Alg. 3 CSHi: search the coarse layer in full, then
+ * only the children of its heavy cells).  With nested meshes (cs_create_multi, G[child] = r * G[parent], r <= 64) the
+ * r^3 sub-cells of each given parent cell become candidates of `child_scale`.  Typical use: cs_scan_all(coarse) ->
+ * cs_topk(coarse, c*k) -> cs_scan_children(coarse, fine, ids) -> cs_topk(fine, k).  parent_ids_dev: device. */
+int cs_scan_children(cs_sketch* s, int parent_scale, int child_scale, const uint64_t* parent_ids_dev, uint64_t m);
+
 /* Top-k (made deterministic, R9): the first min(k, #candidates)
  * candidates in (estimate descending, cell id ascending) order.  ids_out / est_out: any pointer, room for k
  * entries; *n_out (host) = number written.  k <= k_max. */

@@ -44,6 +44,7 @@ SIGNATURES = {
     "cs_scan_host": (ci, [vp, vp, u64, dbl]),
     "cs_scan_cells": (ci, [vp, ci, vp, u64]),
     "cs_scan_all": (ci, [vp, ci]),
+    "cs_scan_children": (ci, [vp, ci, ci, vp, u64]),
     "cs_topk": (ci, [vp, ci, u64, vp, vp, vp]),
     "cs_excursion": (ci, [vp, ci, i32, u64, vp, vp, vp]),
     "cs_scan_stats": (ci, [vp, ci, vp]),
@@ -212,6 +213,12 @@ class CountSketch:
 
     def scan_all(self, scale: int = 0):
         _chk(lib().cs_scan_all(self._h, scale), "cs_scan_all")
+
+    def scan_children(self, parents: torch.Tensor, parent_scale: int, child_scale: int):
+        if not parents.is_cuda or parents.dtype not in (torch.int64, torch.uint64) or not parents.is_contiguous():
+            raise ValueError("parents must be a contiguous CUDA int64/uint64 tensor")
+        _chk(lib().cs_scan_children(self._h, parent_scale, child_scale, vp(parents.data_ptr()), parents.numel()),
+             "cs_scan_children")
 
     def topk(self, k: int, scale: int = 0, device=None):
         """(ids int64 tensor holding the uint64 cell ids, est int32 tensor), on `device` (default: the GPU)."""

@@ -1084,6 +1084,32 @@ int cs_scan_cells(cs_sketch* s, int scale, const uint64_t* cells_dev, uint64_t m
     return CS_OK;
 }
 
+int cs_scan_children(cs_sketch* s, int parent_scale, int child_scale, const uint64_t* parent_ids_dev, uint64_t m) {
+    if (!s) return fail(CS_ERR_ARG, "null handle");
+    if (parent_scale < 0 || parent_scale >= s->n_scales || child_scale < 0 || child_scale >= s->n_scales)
+        return fail(CS_ERR_ARG, "scale out of range");
+    if (m && !parent_ids_dev) return fail(CS_ERR_ARG, "null parents with m > 0");
+    if (!s->scanning) return fail(CS_ERR_STATE, "cs_scan_children before cs_scan_begin");
+    const uint32_t Gp = s->G[parent_scale], Gc = s->G[child_scale];
+    if (Gc % Gp || Gc / Gp < 1 || Gc / Gp > 64) return fail(CS_ERR_ARG, "the child mesh must be a 1..64-fold refinement of the parent mesh");
+    const uint32_t r = Gc / Gp;
+    const uint64_t r3 = (uint64_t)r * r * r;
+    const uint64_t per = (1ull << 21) / r3 ? (1ull << 21) / r3 : 1;      /* parents per expansion: <= 2^21 ids (16 MiB) */
+    uint64_t* ids = nullptr;
+    CS_CUDA(cudaMalloc(&ids, per * r3 * sizeof(uint64_t)));
+    int rc = CS_OK;
+    for (uint64_t off = 0; off < m && rc == CS_OK; off += per) {
+        const uint64_t mm = m - off < per ? m - off : per;
+        cudaError_t e = launch_expand_children(parent_ids_dev + off, mm, Gp, Gc, r, ids, s->stream);
+        if (e != cudaSuccess) { rc = fail(CS_ERR_CUDA, "expand kernel: %s", cudaGetErrorString(e)); break; }
+        s->launches += 1;
+        rc = cs_scan_cells(s, child_scale, ids, mm * r3);
+    }
+    cudaStreamSynchronize(s->stream);
+    cudaFree(ids);
+    return rc;
+}
+
 int cs_scan_all(cs_sketch* s, int scale) {
     if (!s) return fail(CS_ERR_ARG, "null handle");
     if (scale < 0 || scale >= s->n_scales) return fail(CS_ERR_ARG, "scale out of range");

@@ -132,6 +132,33 @@ k_scan_range(const __grid_constant__ PassParams P, const __grid_constant__ ScanP
     }
 }
 
+/* Children of mesh cells on a finer nested mesh (Gc = r * Gp): out[i * r^3 + t] = id on the fine mesh of the t-th
+ * sub-cell of parent i.  Used by the positions-free hierarchical query (Alg. 3: search the coarse
+ * layer, then only the children of its heavy cells). */
+__global__ void __launch_bounds__(256)
+k_expand_children(const uint64_t* __restrict__ parents, uint64_t m, uint32_t Gp, uint32_t Gc, uint32_t r,
+                  uint64_t* __restrict__ out) {
+    const uint64_t r3 = (uint64_t)r * r * r;
+    const uint64_t total = m * r3;
+    const uint64_t stride = (uint64_t)gridDim.x * blockDim.x;
+    for (uint64_t i = (uint64_t)blockIdx.x * blockDim.x + threadIdx.x; i < total; i += stride) {
+        const uint64_t p = parents[i / r3];
+        const uint32_t t = (uint32_t)(i % r3);
+        const uint32_t px = (uint32_t)(p % Gp), py = (uint32_t)((p / Gp) % Gp), pz = (uint32_t)(p / ((uint64_t)Gp * Gp));
+        const uint32_t cx = px * r + t % r, cy = py * r + (t / r) % r, cz = pz * r + t / (r * r);
+        out[i] = (uint64_t)cx + (uint64_t)Gc * ((uint64_t)cy + (uint64_t)Gc * cz);
+    }
+}
+
+cudaError_t launch_expand_children(const uint64_t* parents, uint64_t m, uint32_t Gp, uint32_t Gc, uint32_t r, uint64_t* out,
+                                   cudaStream_t st) {
+    if (!m) return cudaSuccess;
+    uint64_t blocks = (m * r * r * r + 255) / 256;
+    if (blocks > 148 * 8) blocks = 148 * 8;
+    k_expand_children<<<(int)blocks, 256, 0, st>>>(parents, m, Gp, Gc, r, out);
+    return cudaGetLastError();
+}
+
 /* ---- dispatch on (d, w power of two) ------------------------------------------------------------------ */
 
 template <bool POW2>

@@ -440,6 +440,41 @@ def test_full_dictionary_search(cs, G, d, w, k):
     g.close(); o.close()
 
 
+def test_hierarchical_query_over_nested_meshes(cs):
+    """Alg. 3 (CSHi) without positions: full search of the coarse mesh, then only the children of its heavy cells on
+    the finer meshes.  Expected values: the oracle's estimates of exactly those children, sorted (est desc, id asc)."""
+    from paper_1711_00975_b200 import synth
+    Gs = (32, 64, 256)                                     # refinements x2 and x4
+    wl = synth.Workload("hi", N=400000, G=Gs, d=5, w=1 << 14, k=300, H=24, f_bg=0.2, m_min=0, L=100.0, seed=5, gen_seed=77)
+    xyz = synth.generate(wl, device="cuda")
+    o = ora.OracleSketch(wl.d, wl.w, Gs, wl.L, wl.seed)
+    o.update(xyz.cpu().numpy())
+    g = cs.CountSketch(wl.d, wl.w, list(Gs), wl.L, wl.seed)
+    g.update(xyz)
+    g.scan_begin(1000)
+    g.scan_all(0)
+    parents, pest = g.topk(200, 0)
+    oi, ov = o.full_search_topk(200, 0)
+    assert np.array_equal(_ids(parents), oi) and np.array_equal(pest.cpu().numpy(), ov)
+    for ps, cs_, kk in ((0, 1, 400), (1, 2, 1000)):
+        g.scan_children(parents, ps, cs_)
+        kids, kest = g.topk(kk, cs_)
+        r = Gs[cs_] // Gs[ps]
+        p = _ids(parents).astype(np.uint64)
+        Gp, Gc = np.uint64(Gs[ps]), np.uint64(Gs[cs_])
+        px, py, pz = p % Gp, (p // Gp) % Gp, p // (Gp * Gp)
+        t = np.arange(r ** 3, dtype=np.uint64)
+        cx = (px[:, None] * np.uint64(r) + t % np.uint64(r)).ravel()
+        cy = (py[:, None] * np.uint64(r) + (t // np.uint64(r)) % np.uint64(r)).ravel()
+        cz = (pz[:, None] * np.uint64(r) + t // np.uint64(r * r)).ravel()
+        kid = np.unique(cx + Gc * (cy + Gc * cz))
+        est = o.estimate(kid, cs_)
+        order = np.lexsort((kid, -est.astype(np.int64)))[:kk]
+        assert np.array_equal(_ids(kids), kid[order]) and np.array_equal(kest.cpu().numpy(), est[order])
+        parents = kids
+    g.close(); o.close()
+
+
 # ---- BASELINE.json full size (cfg 3: 2^30 particles), in the launch configuration bench.py times ------------------
 
 def test_cfg3_full_size_properties(cs):
