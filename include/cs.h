@@ -191,6 +191,17 @@ int cs_topk(cs_sketch* s, int scale, uint64_t k, uint64_t* ids_out, int32_t* est
 int cs_excursion(cs_sketch* s, int scale, int32_t thr, uint64_t cap, uint64_t* ids_out, int32_t* est_out,
                  uint64_t* n_total);
 
+/* Second pass over the stream restricted to m given cells of `scale` (normally the output of cs_topk / cs_excursion;
+ * PAPER.md:502-506 keep the particles of the heavy cells for an offline halo finder, :548, :556 exact number of
+ * particles in the output cells).  For the n particles at xyz_dev (device, no sampling):
+ *   counts_dev[i] += number of particles whose cell is ids_dev[i]   (device, m words, NOT zeroed by the call, so that
+ *                    batches accumulate; duplicate ids: the first occurrence counts);
+ *   if xyz_out_dev != NULL: those particles are copied there in arbitrary order, at most `cap` of them (device);
+ *   *n_out (host) = how many particles of this call belong to the cells (may exceed cap).
+ * Synchronises the stream.  m <= 2^28. */
+int cs_recount(cs_sketch* s, int scale, const uint64_t* ids_dev, uint64_t m, const float* xyz_dev, uint64_t n,
+               uint32_t* counts_dev, float* xyz_out_dev, uint64_t cap, uint64_t* n_out);
+
 /* out4[0] = candidates currently held, out4[1] = current collection threshold tau as (uint64)(int64)tau,
  * out4[2] = compactions run since cs_scan_begin, out4[3] = scan kernel launches since cs_scan_begin. */
 int cs_scan_stats(cs_sketch* s, int scale, uint64_t* out4_host);

@@ -47,6 +47,7 @@ SIGNATURES = {
     "cs_scan_children": (ci, [vp, ci, ci, vp, u64]),
     "cs_topk": (ci, [vp, ci, u64, vp, vp, vp]),
     "cs_excursion": (ci, [vp, ci, i32, u64, vp, vp, vp]),
+    "cs_recount": (ci, [vp, ci, vp, u64, vp, u64, vp, vp, u64, vp]),
     "cs_scan_stats": (ci, [vp, ci, vp]),
     "cs_sketch_read": (ci, [vp, ci, vp]),
     "cs_sketch_add": (ci, [vp, ci, vp]),
@@ -242,6 +243,23 @@ class CountSketch:
              "cs_excursion")
         m = min(int(n.value), cap)
         return ids[:m], est[:m], int(n.value)
+
+    def recount(self, ids: torch.Tensor, xyz: torch.Tensor, counts: torch.Tensor | None = None, scale: int = 0,
+                extract_cap: int = 0):
+        """Exact recount of the cells `ids` over `xyz` (counts accumulate into `counts` if given) and, with
+        extract_cap > 0, the particles of those cells.  Returns (counts int32 tensor, particles or None, n_members)."""
+        p, n = _dev_xyz(xyz)
+        if not ids.is_cuda or ids.dtype not in (torch.int64, torch.uint64) or not ids.is_contiguous():
+            raise ValueError("ids must be a contiguous CUDA int64/uint64 tensor")
+        m = ids.numel()
+        if counts is None:
+            counts = torch.zeros(max(m, 1), dtype=torch.int32, device=ids.device)
+        out = torch.empty((max(extract_cap, 1), 3), dtype=torch.float32, device=ids.device) if extract_cap else None
+        nm = u64(0)
+        _chk(lib().cs_recount(self._h, scale, vp(ids.data_ptr()), m, vp(p), n, vp(counts.data_ptr()),
+                              vp(out.data_ptr()) if out is not None else None, extract_cap, C.byref(nm)), "cs_recount")
+        k = min(int(nm.value), extract_cap)
+        return counts[:m], (out[:k] if out is not None else None), int(nm.value)
 
     def scan_stats(self, scale: int = 0) -> dict:
         out = (u64 * 4)()

@@ -18,7 +18,7 @@ PKG = Path(__file__).resolve().parent
 CSRC = PKG / "csrc"
 OBJ = CSRC / "build"
 LIB = PKG / "libcs.so"
-SOURCES = ["cs_api.cu", "cs_kernels.cu", "cs_update_binned.cu", "cs_scan.cu", "cs_scan_staged.cu", "cs_scan_bitmap.cu", "cs_select.cu", "cs_probe.cu"]
+SOURCES = ["cs_api.cu", "cs_kernels.cu", "cs_update_binned.cu", "cs_scan.cu", "cs_scan_staged.cu", "cs_scan_bitmap.cu", "cs_select.cu", "cs_recount.cu", "cs_probe.cu"]
 HEADERS = ["cs_internal.h", "cs_hash.h", "cs_device.cuh", "cs_launch.cuh", "cs_scan_common.cuh", "../../include/cs.h"]
 
 NVCC_FLAGS = [

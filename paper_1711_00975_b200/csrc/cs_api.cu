@@ -1203,6 +1203,39 @@ int cs_excursion(cs_sketch* s, int scale, int32_t thr, uint64_t cap, uint64_t* i
     return CS_OK;
 }
 
+int cs_recount(cs_sketch* s, int scale, const uint64_t* ids_dev, uint64_t m, const float* xyz_dev, uint64_t n,
+               uint32_t* counts_dev, float* xyz_out_dev, uint64_t cap, uint64_t* n_out) {
+    if (!s) return fail(CS_ERR_ARG, "null handle");
+    if (scale < 0 || scale >= s->n_scales) return fail(CS_ERR_ARG, "scale out of range");
+    if (m > (1ull << 28)) return fail(CS_ERR_ARG, "at most 2^28 cells");
+    if ((m && (!ids_dev || !counts_dev)) || (n && !xyz_dev)) return fail(CS_ERR_ARG, "null buffer with a non-zero size");
+    if (reinterpret_cast<uintptr_t>(xyz_dev) & 3u) return fail(CS_ERR_ARG, "positions must be 4-byte aligned");
+    if (xyz_out_dev && !n_out) return fail(CS_ERR_ARG, "n_out is required with xyz_out_dev");
+    if (n_out) *n_out = 0;
+    if (!m || !n) return CS_OK;
+    uint64_t size = 1024;
+    while (size < 4 * m) size *= 2;                                   /* load factor <= 1/4 */
+    uint64_t* keys = nullptr;
+    uint32_t* vals = nullptr;
+    CS_CUDA(cudaMalloc(&keys, size * sizeof(uint64_t)));
+    cudaError_t e = cudaMalloc(&vals, size * sizeof(uint32_t));
+    if (e == cudaSuccess) e = cudaMemsetAsync(keys, 0xFF, size * sizeof(uint64_t), s->stream);
+    if (e == cudaSuccess) e = cudaMemsetAsync(vals, 0xFF, size * sizeof(uint32_t), s->stream);
+    if (e == cudaSuccess) e = cudaMemsetAsync(s->word_dev, 0, 4, s->stream);
+    if (e == cudaSuccess) e = launch_ht_build(ids_dev, (uint32_t)m, keys, vals, (uint32_t)(size - 1), s->stream);
+    if (e == cudaSuccess)
+        e = launch_recount(s->P.sc[scale], xyz_dev, n, keys, vals, (uint32_t)(size - 1), counts_dev, xyz_out_dev, s->word_dev,
+                           cap, s->sm_count, s->stream);
+    if (e == cudaSuccess) e = cudaMemcpyAsync(s->word_host, s->word_dev, 4, cudaMemcpyDeviceToHost, s->stream);
+    if (e == cudaSuccess) e = cudaStreamSynchronize(s->stream);
+    cudaFree(keys);
+    if (vals) cudaFree(vals);
+    if (e != cudaSuccess) return fail(e == cudaErrorMemoryAllocation ? CS_ERR_NOMEM : CS_ERR_CUDA, "cs_recount: %s", cudaGetErrorString(e));
+    s->launches += 2;
+    if (n_out) *n_out = *s->word_host;
+    return CS_OK;
+}
+
 int cs_scan_stats(cs_sketch* s, int scale, uint64_t* out4_host) {
     if (!s || !out4_host) return fail(CS_ERR_ARG, "null argument");
     if (scale < 0 || scale >= s->n_scales) return fail(CS_ERR_ARG, "scale out of range");

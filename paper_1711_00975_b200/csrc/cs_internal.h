@@ -116,6 +116,12 @@ cudaError_t launch_estimate(const PassParams& P, int scale, const uint64_t* cell
                             cudaStream_t st);
 cudaError_t launch_table_add(int32_t* T, const int32_t* in, uint64_t n, cudaStream_t st);
 
+/* second pass restricted to output cells (cs_recount.cu) */
+cudaError_t launch_ht_build(const uint64_t* ids, uint32_t m, uint64_t* keys, uint32_t* vals, uint32_t mask, cudaStream_t st);
+cudaError_t launch_recount(const ScaleParams& sp, const float* xyz, uint64_t n, const uint64_t* keys, const uint32_t* vals,
+                           uint32_t mask, uint32_t* counts, float* out, uint32_t* out_count, uint64_t cap, int sm_count,
+                           cudaStream_t st);
+
 /* selection (cs_select.cu): sort the first n candidates of `src` by (ek ascending, id ascending), drop
  * duplicate ids, cut to the entries that can still matter and update *st (count, tau, est_min, est_max).
  * The result is left in `dst`.  scratch: at least select_scratch_words(n) uint32 words. */

@@ -475,6 +475,42 @@ def test_hierarchical_query_over_nested_meshes(cs):
     g.close(); o.close()
 
 
+# ---- second pass restricted to the output cells ------------------------------------------------
+
+def test_recount_and_membership_filter(cs):
+    """cs_recount against exact counting (oracle pin) and a numpy membership filter on the oracle's
+    cell ids: exact counts of the top-k cells in two batches, and the particles of those cells as a multiset."""
+    wl, xyz = _gen("cfg1", (1 << 19) + 3)
+    host = xyz.cpu().numpy()
+    g = cs.CountSketch(wl.d, wl.w, list(wl.G), wl.L, wl.seed)
+    g.update(xyz)
+    g.scan_begin(500)
+    g.scan(xyz)
+    ids, est = g.topk(500)
+    cut = 200001
+    counts, part_a, na = g.recount(ids, xyz[:cut], extract_cap=1 << 19)
+    counts, part_b, nb = g.recount(ids, xyz[cut:], counts=counts, extract_cap=1 << 19)
+    cells = ora.quantise(host, wl.G[0], wl.L)
+    eid, ecnt = ora.exact_counts(host, wl.G[0], wl.L)
+    want = dict(zip(eid.tolist(), ecnt.tolist()))
+    idl = _ids(ids).tolist()
+    assert counts.cpu().numpy().tolist() == [want.get(c, 0) for c in idl]
+    member = np.isin(cells, np.array(idl, dtype=np.uint64))
+    assert na == int(member[:cut].sum()) and nb == int(member[cut:].sum())
+    got = np.concatenate([part_a.cpu().numpy(), part_b.cpu().numpy()])
+    exp = host[member]
+    key = lambda a: a[np.lexsort((a[:, 2], a[:, 1], a[:, 0]))]
+    assert np.array_equal(key(got).view(np.uint32), key(exp).view(np.uint32))
+    # cells that do not occur, duplicates in the id list, truncation by cap, count-only mode
+    probe = torch.tensor([idl[0], 2 ** 40 + 5, idl[0], idl[1]], dtype=torch.int64, device="cuda")
+    c2, p2, n2 = g.recount(probe, xyz, extract_cap=7)
+    assert c2.cpu().numpy().tolist() == [want[idl[0]], 0, 0, want[idl[1]]]
+    assert n2 == want[idl[0]] + want[idl[1]] and p2.shape[0] == 7
+    c3, p3, n3 = g.recount(probe, xyz)
+    assert p3 is None and n3 == n2 and c3.cpu().numpy().tolist() == c2.cpu().numpy().tolist()
+    g.close()
+
+
 # ---- BASELINE.json full size (cfg 3: 2^30 particles), in the launch configuration bench.py times ------------------
 
 def test_cfg3_full_size_properties(cs):
