@@ -33,6 +33,8 @@ CPU_BASELINE_SAMPLE = 1 << 23  # particles of the cpu_baseline leg (about 10-30 
 
 # dram__bytes_read.sum + dram__bytes_write.sum of one k_update launch from the committed `ncu --set full`
 # capture (profiles/), keyed by workload; None until a capture exists for that workload.
+# thread instructions per particle of the update-phase kernels (smsp__inst_executed.sum x 32 / particles), same capture
+NCU_UPDATE_INSTR_PER_PARTICLE = {"cfg3": 490 + 27}
 NCU_TRAFFIC_BYTES = {"cfg3": 39.7e9}     # profiles/r1_kernels_cfg3.md: 8 x (scatter + apply) launches per step
 
 
@@ -205,6 +207,8 @@ def main_arm(args, wl):
     A_red_fp = ops / (red_fp_ms * 1e-3)      # the same at the sketch's whole footprint
     A_gather = ops / (gather_ms * 1e-3)
     hbm_peak, hbm_src = _peaks()
+    props = torch.cuda.get_device_properties(local)
+    sm_count, sm_mhz_max = props.multi_processor_count, 1965.0
 
     for _ in range(args.warmup):
         step()
@@ -254,6 +258,12 @@ def main_arm(args, wl):
                 "frac": N * 12 / (upd_ms * 1e-3) / 1e9 / hbm_peak, "peak_source": hbm_src,
                 "stream_only_gbs": N * 12 / (stream_ms * 1e-3) / 1e9},
         "gather_peak_G_per_s": A_gather / 1e9,
+        "alu": (None if wl.name not in NCU_UPDATE_INSTR_PER_PARTICLE else {
+            "achieved": NCU_UPDATE_INSTR_PER_PARTICLE[wl.name] * N / 32 / (upd_ms * 1e-3) / 1e9,
+            "peak": 4 * sm_count * sm_mhz_max * 1e6 / 1e9, "unit": "G warp-instructions/s",
+            "frac": NCU_UPDATE_INSTR_PER_PARTICLE[wl.name] * N / 32 / (upd_ms * 1e-3) / (4 * sm_count * sm_mhz_max * 1e6),
+            "peak_source": "4 warp schedulers per SM x SM count x max SM clock (B200_PROFILING.md: 148 SMs, 1965 MHz); "
+                           "instruction counts from profiles/r1_kernels_cfg3.md"}),
         "path": {"roof_particles_per_s": path_roof, "frac": (value / world) / path_roof,
                  "formula": "min(HBM/12B, A_L2/(d*scales*p)) per GPU, whole update+scan+select step against it "
                             "(BASELINE.json north_star)"},
