@@ -116,6 +116,12 @@ int cs_set_table_budget(cs_sketch* s, uint64_t bytes);
  *   mode 0 "auto" (default): binned for calls of at least 2^22 particles when the shape allows it. */
 int cs_set_update_mode(cs_sketch* s, int mode, int rows_direct);
 
+/* Counting mode.  0 (default): Count Sketch as described at the top.  1: the Count-Min variant the paper compares with
+ * (Fig. 10): Add increments every row's counter by +1 (no sign hash), Estimate is the MINIMUM
+ * over the rows; everything else (hashes h_j, sampling, re-scan, top-k, excursion sets) is unchanged.  Only allowed
+ * on an empty sketch (after cs_create / cs_reset, before the first cs_update), else CS_ERR_STATE. */
+int cs_set_counting_mode(cs_sketch* s, int mode);
+
 /* How cs_scan evaluates cells.  The result never depends on it.
  *   mode 1 "plain": every cell gets the early-exit estimate from the int32 tables.
  *   mode 2 "bitmap": once the collection threshold tau is >= 1 (and w is a power of two), a 1-bit-per-counter

@@ -22,6 +22,7 @@
  *                                 estimate >= threshold (R8)
  *   ora_full_search_topk          Alg. 1 l.7-13 (CSFS query: Estimate every j in [n])
  *   ora_exact_counts              exact counting, PAPER.md:398-402 (the brute-force pin)
+ *   ora_set_mode(1)               Count-Min variant: Add +1, Estimate = min over the rows
  *
  * Parity pins: tests/test_oracle_pins.py (run with -m "not gpu").  Every function above is pinned there;
  * nothing here is "parity unpinned" except the statistical quality on the paper's real data (out of scope).
@@ -78,6 +79,7 @@ struct Oracle {
     uint64_t upd_index;          /* particles passed to ora_update since create/reset */
     uint64_t scan_index;         /* particles passed to ora_scan since ora_scan_begin */
     bool scanning;
+    int mode;                    /* 0 Count Sketch; 1 Count-Min: Add +1, Estimate = min */
 };
 
 static uint64_t affine_mod_p(uint64_t a, uint64_t c, uint64_t b) {
@@ -119,9 +121,11 @@ static int32_t estimate_cell(const Oracle* o, const Scale& s, uint64_t c) {
     std::vector<int32_t> v((size_t)o->d);
     for (int j = 0; j < o->d; ++j) {
         uint64_t h = bucket_of(s.rows[j], c, o->w);
-        v[j] = wrap_mul_sign(s.T[(size_t)j * o->w + h], sign_of(s.rows[j], c));
+        int32_t sg = o->mode == 1 ? +1 : sign_of(s.rows[j], c);       /* Count-Min has no sign hash */
+        v[j] = wrap_mul_sign(s.T[(size_t)j * o->w + h], sg);
     }
     std::sort(v.begin(), v.end());
+    if (o->mode == 1) return v[0];         /* Count-Min: the minimum over the rows */
     return v[(size_t)((o->d - 1) / 2)];    /* median for odd d, lower median for even d (R4) */
 }
 
@@ -183,7 +187,7 @@ int ora_create_multi(Oracle** out, int n_scales, int d, uint64_t w, const uint32
     Oracle* o = new (std::nothrow) Oracle();
     if (!o) return ORA_ERR_NOMEM;
     o->d = d; o->w = w; o->L = L; o->seed = seed;
-    o->upd_index = 0; o->scan_index = 0; o->scanning = false;
+    o->upd_index = 0; o->scan_index = 0; o->scanning = false; o->mode = 0;
     try {
         o->sc.resize((size_t)n_scales);
         std::vector<uint64_t> co((size_t)4 * d);
@@ -212,6 +216,14 @@ int ora_create(Oracle** out, int d, uint64_t w, uint32_t G, double L, uint64_t s
 
 int ora_destroy(Oracle* o) { delete o; return ORA_OK; }
 
+/* 0: Count Sketch (default).  1: Count-Min variant (Fig. 10): Add increments by +1, Estimate is
+ * the minimum over the rows.  Set it before the first particle is added. */
+int ora_set_mode(Oracle* o, int mode) {
+    if (!o || mode < 0 || mode > 1) return ORA_ERR_ARG;
+    o->mode = mode;
+    return ORA_OK;
+}
+
 int ora_reset(Oracle* o) {
     if (!o) return ORA_ERR_ARG;
     for (Scale& S : o->sc) { std::fill(S.T.begin(), S.T.end(), 0); S.cand.clear(); }
@@ -235,7 +247,7 @@ int ora_update(Oracle* o, const float* xyz, uint64_t n, double sample_p) {
             uint64_t c = cell_of(xyz + 3 * i, S.scale, S.G);
             for (int j = 0; j < o->d; ++j) {
                 uint64_t h = bucket_of(S.rows[j], c, o->w);
-                int32_t s = sign_of(S.rows[j], c);
+                int32_t s = o->mode == 1 ? +1 : sign_of(S.rows[j], c);   /* Add(M, s); Count-Min adds +1 */
                 int32_t& ctr = S.T[(size_t)j * o->w + h];
                 ctr = wrap_add(ctr, s);
             }

@@ -53,6 +53,7 @@ def lib():
             "ora_create": (ci, [vp, ci, u64, u32, dbl, u64]),
             "ora_create_multi": (ci, [vp, ci, ci, u64, vp, dbl, u64]),
             "ora_destroy": (ci, [vp]),
+            "ora_set_mode": (ci, [vp, ci]),
             "ora_reset": (ci, [vp]),
             "ora_set_update_index": (ci, [vp, u64]),
             "ora_set_scan_index": (ci, [vp, u64]),
@@ -176,6 +177,10 @@ class OracleSketch:
 
     def reset(self):
         _chk(lib().ora_reset(self._h), "reset")
+
+    def set_mode(self, mode: int):
+        """0 Count Sketch (default), 1 Count-Min (Add +1, Estimate = min); before the first update."""
+        _chk(lib().ora_set_mode(self._h, mode), "set_mode")
 
     def set_update_index(self, index: int):
         _chk(lib().ora_set_update_index(self._h, index), "set_update_index")

@@ -31,6 +31,7 @@ SIGNATURES = {
     "cs_set_stream": (ci, [vp, vp]),
     "cs_set_table_budget": (ci, [vp, u64]),
     "cs_set_update_mode": (ci, [vp, ci, ci]),
+    "cs_set_counting_mode": (ci, [vp, ci]),
     "cs_set_scan_mode": (ci, [vp, ci]),
     "cs_set_update_index": (ci, [vp, u64]),
     "cs_set_scan_index": (ci, [vp, u64]),
@@ -161,6 +162,9 @@ class CountSketch:
 
     def set_update_mode(self, mode: int, rows_direct: int = -1):
         _chk(lib().cs_set_update_mode(self._h, mode, rows_direct), "cs_set_update_mode")
+
+    def set_counting_mode(self, mode: int):
+        _chk(lib().cs_set_counting_mode(self._h, mode), "cs_set_counting_mode")
 
     def set_scan_mode(self, mode: int):
         _chk(lib().cs_set_scan_mode(self._h, mode), "cs_set_scan_mode")

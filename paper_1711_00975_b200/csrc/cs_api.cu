@@ -429,7 +429,7 @@ int launch_scan_chunk(cs_sketch* s, const float* xyz, uint64_t n, uint64_t index
     /* bitmap prefilter: valid once every scale collects against a tau >= 1 (|T| >= tau is then necessary for a row
      * to pass); rebuilt (d*w/8 bytes, microseconds) whenever a compaction has raised tau */
     uint32_t cg0 = 0, crw0 = 0;
-    const bool staged_bm = s->n_scales == 1 && coarse_shape(s->d, s->w, &cg0, &crw0);
+    const bool staged_bm = s->n_scales == 1 && coarse_shape(s->d, s->P.rank, s->w, &cg0, &crw0);
     bool use_bm = (s->scan_mode == 2 || s->scan_mode == 3 || (s->scan_mode == 0 && staged_bm)) && (s->w & (s->w - 1)) == 0;
     for (int i = 0; i < s->n_scales && use_bm; ++i) use_bm = s->st_host[i].tau >= 1;
     if (use_bm) {
@@ -447,7 +447,7 @@ int launch_scan_chunk(cs_sketch* s, const float* xyz, uint64_t n, uint64_t index
             }
         }
         uint32_t cg = 0, crw = 0;
-        if (s->scan_mode != 2 && s->n_scales == 1 && coarse_shape(s->d, s->w, &cg, &crw)) {
+        if (s->scan_mode != 2 && s->n_scales == 1 && coarse_shape(s->d, s->P.rank, s->w, &cg, &crw)) {
             /* bitmap first stage (coarse bitmap in shared memory) + the remaining rows on dense warps */
             int rc = ensure_stage_lists(s, n);
             if (rc) return rc;
@@ -805,7 +805,7 @@ int cs_create_multi(cs_sketch** out, int n_scales, int d, uint64_t w, const uint
     if (cudaDeviceGetAttribute(&sm, cudaDevAttrMultiProcessorCount, dev) == cudaSuccess && sm > 0) s->sm_count = sm;
 
     PassParams& P = s->P;
-    P.w = w; P.d = d; P.n_scales = n_scales;
+    P.w = w; P.d = d; P.n_scales = n_scales; P.rank = (d - 1) / 2;
     for (int i = 0; i < n_scales; ++i) {
         uint64_t Ki = 0;
         derive_coeffs(seed + (uint64_t)i, d, s->coef[i], &Ki);
@@ -906,6 +906,25 @@ int cs_set_update_mode(cs_sketch* s, int mode, int rows_direct) {
         return fail(CS_ERR_ARG, "mode must be 0 (auto), 1 (direct) or 2 (binned); rows_direct in [-1, 32]");
     s->update_mode = mode;
     s->bin_rows_direct = rows_direct;
+    return CS_OK;
+}
+
+int cs_set_counting_mode(cs_sketch* s, int mode) {
+    if (!s) return fail(CS_ERR_ARG, "null handle");
+    if (mode < 0 || mode > 1) return fail(CS_ERR_ARG, "mode must be 0 (Count Sketch) or 1 (Count-Min)");
+    if (s->upd_index != 0 || s->scanning) return fail(CS_ERR_STATE, "the counting mode can only change on an empty sketch");
+    for (int i = 0; i < s->n_scales; ++i)
+        for (int j = 0; j < s->d; ++j) {
+            const uint64_t* c = &s->coef[i][4 * j];
+            /* Count-Min: a sign hash with all-zero limbs evaluates to residue 0, i.e. sign +1, in every form of cs_hash.h */
+            s->P.rows[i * s->d + j].s = mode ? HashCoef{0, 0, 0, 0, 0, 0} : split_coef(c[2], c[3]);
+        }
+    s->P.rank = mode ? 0 : (s->d - 1) / 2;
+    if (s->coarse) {                                   /* its shape depends on the rank */
+        CS_CUDA(cudaStreamSynchronize(s->stream));
+        cudaFree(s->coarse);
+        s->coarse = nullptr;
+    }
     return CS_OK;
 }
 

@@ -71,25 +71,27 @@ __device__ __forceinline__ void cswap(int32_t& a, int32_t& b) {
     a = lo; b = hi;
 }
 
-/* floor((D-1)/2)-th smallest of v[0..D-1]: odd-even transposition network, fully unrolled for D <= 8. */
+/* rank-th smallest (0-based) of v[0..D-1] -- rank = (D-1)/2 is the (lower) median, rank = 0 the Count-Min minimum:
+ * odd-even transposition network, fully unrolled for D <= 8. */
 template <int D>
-__device__ __forceinline__ int32_t median_of(int32_t (&v)[D]) {
+__device__ __forceinline__ int32_t select_of(int32_t (&v)[D], int rank) {
 #pragma unroll
     for (int r = 0; r < D; ++r) {
 #pragma unroll
         for (int i = (r & 1); i + 1 < D; i += 2) cswap(v[i], v[i + 1]);
     }
-    return v[(D - 1) / 2];
+    if (rank == (D - 1) / 2) return v[(D - 1) / 2];
+    return v[rank];
 }
 
-__device__ __forceinline__ int32_t median_rt(int32_t* v, int d) {
+__device__ __forceinline__ int32_t select_rt(int32_t* v, int d, int rank) {
     for (int i = 1; i < d; ++i) {
         int32_t x = v[i];
         int j = i - 1;
         while (j >= 0 && v[j] > x) { v[j + 1] = v[j]; --j; }
         v[j + 1] = x;
     }
-    return v[(d - 1) / 2];
+    return v[rank];
 }
 
 __host__ __device__ __forceinline__ uint32_t est_to_key(int32_t est) { return 0x7FFFFFFFu - (uint32_t)est; }

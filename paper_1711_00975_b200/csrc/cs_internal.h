@@ -58,7 +58,7 @@ struct PassParams {
     int32_t d;
     int32_t n_scales;
     int32_t sample;                      // 0: keep everything (sample_p >= 1)
-    int32_t pad;
+    int32_t rank;                        // Estimate = the rank-th smallest row value: (d-1)/2 (median), 0 for Count-Min
 };
 
 struct ScanParams {
@@ -102,7 +102,7 @@ struct StageBuffers {
 uint64_t staged_list_entries(uint64_t n, uint32_t blocks);
 cudaError_t launch_scan_staged(const PassParams& P, const ScanTarget& tg, const StageBuffers& B, int rows_per_stage,
                                const float* xyz, uint64_t n, cudaStream_t st, uint64_t* launches);
-bool coarse_shape(int d, uint64_t w, uint32_t* g_out, uint32_t* row_words_out);
+bool coarse_shape(int d, int rank, uint64_t w, uint32_t* g_out, uint32_t* row_words_out);
 cudaError_t launch_scan_staged_cb(const PassParams& P, const ScanTarget& tg, const StageBuffers& B, const uint32_t* fine,
                                   uint32_t* coarse, uint32_t g, uint32_t row_words, bool rebuild_coarse, const float* xyz,
                                   uint64_t n, int sm_count, cudaStream_t st, uint64_t* launches);

@@ -54,7 +54,7 @@ template <int D, int HM>
 __device__ __forceinline__ bool bitmap_survives(const PassParams& P, int s, const uint32_t* __restrict__ bm, uint32_t c0,
                                                 uint32_t c1, uint32_t tb_addr) {
     const int d = D ? D : P.d;
-    const int max_fail = (d - 1) / 2;
+    const int max_fail = P.rank;
     const uint32_t wmask = (uint32_t)(P.w - 1);
     const RowCoef* rows = &P.rows[s * d];
     int fails = 0;

@@ -31,7 +31,7 @@ __device__ __forceinline__ int32_t row_value(const PassParams& P, const int32_t*
 template <int D, bool POW2, bool BIG>
 __device__ __forceinline__ bool estimate_ge(const PassParams& P, int s, uint64_t c, int32_t tau, int32_t& est) {
     const int d = D ? D : P.d;
-    const int max_fail = (d - 1) / 2;            // est >= tau  <=>  at most (d-1)/2 row values are < tau
+    const int max_fail = P.rank;                 // est >= tau  <=>  at most rank row values are < tau (rank = (d-1)/2)
     const uint32_t c0 = cell_c0(c), c1 = cell_c1(c);
     const int32_t* T = P.sc[s].T;
     const RowCoef* rows = &P.rows[s * d];
@@ -45,8 +45,8 @@ __device__ __forceinline__ bool estimate_ge(const PassParams& P, int s, uint64_t
         }
     }
     if (fail > max_fail) return false;
-    if constexpr (D > 0) est = median_of<D>(v);
-    else                 est = median_rt(v, d);
+    if constexpr (D > 0) est = select_of<D>(v, P.rank);
+    else                 est = select_rt(v, d, P.rank);
     return true;
 }
 
@@ -95,7 +95,7 @@ __device__ __forceinline__ int32_t estimate_any(const PassParams& P, int s, uint
         uint32_t b = POW2 ? ((uint32_t)r & (uint32_t)(P.w - 1)) : (uint32_t)(r % P.w);
         v[j] = mul_sign(ld_table(P.sc[s].T + (uint64_t)j * P.w + b), 1 - 2 * (int32_t)((uint32_t)r2 & 1u));
     }
-    return median_rt(v, d);
+    return select_rt(v, d, P.rank);
 }
 
 /* ---- helpers of the bitmap prefilters (cs_scan_bitmap.cu, cs_scan_staged.cu) --------------------------------- */

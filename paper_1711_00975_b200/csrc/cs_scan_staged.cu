@@ -53,7 +53,7 @@ __device__ __noinline__ int32_t estimate_all_rows(const PassParams& P, int d, ui
     const uint32_t c0 = cell_c0(c), c1 = cell_c1(c);
     int32_t v[CS_MAX_ROWS];
     for (int j = 0; j < d; ++j) v[j] = row_value<BIG, POW2>(P, P.sc[0].T, P.rows[j], j, c0, c1);
-    return median_rt(v, d);
+    return select_rt(v, d, P.rank);
 }
 
 /* One cell through one stage.  Must be reached by all 32 lanes (the appends are warp-aggregated). */
@@ -95,7 +95,7 @@ k_stage_first(const __grid_constant__ PassParams P, const __grid_constant__ Stag
     if (threadIdx.x == 0) s_cnt = 0;
     __syncthreads();
     const int32_t tau = tg.st->tau;
-    const int max_fail = (Q.d_all - 1) / 2;
+    const int max_fail = P.rank;
     uint64_t* seg = LAST ? nullptr : Q.out + (uint64_t)blockIdx.x * Q.seg_cap;
     const float4* body = reinterpret_cast<const float4*>(xyz + 3 * (uint64_t)head);
     const uint64_t g_lo = (uint64_t)blockIdx.x * gpb;
@@ -151,7 +151,7 @@ k_stage_next(const __grid_constant__ PassParams P, const __grid_constant__ Stage
     if (threadIdx.x == 0) s_cnt = 0;
     __syncthreads();
     const int32_t tau = tg.st->tau;
-    const int max_fail = (Q.d_all - 1) / 2;
+    const int max_fail = P.rank;
     const uint64_t* seg_in = Q.in + (uint64_t)blockIdx.x * Q.seg_cap;
     uint64_t* seg = LAST ? nullptr : Q.out + (uint64_t)blockIdx.x * Q.seg_cap;
     const uint32_t cnt = Q.cnt_in[blockIdx.x];
@@ -282,7 +282,7 @@ k_stage_first_cb(const __grid_constant__ PassParams P, const __grid_constant__ S
                     uint32_t fails = 0;
 #pragma unroll
                     for (int j = 0; j < FIRST; ++j) fails += 1u - ((wd[q][j] >> (h[q][j] & 31u)) & 1u);
-                    const bool live = keep[2 * half + q] && fails < (uint32_t)FIRST;  // FIRST fails = more than (d-1)/2
+                    const bool live = keep[2 * half + q] && fails < (uint32_t)FIRST;  // FIRST = rank + 1 fails reject
                     const uint32_t mask = __ballot_sync(0xFFFFFFFFu, live);
                     if (mask) {
                         const int leader = __ffs(mask) - 1;
@@ -414,8 +414,8 @@ k_build_coarse(const uint32_t* __restrict__ fine, uint64_t n_coarse_words, int g
 
 /* Group size 2^g of the coarse bitmap: the smallest whose FIRST rows fit the shared-memory budget.
  * false: shape not supported by the bitmap first stage (the caller uses the plain stages). */
-bool coarse_shape(int d, uint64_t w, uint32_t* g_out, uint32_t* row_words_out) {
-    const int first = (d - 1) / 2 + 1, rest = d - first;
+bool coarse_shape(int d, int rank, uint64_t w, uint32_t* g_out, uint32_t* row_words_out) {
+    const int first = rank + 1, rest = d - first;
     if (first > 5 || rest < 1 || rest > 8 || (w & (w - 1)) || w < 4096) return false;
     for (uint32_t g = 0; g <= 8; ++g) {
         if ((w >> g) < 128) break;
@@ -432,7 +432,7 @@ bool coarse_shape(int d, uint64_t w, uint32_t* g_out, uint32_t* row_words_out) {
 cudaError_t launch_scan_staged_cb(const PassParams& P, const ScanTarget& tg, const StageBuffers& B, const uint32_t* fine,
                                   uint32_t* coarse, uint32_t g, uint32_t row_words, bool rebuild_coarse, const float* xyz,
                                   uint64_t n, int sm_count, cudaStream_t st, uint64_t* launches) {
-    const int first = (P.d - 1) / 2 + 1, rest = P.d - first;
+    const int first = P.rank + 1, rest = P.d - first;
     if (rebuild_coarse) {
         const uint64_t words = (uint64_t)first * row_words;
         uint64_t blocks = (words + 255) / 256;

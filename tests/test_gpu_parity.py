@@ -37,12 +37,15 @@ def _ids(t):
 
 
 def _check_all(cs, wl, xyz, sample_p=1.0, k=None, thresholds=(), probe_cells=4096, split=None, cap=None, budget=None,
-               mode=None, scan_mode=None):
+               mode=None, scan_mode=None, counting=0):
     """Update + estimate + scan + top-k (+ excursion) on both sides; everything must be identical."""
     k = wl.k if k is None else k
     host = xyz.cpu().numpy()
     o = ora.OracleSketch(wl.d, wl.w, wl.G, wl.L, wl.seed)
     g = cs.CountSketch(wl.d, wl.w, list(wl.G), wl.L, wl.seed)
+    if counting:
+        o.set_mode(counting)
+        g.set_counting_mode(counting)
     if budget:
         g.set_table_budget(budget)
     if mode is not None:
@@ -473,6 +476,32 @@ def test_hierarchical_query_over_nested_meshes(cs):
         assert np.array_equal(_ids(kids), kid[order]) and np.array_equal(kest.cpu().numpy(), est[order])
         parents = kids
     g.close(); o.close()
+
+
+# ---- Count-Min mode ---------------------------------------------------------
+
+def test_count_min_mode_on_every_path(cs):
+    """Add +1 / Estimate = min through the direct and the binned update, the plain, staged and bitmap scans, several
+    scales with sampling, even d, a table that is not a power of two."""
+    from paper_1711_00975_b200 import synth
+    wl, xyz = _gen("cfg1")
+    _check_all(cs, wl, xyz, thresholds=(50, 70), counting=1)
+    _check_all(cs, wl, xyz, thresholds=(50,), counting=1, mode=(2, 1), scan_mode=2)
+    wl, xyz = _gen("cfg3", (1 << 22) + 1)
+    _check_all(cs, wl, xyz, k=3000, thresholds=(40,), counting=1, mode=(2, 3))
+    _check_all(cs, wl, xyz, k=3000, counting=1, mode=(1, 0), scan_mode=1, budget=3 * wl.w * 4)
+    wl, xyz = _gen("cfg5", 1 << 21)
+    _check_all(cs, wl, xyz, sample_p=0.3, k=500, thresholds=(4,), counting=1)
+    for d, w in ((4, 3001), (6, 1 << 13), (1, 1 << 12), (2, 1 << 12)):
+        wl = synth.Workload("cm", N=120001, G=(300,), d=d, w=w, k=200, H=16, f_bg=0.3, m_min=0, L=100.0, seed=w, gen_seed=d)
+        _check_all(cs, wl, synth.generate(wl, device="cuda"), thresholds=(30,), probe_cells=512, counting=1)
+    # the mode can only change on an empty sketch
+    g = cs.CountSketch(3, 64, [8], 1.0, 1)
+    g.update(torch.rand((10, 3), device="cuda"))
+    with pytest.raises(cs.CsError) as e:
+        g.set_counting_mode(1)
+    assert e.value.code == cs.CS_ERR_STATE
+    g.reset(); g.set_counting_mode(1); g.close()
 
 
 # ---- second pass restricted to the output cells (SURVEY 8.f row f3) ------------------------------------------------

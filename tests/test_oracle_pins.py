@@ -180,6 +180,41 @@ def test_mini_pipeline(golden):
     assert T.tolist() == g["T"]
 
 
+def test_count_min_mini_pipeline_and_one_sided_error(golden):
+    """Count-Min mode: hand-worked tables / estimates of the mini pipeline; on a random stream
+    the estimate never undercounts (every row holds the cell's own count plus non-negative collisions) and is exact
+    when w is far larger than the number of cells; the Count-Sketch default is untouched by the switch."""
+    g, gm = golden["mini_pipeline_count_min"], golden["mini_pipeline"]
+    xyz = _centres(gm["stream_cells"], 4, 4.0)
+    o = ora.OracleSketch(3, 8, 4, 4.0, 1)
+    o.set_mode(1)
+    o.update(xyz)
+    assert o.sketch().tolist() == g["T"]
+    cells = [int(c) for c in g["est"]]
+    assert o.estimate(cells).tolist() == [g["est"][str(c)] for c in cells]
+    o.scan_begin(); o.scan(xyz)
+    ids, est = o.topk(2)
+    assert [[int(a), int(b)] for a, b in zip(ids, est)] == g["top2"]
+    o.set_mode(0); o.reset(); o.update(xyz)
+    assert o.sketch().tolist() == gm["T"]
+    rng = np.random.default_rng(11)
+    pts = (rng.random((20000, 3)) ** 3 * 50.0).astype(np.float32)           # skewed: heavy cells near the origin
+    eid, ecnt = ora.exact_counts(pts, 40, 50.0)
+    for w, exact in ((64, False), (1 << 22, True)):
+        o = ora.OracleSketch(4, w, 40, 50.0, 9)
+        o.set_mode(1)
+        o.update(pts)
+        assert int(o.sketch().min()) >= 0 and o.sketch().sum(axis=1).tolist() == [len(pts)] * 4
+        est = o.estimate(eid)
+        assert bool((est.astype(np.int64) >= ecnt.astype(np.int64)).all())
+        if exact:
+            hb, _ = o.hashes(eid)
+            if all(len(set(hb[:, j].tolist())) == len(eid) for j in range(4)):    # collision-free rows
+                assert np.array_equal(est.astype(np.uint64), ecnt)
+        else:
+            assert bool((est.astype(np.int64) > ecnt.astype(np.int64)).any())       # collisions do overcount
+
+
 # ---- sampler --------------------------------------------------------------------------------------------
 
 def test_sampler_pins(golden):
