@@ -306,38 +306,47 @@ def streamed_arm(args, wl):
     binding.lib()
     N, B = (args.n or wl.N), wl.batch
     k, p = wl.k, wl.sample_p
+    packed = args.packed               # 8-byte records (cs_pack_records) instead of 12-byte float32 positions
+    bpp = 8 if packed else 12
+    g = binding.CountSketch(wl.d, wl.w, list(wl.G), wl.L, wl.seed)
     t0 = time.perf_counter()
-    host = torch.empty((N, 3), dtype=torch.float32, pin_memory=True)
+    host = (torch.empty(N, dtype=torch.int64, pin_memory=True) if packed
+            else torch.empty((N, 3), dtype=torch.float32, pin_memory=True))
     t_pin = time.perf_counter() - t0
     cat = synth.Catalogue(wl, "cuda")
     t0 = time.perf_counter()
+    checksum = None
     for b, lo in enumerate(range(0, N, B)):
         m = min(B, N - lo)
-        host[lo:lo + m].copy_(synth.generate(wl, device="cuda", batch=b, n=m, catalogue=cat))
+        xb = synth.generate(wl, device="cuda", batch=b, n=m, catalogue=cat)
+        if checksum is None:
+            checksum = synth.checksum(xb[: 1 << 20])
+        host[lo:lo + m].copy_(g.pack_records(xb) if packed else xb)
+        del xb
     torch.cuda.synchronize()
     t_gen = time.perf_counter() - t0
-    checksum = synth.checksum(host[: 1 << 20])
     # pinned H2D bandwidth: the stream term of this workload's roofline
-    dev = torch.empty((1 << 28, 3), dtype=torch.float32, device="cuda")
+    probe_n = min(N, 1 << 28)
+    dev = torch.empty_like(host[:probe_n], device="cuda")
     e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
-    dev.copy_(host[: 1 << 28], non_blocking=True)
+    dev.copy_(host[:probe_n], non_blocking=True)
     e0.record()
     for _ in range(3):
-        dev.copy_(host[: 1 << 28], non_blocking=True)
+        dev.copy_(host[:probe_n], non_blocking=True)
     e1.record()
     torch.cuda.synchronize()
-    h2d_gbs = 3 * (1 << 28) * 12 / (e0.elapsed_time(e1) * 1e-3) / 1e9
+    h2d_gbs = 3 * probe_n * bpp / (e0.elapsed_time(e1) * 1e-3) / 1e9
     del dev
-    g = binding.CountSketch(wl.d, wl.w, list(wl.G), wl.L, wl.seed)
 
     def step(ev=None):
         def upd(x, sp):
             if ev:
                 ev[0].record()
-            g.update_host(x, sp)
+            (g.update_records_host if packed else g.update_host)(x, sp)
             if ev:
                 ev[1].record()
-        return sharded.sharded_pass(g, host, 0, p, k, binding.INT32_MAX, update=upd, scan=g.scan_host, topk_device="cpu")
+        return sharded.sharded_pass(g, host, 0, p, k, binding.INT32_MAX, update=upd,
+                                    scan=g.scan_records_host if packed else g.scan_host, topk_device="cpu")
 
     for _ in range(args.warmup):
         step()
@@ -356,24 +365,25 @@ def streamed_arm(args, wl):
     upd_ms = sum(a.elapsed_time(b) for a, b in ev) / args.steps
     value = N / (ms_per_step * 1e-3)
     stats = g.scan_stats(0)
-    roof = h2d_gbs * 1e9 / 12.0 / 2.0       # the stream crosses PCIe twice per step (update, re-scan)
+    roof = h2d_gbs * 1e9 / bpp / 2.0        # the stream crosses PCIe twice per step (update, re-scan)
     line = {
         "metric": METRIC, "value": value, "unit": UNIT, "n_gpus": 1, "steps": args.steps, "warmup": args.warmup,
         "ms_per_step": ms_per_step, "higher_is_better": True, "scaling": "weak", "vs_baseline": None, "dtype": "int32",
         "data": "synthetic",
         "config": {"workload": wl.name, "N": N, "d": wl.d, "w": wl.w, "G": list(wl.G), "k": k, "sample_p": p,
                    "batches": (N + B - 1) // B, "host_streamed": True,
+                   "input": "packed 64-bit records (integer cell rule, cs.h)" if packed else "float32 xyz",
                    "l2_between_iterations": "inputs (12 B x N) larger than L2", "positions_checksum_first_2^20": checksum,
                    "pin_s": t_pin, "generate_s": t_gen, "parallelism": "1 GPU"},
         "roofline": {"bound": "pcie", "kernel": "cs_update_host (H2D ring + update kernels)",
-                     "achieved": N * 12 / (upd_ms * 1e-3) / 1e9, "peak": h2d_gbs, "unit": "GB/s",
-                     "frac": N * 12 / (upd_ms * 1e-3) / 1e9 / h2d_gbs, "traffic": None,
-                     "peak_source": "pinned host -> device copy of 3.2 GB blocks measured in this run",
+                     "achieved": N * bpp / (upd_ms * 1e-3) / 1e9, "peak": h2d_gbs, "unit": "GB/s",
+                     "frac": N * bpp / (upd_ms * 1e-3) / 1e9 / h2d_gbs, "traffic": None,
+                     "peak_source": "pinned host -> device copy of 2^28-particle blocks measured in this run",
                      "kernel_ms": upd_ms, "kernel_share_of_step": upd_ms / ms_per_step,
                      "path": {"roof_particles_per_s": roof, "frac": value / roof,
-                              "formula": "PCIe bandwidth / 12 B / 2 passes (BASELINE.json north_star: PCIe for host-streamed runs)"}},
+                              "formula": f"PCIe bandwidth / {bpp} B / 2 passes (BASELINE.json north_star: PCIe for host-streamed runs)"}},
         "cpu_baseline": None,
-        "e2e": {"value": value, "unit": UNIT, "h2d_bytes_per_step": 2 * N * 12,
+        "e2e": {"value": value, "unit": UNIT, "h2d_bytes_per_step": 2 * N * bpp,
                 "d2h_bytes_per_step": sum(int(r[0].numel()) * 12 for r in res), "steps": args.steps, "ms_per_step": ms_per_step},
         "gpu_launches": g.launch_count() - launches0, "clocks": clk,
         "scan": {"candidates": stats["candidates"], "tau": stats["tau"], "compactions": stats["compactions"],
@@ -395,6 +405,7 @@ def main():
     ap.add_argument("--e2e-steps", type=int, default=2)
     ap.add_argument("--no-e2e", action="store_true")
     ap.add_argument("--no-cpu-baseline", action="store_true")
+    ap.add_argument("--packed", action="store_true", help="host-streamed workloads: 8-byte packed records instead of float32 xyz")
     ap.add_argument("--scan-mode", type=int, default=0, help="cs_set_scan_mode: 0 auto, 1 plain, 2 bitmap, 3 bitmap stages")
     ap.add_argument("--update-mode", type=int, default=0, help="cs_set_update_mode: 0 auto, 1 direct, 2 binned")
     ap.add_argument("--rows-direct", type=int, default=-1, help="rows of each binned pass that use red.global")

@@ -150,6 +150,19 @@ int cs_update(cs_sketch* s, const float* xyz_dev, uint64_t n, double sample_p);
  * (PAPER.md:295-298 batch flow, :570 I/O overlapped with compute). */
 int cs_update_host(cs_sketch* s, const float* xyz_host, uint64_t n, double sample_p);
 
+/* ---- packed 64-bit particle records ("3 coordinates in 64 bits"; R23) --------------------
+ * A record is the particle's cell on the 2^21 mesh: rec = qx | qy << 21 | qz << 42 with q = the quantisation above for
+ * G = 2^21.  Its cell on a mesh of G <= 2^20 cells per axis is, per axis, i = (q * G) >> 21 (exact integer rule; it can
+ * differ from the float32 rule by one cell for positions within 2^-21 L of a cell boundary).  8 bytes instead of 12
+ * cross PCIe in the host-streamed calls.  All meshes of the handle must divide its finest mesh, else CS_ERR_ARG.
+ * cs_pack_records converts device positions to records (asynchronous on the handle's stream); the other four calls
+ * mirror cs_update / cs_update_host / cs_scan / cs_scan_host, running index and sampling included. */
+int cs_pack_records(cs_sketch* s, const float* xyz_dev, uint64_t n, uint64_t* recs_dev);
+int cs_update_records(cs_sketch* s, const uint64_t* recs_dev, uint64_t n, double sample_p);
+int cs_update_records_host(cs_sketch* s, const uint64_t* recs_host, uint64_t n, double sample_p);
+int cs_scan_records(cs_sketch* s, const uint64_t* recs_dev, uint64_t n, double sample_p);
+int cs_scan_records_host(cs_sketch* s, const uint64_t* recs_host, uint64_t n, double sample_p);
+
 /* ---- queries ------------------------------------------------------------------------------------------ */
 
 /* est_dev[i] = Estimate(cells_dev[i]) against scale `scale`.  m = 0 is a no-op.

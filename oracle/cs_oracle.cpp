@@ -22,6 +22,8 @@
  *                                 estimate >= threshold (R8)
  *   ora_full_search_topk          Alg. 1 l.7-13 (CSFS query: Estimate every j in [n])
  *   ora_exact_counts              exact counting, PAPER.md:398-402 (the brute-force pin)
+ *   ora_update_records / ora_scan_records / ora_cells_of_records
+ *                                 the same passes over packed 64-bit records; R23
  *   ora_set_mode(1)               Count-Min variant: Add +1, Estimate = min over the rows
  *
  * Parity pins: tests/test_oracle_pins.py (run with -m "not gpu").  Every function above is pinned there;
@@ -279,6 +281,49 @@ int ora_scan(Oracle* o, const float* xyz, uint64_t n, double sample_p) {
         uint64_t index = o->scan_index + i;
         if (!keep_particle(o->K, index, sample_p)) continue;
         for (Scale& S : o->sc) S.cand.insert(cell_of(xyz + 3 * i, S.scale, S.G));
+    }
+    o->scan_index += n;
+    return ORA_OK;
+}
+
+/* ---- packed 64-bit particle records ("3 coordinates in 64 bits"; R23) -----------------------
+ * A record holds the particle's cell on the 2^21 mesh: rec = qx | qy << 21 | qz << 42, q < 2^21 (= the id that
+ * ora_quantise gives for G = 2^21).  Its cell on a mesh of G <= 2^20 cells per axis is, per axis, i = (q * G) >> 21
+ * (exact integers), c = ix + G*(iy + G*iz). */
+static uint64_t cell_of_record(uint64_t rec, uint32_t G) {
+    const uint64_t M = (((uint64_t)1) << 21) - 1;
+    uint64_t ix = ((rec & M) * G) >> 21, iy = (((rec >> 21) & M) * G) >> 21, iz = (((rec >> 42) & M) * G) >> 21;
+    return ix + (uint64_t)G * (iy + (uint64_t)G * iz);
+}
+
+void ora_cells_of_records(const uint64_t* recs, uint64_t n, uint32_t G, uint64_t* cells_out) {
+    for (uint64_t i = 0; i < n; ++i) cells_out[i] = cell_of_record(recs[i], G);
+}
+
+int ora_update_records(Oracle* o, const uint64_t* recs, uint64_t n, double sample_p) {
+    if (!o || bad_p(sample_p) || (!recs && n)) return ORA_ERR_ARG;
+    for (uint64_t i = 0; i < n; ++i) {
+        if (!keep_particle(o->K, o->upd_index + i, sample_p)) continue;
+        for (Scale& S : o->sc) {
+            uint64_t c = cell_of_record(recs[i], S.G);
+            for (int j = 0; j < o->d; ++j) {
+                uint64_t h = bucket_of(S.rows[j], c, o->w);
+                int32_t s = o->mode == 1 ? +1 : sign_of(S.rows[j], c);
+                int32_t& ctr = S.T[(size_t)j * o->w + h];
+                ctr = wrap_add(ctr, s);
+            }
+        }
+    }
+    o->upd_index += n;
+    return ORA_OK;
+}
+
+int ora_scan_records(Oracle* o, const uint64_t* recs, uint64_t n, double sample_p) {
+    if (!o || bad_p(sample_p) || (!recs && n)) return ORA_ERR_ARG;
+    if (!o->scanning) return ORA_ERR_STATE;
+    for (uint64_t i = 0; i < n; ++i) {
+        if (!keep_particle(o->K, o->scan_index + i, sample_p)) continue;
+        for (Scale& S : o->sc) S.cand.insert(cell_of_record(recs[i], S.G));
     }
     o->scan_index += n;
     return ORA_OK;

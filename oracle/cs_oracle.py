@@ -61,6 +61,9 @@ def lib():
             "ora_estimate": (ci, [vp, ci, vp, u64, vp]),
             "ora_scan_begin": (ci, [vp]),
             "ora_scan": (ci, [vp, vp, u64, dbl]),
+            "ora_update_records": (ci, [vp, vp, u64, dbl]),
+            "ora_scan_records": (ci, [vp, vp, u64, dbl]),
+            "ora_cells_of_records": (None, [vp, u64, u32, vp]),
             "ora_candidate_count": (ci, [vp, ci, vp]),
             "ora_topk": (ci, [vp, ci, u64, vp, vp, vp]),
             "ora_excursion": (ci, [vp, ci, i32, u64, vp, vp, vp]),
@@ -128,6 +131,19 @@ def quantise(xyz, G: int, L: float) -> np.ndarray:
     out = np.empty(p.shape[0], dtype=np.uint64)
     lib().ora_quantise(_ptr(p), p.shape[0], G, L, _ptr(out))
     return out
+
+
+def cells_of_records(recs, G: int) -> np.ndarray:
+    """Cell ids on the G mesh of packed 64-bit records (qx | qy << 21 | qz << 42)."""
+    r = np.ascontiguousarray(np.asarray(recs, dtype=np.uint64))
+    out = np.empty(r.shape[0], dtype=np.uint64)
+    lib().ora_cells_of_records(_ptr(r), r.shape[0], G, _ptr(out))
+    return out
+
+
+def pack_records(xyz, L: float) -> np.ndarray:
+    """Packed record of each particle = its cell id on the 2^21 mesh (quantise with G = 2^21)."""
+    return quantise(xyz, 1 << 21, L)
 
 
 def sample_threshold(p: float) -> int:
@@ -204,6 +220,14 @@ class OracleSketch:
     def scan(self, xyz, sample_p: float = 1.0):
         p = _xyz(xyz)
         _chk(lib().ora_scan(self._h, _ptr(p), p.shape[0], sample_p), "scan")
+
+    def update_records(self, recs, sample_p: float = 1.0):
+        r = np.ascontiguousarray(np.asarray(recs, dtype=np.uint64))
+        _chk(lib().ora_update_records(self._h, _ptr(r), r.shape[0], sample_p), "update_records")
+
+    def scan_records(self, recs, sample_p: float = 1.0):
+        r = np.ascontiguousarray(np.asarray(recs, dtype=np.uint64))
+        _chk(lib().ora_scan_records(self._h, _ptr(r), r.shape[0], sample_p), "scan_records")
 
     def candidate_count(self, scale: int = 0) -> int:
         n = C.c_uint64(0)

@@ -38,6 +38,11 @@ SIGNATURES = {
     "cs_get_update_index": (ci, [vp, vp]),
     "cs_update": (ci, [vp, vp, u64, dbl]),
     "cs_update_host": (ci, [vp, vp, u64, dbl]),
+    "cs_pack_records": (ci, [vp, vp, u64, vp]),
+    "cs_update_records": (ci, [vp, vp, u64, dbl]),
+    "cs_update_records_host": (ci, [vp, vp, u64, dbl]),
+    "cs_scan_records": (ci, [vp, vp, u64, dbl]),
+    "cs_scan_records_host": (ci, [vp, vp, u64, dbl]),
     "cs_estimate": (ci, [vp, ci, vp, u64, vp]),
     "cs_scan_begin": (ci, [vp, u64, i32]),
     "cs_set_candidate_capacity": (ci, [vp, u64]),
@@ -188,6 +193,30 @@ class CountSketch:
     def update_host(self, xyz: torch.Tensor, sample_p: float = 1.0):
         p, n = _host_xyz(xyz)
         _chk(lib().cs_update_host(self._h, vp(p), n, sample_p), "cs_update_host")
+
+    # -- packed 64-bit records
+    def pack_records(self, xyz: torch.Tensor) -> torch.Tensor:
+        p, n = _dev_xyz(xyz)
+        out = torch.empty(n, dtype=torch.int64, device=xyz.device)
+        _chk(lib().cs_pack_records(self._h, vp(p), n, vp(out.data_ptr())), "cs_pack_records")
+        return out
+
+    def _records(self, fn: str, recs: torch.Tensor, sample_p: float, cuda: bool):
+        if recs.is_cuda != cuda or recs.dtype not in (torch.int64, torch.uint64) or not recs.is_contiguous():
+            raise ValueError("records must be a contiguous int64/uint64 tensor on the %s" % ("device" if cuda else "host"))
+        _chk(getattr(lib(), fn)(self._h, vp(recs.data_ptr()), recs.numel(), sample_p), fn)
+
+    def update_records(self, recs: torch.Tensor, sample_p: float = 1.0):
+        self._records("cs_update_records", recs, sample_p, True)
+
+    def update_records_host(self, recs: torch.Tensor, sample_p: float = 1.0):
+        self._records("cs_update_records_host", recs, sample_p, False)
+
+    def scan_records(self, recs: torch.Tensor, sample_p: float = 1.0):
+        self._records("cs_scan_records", recs, sample_p, True)
+
+    def scan_records_host(self, recs: torch.Tensor, sample_p: float = 1.0):
+        self._records("cs_scan_records_host", recs, sample_p, False)
 
     # -- queries
     def estimate(self, cells: torch.Tensor, scale: int = 0) -> torch.Tensor:

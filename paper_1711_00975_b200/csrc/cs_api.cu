@@ -127,6 +127,9 @@ struct cs_sketch {
     float* kept = nullptr;
     uint64_t kept_cap = 0;             /* particles */
 
+    /* packed records: positions of one batch unpacked to cell centres of the finest mesh */
+    float* unpacked = nullptr;         /* STAGE_PARTICLES particles */
+
     /* survivor lists of the row-partitioned scan */
     StageBuffers stb = {};
 
@@ -746,6 +749,81 @@ int check_xyz(const cs_sketch* s, const float* xyz, uint64_t n, double sample_p)
 
 }  // namespace
 
+namespace {
+
+/* Finest mesh of the handle if every other mesh divides it (packed records need nested meshes), else 0. */
+uint32_t finest_nested_mesh(const cs_sketch* s) {
+    uint32_t gf = 0;
+    for (int i = 0; i < s->n_scales; ++i) if (s->G[i] > gf) gf = s->G[i];
+    for (int i = 0; i < s->n_scales; ++i) if (gf % s->G[i]) return 0;
+    return gf;
+}
+
+int check_records(const cs_sketch* s, const uint64_t* recs, uint64_t n, double sample_p) {
+    if (!s) return fail(CS_ERR_ARG, "null handle");
+    if (bad_p(sample_p)) return fail(CS_ERR_ARG, "sample_p must be in (0, 1]");
+    if (n && !recs) return fail(CS_ERR_ARG, "null records with n > 0");
+    if (reinterpret_cast<uintptr_t>(recs) & 7u) return fail(CS_ERR_ARG, "records must be 8-byte aligned");
+    if (!finest_nested_mesh(s)) return fail(CS_ERR_ARG, "packed records need meshes that all divide the finest one");
+    return CS_OK;
+}
+
+/* m <= STAGE_PARTICLES device records -> s->unpacked -> the ordinary update / scan passes */
+int records_batch(cs_sketch* s, const uint64_t* recs_dev, uint64_t m, uint64_t index0, double sample_p, bool scan) {
+    if (!s->unpacked) CS_CUDA(cudaMalloc(&s->unpacked, STAGE_PARTICLES * 12));
+    const uint32_t gf = finest_nested_mesh(s);
+    cudaError_t e = launch_unpack_centres(recs_dev, m, gf, (float)(s->L / (double)gf), s->unpacked, s->stream);
+    if (e != cudaSuccess) return fail(CS_ERR_CUDA, "unpack kernel: %s", cudaGetErrorString(e));
+    s->launches += 1;
+    return scan ? scan_device(s, s->unpacked, m, sample_p) : update_passes(s, s->unpacked, m, index0, sample_p);
+}
+
+int records_device(cs_sketch* s, const uint64_t* recs_dev, uint64_t n, double sample_p, bool scan) {
+    for (uint64_t off = 0; off < n; off += STAGE_PARTICLES) {
+        const uint64_t m = n - off < STAGE_PARTICLES ? n - off : STAGE_PARTICLES;
+        int rc = records_batch(s, recs_dev + off, m, s->upd_index + off, sample_p, scan);
+        if (rc) return rc;
+    }
+    if (!scan) s->upd_index += n;
+    return CS_OK;
+}
+
+/* records in host memory: 8 B per particle over PCIe through the same ring of staging slots */
+int records_host(cs_sketch* s, const uint64_t* recs_host, uint64_t n, double sample_p, bool scan) {
+    int rc = ensure_staging(s);
+    if (rc) return rc;
+    const uint64_t batches = (n + STAGE_PARTICLES - 1) / STAGE_PARTICLES;
+    auto stage = [&](uint64_t b) -> int {
+        const int slot = (int)(b % STAGE_SLOTS);
+        const uint64_t off = b * STAGE_PARTICLES;
+        const uint64_t m = n - off < STAGE_PARTICLES ? n - off : STAGE_PARTICLES;
+        CS_CUDA(cudaStreamWaitEvent(s->copy_stream, s->ev_free[slot], 0));
+        CS_CUDA(cudaMemcpyAsync(s->stage[slot], recs_host + off, m * 8, cudaMemcpyHostToDevice, s->copy_stream));
+        CS_CUDA(cudaEventRecord(s->ev_full[slot], s->copy_stream));
+        return CS_OK;
+    };
+    rc = stage(0);
+    if (rc) return rc;
+    for (uint64_t b = 0; b < batches; ++b) {
+        if (b + 1 < batches) {
+            rc = stage(b + 1);
+            if (rc) return rc;
+        }
+        const int slot = (int)(b % STAGE_SLOTS);
+        const uint64_t off = b * STAGE_PARTICLES;
+        const uint64_t m = n - off < STAGE_PARTICLES ? n - off : STAGE_PARTICLES;
+        CS_CUDA(cudaStreamWaitEvent(s->stream, s->ev_full[slot], 0));
+        rc = records_batch(s, reinterpret_cast<const uint64_t*>(s->stage[slot]), m, s->upd_index + off, sample_p, scan);
+        if (rc) return rc;
+        CS_CUDA(cudaEventRecord(s->ev_free[slot], s->stream));
+    }
+    CS_CUDA(cudaStreamSynchronize(s->copy_stream));
+    if (!scan) s->upd_index += n;
+    return CS_OK;
+}
+
+}  // namespace
+
 /* =========================================================================================================
  * C ABI
  * ========================================================================================================= */
@@ -857,6 +935,7 @@ int cs_destroy(cs_sketch* s) {
     if (s->bins) cudaFree(s->bins);
     if (s->cursor) cudaFree(s->cursor);
     if (s->kept) cudaFree(s->kept);
+    if (s->unpacked) cudaFree(s->unpacked);
     for (int i = 0; i < CS_MAX_SCALES; ++i) if (s->bm[i]) cudaFree(s->bm[i]);
     if (s->coarse) cudaFree(s->coarse);
     for (int i = 0; i < CS_MAX_SCALES; ++i) if (s->T[i]) cudaFree(s->T[i]);
@@ -984,6 +1063,45 @@ int cs_update_host(cs_sketch* s, const float* xyz_host, uint64_t n, double sampl
     CS_CUDA(cudaStreamSynchronize(s->copy_stream));      /* the host buffer may be reused on return */
     s->upd_index += n;
     return CS_OK;
+}
+
+int cs_pack_records(cs_sketch* s, const float* xyz_dev, uint64_t n, uint64_t* recs_dev) {
+    if (!s) return fail(CS_ERR_ARG, "null handle");
+    if (n && (!xyz_dev || !recs_dev)) return fail(CS_ERR_ARG, "null buffer with n > 0");
+    if ((reinterpret_cast<uintptr_t>(xyz_dev) & 3u) || (reinterpret_cast<uintptr_t>(recs_dev) & 7u))
+        return fail(CS_ERR_ARG, "positions must be 4-byte aligned, records 8-byte aligned");
+    cudaError_t e = launch_pack_records(xyz_dev, n, (float)((double)(1u << 21) / s->L), recs_dev, s->stream);
+    if (e != cudaSuccess) return fail(CS_ERR_CUDA, "pack kernel: %s", cudaGetErrorString(e));
+    s->launches += n ? 1 : 0;
+    return CS_OK;
+}
+
+int cs_update_records(cs_sketch* s, const uint64_t* recs_dev, uint64_t n, double sample_p) {
+    int rc = check_records(s, recs_dev, n, sample_p);
+    if (rc || !n) return rc;
+    return records_device(s, recs_dev, n, sample_p, false);
+}
+
+int cs_update_records_host(cs_sketch* s, const uint64_t* recs_host, uint64_t n, double sample_p) {
+    int rc = check_records(s, recs_host, n, sample_p);
+    if (rc || !n) return rc;
+    return records_host(s, recs_host, n, sample_p, false);
+}
+
+int cs_scan_records(cs_sketch* s, const uint64_t* recs_dev, uint64_t n, double sample_p) {
+    int rc = check_records(s, recs_dev, n, sample_p);
+    if (rc) return rc;
+    if (!s->scanning) return fail(CS_ERR_STATE, "cs_scan_records before cs_scan_begin");
+    if (!n) return CS_OK;
+    return records_device(s, recs_dev, n, sample_p, true);
+}
+
+int cs_scan_records_host(cs_sketch* s, const uint64_t* recs_host, uint64_t n, double sample_p) {
+    int rc = check_records(s, recs_host, n, sample_p);
+    if (rc) return rc;
+    if (!s->scanning) return fail(CS_ERR_STATE, "cs_scan_records_host before cs_scan_begin");
+    if (!n) return CS_OK;
+    return records_host(s, recs_host, n, sample_p, true);
 }
 
 int cs_estimate(cs_sketch* s, int scale, const uint64_t* cells_dev, uint64_t m, int32_t* est_dev) {

@@ -83,6 +83,8 @@ cudaError_t launch_update_binned(const PassParams& P, const BinParams& B, const 
                                  cudaStream_t st);
 
 /* kernel launchers (cs_kernels.cu) */
+cudaError_t launch_pack_records(const float* xyz, uint64_t n, float qscale21, uint64_t* recs, cudaStream_t st);
+cudaError_t launch_unpack_centres(const uint64_t* recs, uint64_t n, uint32_t Gf, float cell_f, float* xyz, cudaStream_t st);
 cudaError_t launch_compact_kept(const float* xyz, uint64_t n, uint64_t index0, uint64_t K, uint64_t Tp, float* out,
                                 uint32_t* count, uint32_t cap, int sm_count, cudaStream_t st);
 cudaError_t launch_update(const PassParams& P, const float* xyz, uint64_t n, int sm_count, cudaStream_t st);

@@ -197,6 +197,59 @@ cudaError_t launch_compact_kept(const float* xyz, uint64_t n, uint64_t index0, u
     return cudaGetLastError();
 }
 
+/* ------------------------------------------------------------------------------------------------------
+ * packed 64-bit particle records ("3 coordinates in 64 bits"; R23)
+ * rec = qx | qy << 21 | qz << 42 = the particle's cell on the 2^21 mesh; cell on a mesh of G: i = (q*G) >> 21 per axis.
+ * k_pack_records    float32 positions -> records (quantise with G = 2^21).
+ * k_unpack_centres  records -> float32 positions at the centre of the record's cell on the FINEST mesh Gf of the
+ *                   handle.  The float quantisation of that centre gives back exactly i = (q*Gf) >> 21 (the centre is
+ *                   0.5 cells from either boundary and float32 rounding moves x*scale by < 0.25 for Gf <= 2^20), and
+ *                   for every coarser mesh that divides Gf the nested floors agree, so the ordinary passes run on
+ *                   the unpacked buffer unchanged and compute the integer rule bit for bit.
+ * ------------------------------------------------------------------------------------------------------ */
+__global__ void __launch_bounds__(256)
+k_pack_records(const float* __restrict__ xyz, uint64_t n, float qscale21, uint64_t* __restrict__ recs) {
+    const float top = (float)((1u << 21) - 1);
+    const uint64_t stride = (uint64_t)gridDim.x * blockDim.x;
+    for (uint64_t i = (uint64_t)blockIdx.x * blockDim.x + threadIdx.x; i < n; i += stride) {
+        const float* p = xyz + 3 * i;
+        const uint64_t qx = quantise_axis(ld_stream4(p), qscale21, top), qy = quantise_axis(ld_stream4(p + 1), qscale21, top),
+                       qz = quantise_axis(ld_stream4(p + 2), qscale21, top);
+        recs[i] = qx | (qy << 21) | (qz << 42);
+    }
+}
+
+__global__ void __launch_bounds__(256)
+k_unpack_centres(const uint64_t* __restrict__ recs, uint64_t n, uint32_t Gf, float cell_f, float* __restrict__ xyz) {
+    const uint64_t M = (1ull << 21) - 1;
+    const uint64_t stride = (uint64_t)gridDim.x * blockDim.x;
+    for (uint64_t i = (uint64_t)blockIdx.x * blockDim.x + threadIdx.x; i < n; i += stride) {
+        const uint64_t r = recs[i];
+        const uint32_t ix = (uint32_t)(((r & M) * Gf) >> 21), iy = (uint32_t)((((r >> 21) & M) * Gf) >> 21),
+                       iz = (uint32_t)((((r >> 42) & M) * Gf) >> 21);
+        float* p = xyz + 3 * i;
+        p[0] = __fmul_rn(__fadd_rn((float)ix, 0.5f), cell_f);
+        p[1] = __fmul_rn(__fadd_rn((float)iy, 0.5f), cell_f);
+        p[2] = __fmul_rn(__fadd_rn((float)iz, 0.5f), cell_f);
+    }
+}
+
+cudaError_t launch_pack_records(const float* xyz, uint64_t n, float qscale21, uint64_t* recs, cudaStream_t st) {
+    if (!n) return cudaSuccess;
+    uint64_t blocks = (n + 255) / 256;
+    if (blocks > 148 * 16) blocks = 148 * 16;
+    k_pack_records<<<(int)blocks, 256, 0, st>>>(xyz, n, qscale21, recs);
+    return cudaGetLastError();
+}
+
+cudaError_t launch_unpack_centres(const uint64_t* recs, uint64_t n, uint32_t Gf, float cell_f, float* xyz, cudaStream_t st) {
+    if (!n) return cudaSuccess;
+    uint64_t blocks = (n + 255) / 256;
+    if (blocks > 148 * 16) blocks = 148 * 16;
+    k_unpack_centres<<<(int)blocks, 256, 0, st>>>(recs, n, Gf, cell_f, xyz);
+    return cudaGetLastError();
+}
+
 /* T += in (merge / restore by linearity), wraparound. */
 __global__ void __launch_bounds__(256) k_table_add(int32_t* __restrict__ T, const int32_t* __restrict__ in, uint64_t n) {
     const uint64_t stride = (uint64_t)gridDim.x * blockDim.x;

@@ -504,6 +504,66 @@ def test_count_min_mode_on_every_path(cs):
     g.reset(); g.set_counting_mode(1); g.close()
 
 
+# ---- packed 64-bit records ------------------------------------------------------------
+
+def _check_records(cs, wl, xyz, sample_p=1.0, k=None, host=False, split=None):
+    k = wl.k if k is None else k
+    g = cs.CountSketch(wl.d, wl.w, list(wl.G), wl.L, wl.seed)
+    o = ora.OracleSketch(wl.d, wl.w, wl.G, wl.L, wl.seed)
+    recs = g.pack_records(xyz)
+    hrecs = recs.cpu()
+    want = ora.pack_records(xyz.cpu().numpy(), wl.L)
+    assert np.array_equal(hrecs.numpy().view(np.uint64), want), "cs_pack_records differs from the oracle's packing"
+    n = recs.numel()
+    cuts = [0, n] if not split else [0] + sorted(split) + [n]
+    for a, b in zip(cuts[:-1], cuts[1:]):
+        o.update_records(want[a:b], sample_p)
+        if host:
+            g.update_records_host(hrecs[a:b].contiguous(), sample_p)
+        else:
+            g.update_records(recs[a:b], sample_p)
+    o.scan_begin()
+    g.scan_begin(k)
+    for a, b in zip(cuts[:-1], cuts[1:]):
+        o.scan_records(want[a:b], sample_p)
+        if host:
+            g.scan_records_host(hrecs[a:b].contiguous(), sample_p)
+        else:
+            g.scan_records(recs[a:b], sample_p)
+    for s_ in range(len(wl.G)):
+        assert np.array_equal(g.sketch(s_).cpu().numpy(), o.sketch(s_)), f"sketch differs at scale {s_}"
+        gi, gv = g.topk(k, s_)
+        oi, ov = o.topk(k, s_)
+        assert np.array_equal(_ids(gi), oi) and np.array_equal(gv.cpu().numpy(), ov), f"top-k differs at scale {s_}"
+    g.close(); o.close()
+
+
+def test_packed_records_paths(cs):
+    """Integer rule i = (q*G) >> 21 through the unpack-to-centre route, against the oracle's record passes: big meshes,
+    a mesh that is not a power of two, nested multi-scale with sampling, device and host-streamed calls, edge values."""
+    wl, xyz = _gen("cfg3", (1 << 22) + 5)
+    _check_records(cs, wl, xyz, k=3000, split=[1234567])
+    wl, xyz = _gen("cfg4", (1 << 21) + 1)
+    _check_records(cs, wl, xyz, k=3000, host=True)
+    wl, xyz = _gen("cfg5", 1 << 21)
+    _check_records(cs, wl, xyz, sample_p=0.3, k=500, split=[700001])
+    _check_records(cs, wl, xyz, sample_p=0.3, k=500, host=True)
+    from paper_1711_00975_b200 import synth
+    L = 500.0
+    vals = np.array([0.0, L, np.nextafter(np.float32(L), np.float32(0)), -3.0, np.nan, np.inf, 1e-30, 249.99998, 250.0,
+                     250.00002, 499.9, 0.00024], dtype=np.float32)
+    rng = np.random.default_rng(2)
+    pos = np.concatenate([vals[rng.integers(0, len(vals), size=(4099, 3))], (rng.random((60000, 3)) * L).astype(np.float32)])
+    for G in (1, 7, 1 << 20):
+        wl = synth.Workload("pk", N=len(pos), G=(G,), d=3, w=1 << 12, k=50, H=1, f_bg=1.0, m_min=0, L=L, seed=G)
+        _check_records(cs, wl, torch.from_numpy(pos).cuda(), k=50)
+    g = cs.CountSketch(3, 64, [6, 4], 1.0, 1)                    # 4 does not divide 6
+    with pytest.raises(cs.CsError) as e:
+        g.update_records(torch.zeros(4, dtype=torch.int64, device="cuda"))
+    assert e.value.code == cs.CS_ERR_ARG
+    g.close()
+
+
 # ---- second pass restricted to the output cells (SURVEY 8.f row f3) ------------------------------------------------
 
 def test_recount_and_membership_filter(cs):

@@ -215,6 +215,45 @@ def test_count_min_mini_pipeline_and_one_sided_error(golden):
             assert bool((est.astype(np.int64) > ecnt.astype(np.int64)).any())       # collisions do overcount
 
 
+def test_packed_records():
+    """Packed 64-bit records (R23): the per-axis rule i = (q*G) >> 21 against Python integers,
+    nested meshes are consistent (coarse cell = fine cell // r per axis), and the record passes equal the float passes
+    on the centres of the 2^20-mesh cells the records fall in (where both quantisations agree by construction)."""
+    rng = np.random.default_rng(5)
+    q = rng.integers(0, 1 << 21, size=(5000, 3), dtype=np.uint64)
+    q[:8] = [[0, 0, 0], [2 ** 21 - 1] * 3, [1, 2 ** 20, 2 ** 21 - 1], [2 ** 20 - 1, 2 ** 20, 2 ** 20 + 1], [511, 512, 513],
+             [4095, 4096, 4097], [2 ** 21 - 2, 0, 7], [3, 3, 3]]
+    recs = q[:, 0] | (q[:, 1] << np.uint64(21)) | (q[:, 2] << np.uint64(42))
+    for G in (1, 2, 3, 256, 1000, 4096, 4642, 1 << 20):
+        got = ora.cells_of_records(recs, G)
+        ix, iy, iz = [[(int(v) * G) >> 21 for v in q[:, a]] for a in range(3)]
+        want = [x + G * (y + G * z) for x, y, z in zip(ix, iy, iz)]
+        assert got.tolist() == want
+        assert max(max(ix), max(iy), max(iz)) <= G - 1
+    c512, c4096 = ora.cells_of_records(recs, 512), ora.cells_of_records(recs, 4096)
+    f = [c4096 % 4096, (c4096 // 4096) % 4096, c4096 // 4096 ** 2]
+    assert np.array_equal(c512, f[0] // 8 + 512 * (f[1] // 8 + 512 * (f[2] // 8)))
+    # pack = quantise on the 2^21 mesh
+    L = 500.0
+    pts = (rng.random((3000, 3)) * L).astype(np.float32)
+    rp = ora.pack_records(pts, L)
+    sc = np.float32((1 << 21) / L)
+    qq = np.clip(np.floor(pts * sc), 0, (1 << 21) - 1).astype(np.uint64)
+    assert np.array_equal(rp, qq[:, 0] | (qq[:, 1] << np.uint64(21)) | (qq[:, 2] << np.uint64(42)))
+    # record passes == float passes on cell centres of the finest mesh
+    Gs = (64, 256)
+    cf = ora.cells_of_records(rp, 256)
+    centres = _centres(cf.tolist(), 256, L)
+    a, b = ora.OracleSketch(3, 1 << 10, Gs, L, 3), ora.OracleSketch(3, 1 << 10, Gs, L, 3)
+    a.update_records(rp, 0.6); b.update(centres, 0.6)
+    a.scan_begin(); b.scan_begin()
+    a.scan_records(rp, 0.6); b.scan(centres, 0.6)
+    for s_ in range(2):
+        assert np.array_equal(a.sketch(s_), b.sketch(s_))
+        ia, ea = a.topk(50, s_); ib, eb = b.topk(50, s_)
+        assert np.array_equal(ia, ib) and np.array_equal(ea, eb)
+
+
 # ---- sampler --------------------------------------------------------------------------------------------
 
 def test_sampler_pins(golden):
