@@ -1,0 +1,36 @@
+"""CPU-side checks of bench.py's contract: the reference arm (the oracle on host cores) prints one JSON line with the
+keys the driver reads, and the product arm refuses to run without a CUDA device instead of falling back."""
+import json
+import subprocess
+import sys
+from pathlib import Path
+
+import pytest
+import torch
+
+ROOT = Path(__file__).resolve().parent.parent
+
+
+def _run(*args, env=None):
+    return subprocess.run([sys.executable, str(ROOT / "bench.py"), *args], capture_output=True, text=True, timeout=600,
+                          cwd=str(ROOT), env=env)
+
+
+def test_reference_arm_prints_the_contract_line():
+    r = _run("--impl", "reference", "--workload", "cfg1", "--steps", "1", "--warmup", "0")
+    assert r.returncode == 0, r.stderr[-2000:]
+    lines = [l for l in r.stdout.splitlines() if l.startswith("{")]
+    assert len(lines) == 1
+    d = json.loads(lines[0])
+    assert d["impl"] == "reference" and d["unit"] == "particles/s" and d["higher_is_better"] is True
+    assert d["metric"].startswith("particles/sec") and d["value"] > 0 and d["config"]["workload"] == "cfg1"
+    assert d["cpu_baseline"]["kind"] == "oracle" and d["cpu_baseline"]["cores"] == 1
+    assert d["e2e"] == {"value": d["value"], "unit": d["unit"], "h2d_bytes_per_step": 0, "d2h_bytes_per_step": 0}
+    assert d["gpu_launches"] == 0
+
+
+@pytest.mark.skipif(torch.cuda.is_available(), reason="only meaningful on a box without a GPU")
+def test_product_arm_fails_loudly_without_cuda():
+    r = _run("--workload", "cfg1", "--steps", "1", "--warmup", "0")
+    assert r.returncode != 0
+    assert "CUDA" in (r.stderr + r.stdout)
