@@ -39,6 +39,12 @@ __device__ __forceinline__ uint4 ld_stream16u(const uint4* p) {
     return v;
 }
 
+/* records are written once and read once by k_bin_apply: streaming stores, so that they do not push the counters of the
+ * direct rows out of L2 */
+__device__ __forceinline__ void st_stream16u(uint4* p, const uint4& v) {
+    asm volatile("st.global.cs.v4.u32 [%0], {%1, %2, %3, %4};" :: "l"(p), "r"(v.x), "r"(v.y), "r"(v.z), "r"(v.w) : "memory");
+}
+
 /* Shared-memory layout of k_bin_scatter (dynamic):
  *   cnt[NB] | qlen | pad | queue[NB] (u16) | buf[NB*C] (u16) | 64 B pad | tb[64][2R] (u64, hash tables, HM == 1)
  * All accesses of the hot loop use 32-bit shared-space addresses (no generic-to-shared conversion per access). */
@@ -213,7 +219,7 @@ k_bin_scatter(const __grid_constant__ PassParams P, const __grid_constant__ BinP
                     const uint4 v = *reinterpret_cast<const uint4*>(src + u * UNIT + l4 * 8);
                     const uint32_t at = base + u * UNIT;
                     if (at + UNIT <= B.cap) {
-                        *reinterpret_cast<uint4*>(B.bins + (uint64_t)bin * B.cap + at + l4 * 8) = v;
+                        st_stream16u(reinterpret_cast<uint4*>(B.bins + (uint64_t)bin * B.cap + at + l4 * 8), v);
                     } else {                                           // bin region full: apply directly
                         const uint32_t wds[4] = {v.x, v.y, v.z, v.w};
 #pragma unroll
