@@ -46,19 +46,32 @@ k_hist(const uint64_t* __restrict__ id, const uint32_t* __restrict__ ek, uint32_
 }
 
 /* In-place exclusive prefix sum of a[0..len) by one block of 1024 threads; *total_out (optional) = sum.
- * Tiles of 4096 words: coalesced 4-word loads per thread, warp-shuffle scans, a running carry between tiles. */
+ * Tiles of 16384 words: 16 words per thread (four 16-byte accesses when aligned), warp-shuffle scans, a running carry
+ * between tiles. */
+constexpr int EX_PER = 16;
 __global__ void __launch_bounds__(1024) k_exscan(uint32_t* __restrict__ a, uint32_t len, uint32_t* total_out) {
     __shared__ uint32_t wsum[32];
     __shared__ uint32_t s_carry;
     const uint32_t lane = threadIdx.x & 31u, warp = threadIdx.x >> 5;
     if (threadIdx.x == 0) s_carry = 0;
     __syncthreads();
-    for (uint32_t t0 = 0; t0 < len; t0 += 4096) {
-        const uint32_t i = t0 + threadIdx.x * 4;
-        uint32_t v[4];
+    const bool vec = (reinterpret_cast<uintptr_t>(a) & 15u) == 0;
+    for (uint32_t t0 = 0; t0 < len; t0 += 1024 * EX_PER) {
+        const uint32_t i = t0 + threadIdx.x * EX_PER;
+        uint32_t v[EX_PER];
+        if (vec && i + EX_PER <= len) {
 #pragma unroll
-        for (int k = 0; k < 4; ++k) v[k] = i + k < len ? a[i + k] : 0;
-        const uint32_t mine = v[0] + v[1] + v[2] + v[3];
+            for (int q = 0; q < EX_PER / 4; ++q) {
+                const uint4 u = reinterpret_cast<const uint4*>(a + i)[q];
+                v[4 * q] = u.x; v[4 * q + 1] = u.y; v[4 * q + 2] = u.z; v[4 * q + 3] = u.w;
+            }
+        } else {
+#pragma unroll
+            for (int k = 0; k < EX_PER; ++k) v[k] = i + k < len ? a[i + k] : 0;
+        }
+        uint32_t mine = 0;
+#pragma unroll
+        for (int k = 0; k < EX_PER; ++k) mine += v[k];
         uint32_t incl = mine;
 #pragma unroll
         for (int off = 1; off < 32; off <<= 1) {
@@ -77,12 +90,21 @@ __global__ void __launch_bounds__(1024) k_exscan(uint32_t* __restrict__ a, uint3
             wsum[lane] = wi - w;                                   // exclusive prefix of the warp totals
         }
         __syncthreads();
-        const uint32_t carry = s_carry;
-        uint32_t run = carry + wsum[warp] + incl - mine;
+        uint32_t run = s_carry + wsum[warp] + incl - mine;
 #pragma unroll
-        for (int k = 0; k < 4; ++k) {
-            if (i + k < len) a[i + k] = run;
-            run += v[k];
+        for (int k = 0; k < EX_PER; ++k) {
+            const uint32_t x = v[k];
+            v[k] = run;
+            run += x;
+        }
+        if (vec && i + EX_PER <= len) {
+#pragma unroll
+            for (int q = 0; q < EX_PER / 4; ++q)
+                reinterpret_cast<uint4*>(a + i)[q] = make_uint4(v[4 * q], v[4 * q + 1], v[4 * q + 2], v[4 * q + 3]);
+        } else {
+#pragma unroll
+            for (int k = 0; k < EX_PER; ++k)
+                if (i + k < len) a[i + k] = v[k];
         }
         __syncthreads();
         if (threadIdx.x == 1023) s_carry = run;                    // total up to the end of this tile
