@@ -249,7 +249,7 @@ struct BinPlan {
 int ilog2(uint64_t v) { return bit_length(v) - 1; }
 
 uint32_t staging_capacity(uint32_t threads, uint32_t SL) {
-    const double lambda = 2.0 * threads / SL;          /* records per bin, round and CTA (2 particles per thread) */
+    const double lambda = 2.0 * SCATTER_PAIRS_PER_ROUND * threads / SL;    /* records per bin, round and CTA */
     uint32_t C = (uint32_t)(32.0 + lambda + 6.0 * std::sqrt(lambda) + 8.0);
     C = (C + 7u) & ~7u;
     return C > 256 ? 256 : C;                          /* beyond: staging overflows go through red.global */

@@ -78,6 +78,7 @@ struct BinParams {
     uint32_t log2w;
     int32_t rows_direct;  // the first rows_direct rows of the pass use red.global instead of the bins
 };
+constexpr int SCATTER_PAIRS_PER_ROUND = 5;      // pairs of particles per thread between two flush phases of k_bin_scatter
 size_t scatter_smem_bytes(uint32_t nb, uint32_t C);
 cudaError_t launch_update_binned(const PassParams& P, const BinParams& B, const float* xyz, uint64_t n, int sm_count,
                                  cudaStream_t st);

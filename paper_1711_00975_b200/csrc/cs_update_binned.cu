@@ -27,6 +27,8 @@ namespace cs {
 
 constexpr int BIN_THREADS = 1024;
 constexpr uint32_t UNIT = 32;            // records per flush unit (64 bytes)
+// pairs of particles a thread bins between two flush phases: cs_internal.h SCATTER_PAIRS_PER_ROUND (the host sizes the
+// staging buffers with it)
 
 __device__ __forceinline__ float2 ld_stream8(const float2* p) {
     float2 v;
@@ -169,7 +171,8 @@ k_bin_scatter(const __grid_constant__ PassParams P, const __grid_constant__ BinP
     X.rows_direct = B.rows_direct;
 
     const float2* body = reinterpret_cast<const float2*>(xyz + 3 * (uint64_t)head);
-    const uint64_t per_round = (uint64_t)gridDim.x * NT;
+    const uint64_t per_sub = (uint64_t)gridDim.x * NT;                 // pairs of one sub-round over the grid
+    const uint64_t per_round = per_sub * SCATTER_PAIRS_PER_ROUND;
     const uint64_t rounds = (pairs + per_round - 1) / per_round;
     const uint32_t lane = threadIdx.x & 31u, warp = threadIdx.x >> 5;
     const uint32_t grp = lane >> 2, l4 = lane & 3u;
@@ -177,14 +180,17 @@ k_bin_scatter(const __grid_constant__ PassParams P, const __grid_constant__ BinP
 
     for (uint64_t r = 0; r < rounds; ++r) {
         if (threadIdx.x == 0) *qlen = 0;                               // last read before the previous barrier
-        const uint64_t g = r * per_round + (uint64_t)blockIdx.x * NT + threadIdx.x;
-        if (g < pairs) {
-            const float2 q0 = ld_stream8(body + 3 * g);
-            const float2 q1 = ld_stream8(body + 3 * g + 1);
-            const float2 q2 = ld_stream8(body + 3 * g + 2);
-            const uint64_t i0 = P.index0 + head + 2 * g;
-            if (!P.sample || keep_particle(P.K, i0, P.Tp)) bin_particle<R, HM>(P, X, q0.x, q0.y, q1.x);
-            if (!P.sample || keep_particle(P.K, i0 + 1, P.Tp)) bin_particle<R, HM>(P, X, q1.y, q2.x, q2.y);
+#pragma unroll 1
+        for (int u = 0; u < SCATTER_PAIRS_PER_ROUND; ++u) {
+            const uint64_t g = r * per_round + u * per_sub + (uint64_t)blockIdx.x * NT + threadIdx.x;
+            if (g < pairs) {
+                const float2 q0 = ld_stream8(body + 3 * g);
+                const float2 q1 = ld_stream8(body + 3 * g + 1);
+                const float2 q2 = ld_stream8(body + 3 * g + 2);
+                const uint64_t i0 = P.index0 + head + 2 * g;
+                if (!P.sample || keep_particle(P.K, i0, P.Tp)) bin_particle<R, HM>(P, X, q0.x, q0.y, q1.x);
+                if (!P.sample || keep_particle(P.K, i0 + 1, P.Tp)) bin_particle<R, HM>(P, X, q1.y, q2.x, q2.y);
+            }
         }
         __syncthreads();
         /* queue the bins that hold at least one full unit */
