@@ -34,8 +34,8 @@ CPU_BASELINE_SAMPLE = 1 << 23  # particles of the cpu_baseline leg (about 10-30 
 # dram__bytes_read.sum + dram__bytes_write.sum of one k_update launch from the committed `ncu --set full`
 # capture (profiles/), keyed by workload; None until a capture exists for that workload.
 # thread instructions per particle of the update-phase kernels (smsp__inst_executed.sum x 32 / particles), same capture
-NCU_UPDATE_INSTR_PER_PARTICLE = {"cfg3": 490 + 27}
-NCU_TRAFFIC_BYTES = {"cfg3": 39.7e9}     # profiles/r1_kernels_cfg3.md: 8 x (scatter + apply) launches per step
+NCU_UPDATE_INSTR_PER_PARTICLE = {"cfg3": 425 + 27}
+NCU_TRAFFIC_BYTES = {"cfg3": 32.4e9}     # profiles/r1_kernels_cfg3.md: 8 x (scatter + apply) launches per step
 
 
 def _peaks():
