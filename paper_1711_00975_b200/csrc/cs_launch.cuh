@@ -9,7 +9,7 @@
 namespace cs {
 
 /* Split n particles at xyz into (head, groups of 4, tail) so that the grouped part is 16-byte aligned. */
-static void split_aligned(const float* xyz, uint64_t n, uint32_t* head, uint64_t* groups) {
+static inline void split_aligned(const float* xyz, uint64_t n, uint32_t* head, uint64_t* groups) {
     /* xyz is 4-byte aligned (checked by the API), so one of the first four particles starts on a 16-byte line */
     uint32_t h = 0;
     uintptr_t a = reinterpret_cast<uintptr_t>(xyz);
