@@ -91,8 +91,10 @@ template <int HM>
 __device__ __forceinline__ void row_hashes(const RowCoef& rc, uint32_t c0, uint32_t c1, uint32_t tb_row_addr,
                                            uint32_t& h, uint32_t& sb) {
     if (HM == 1) {
-        h = affine_low32_tb(rc.h, c0, lds_u64(tb_row_addr));
-        sb = affine_low32_tb(rc.s, c0, lds_u64(tb_row_addr + 8)) & 1u;
+        uint64_t th, ts;                                  // both table entries of the row with one 16-byte load
+        asm volatile("ld.shared.v2.u64 {%0, %1}, [%2];" : "=l"(th), "=l"(ts) : "r"(tb_row_addr));
+        h = affine_low32_tb(rc.h, c0, th);
+        sb = affine_low32_tb(rc.s, c0, ts) & 1u;
     } else {
         h = affine_low32<HM == 2>(rc.h, c0, c1);
         sb = affine_low32<HM == 2>(rc.s, c0, c1) & 1u;
