@@ -34,3 +34,20 @@ def test_product_arm_fails_loudly_without_cuda():
     r = _run("--workload", "cfg1", "--steps", "1", "--warmup", "0")
     assert r.returncode != 0
     assert "CUDA" in (r.stderr + r.stdout)
+
+
+def test_reference_arm_under_torchrun_only_rank0_works():
+    """N > 1: the driver launches the reference arm with torchrun; rank 0 alone runs and prints, the others exit 0."""
+    import socket
+    with socket.socket() as s:
+        s.bind(("127.0.0.1", 0))
+        port = s.getsockname()[1]
+    r = subprocess.run([sys.executable, "-m", "torch.distributed.run", "--nnodes=1", "--nproc-per-node", "2",
+                        "--master-addr", "127.0.0.1", "--master-port", str(port), str(ROOT / "bench.py"), "--gpus", "2",
+                        "--impl", "reference", "--workload", "cfg1", "--steps", "1", "--warmup", "0"],
+                       capture_output=True, text=True, timeout=900, cwd=str(ROOT))
+    assert r.returncode == 0, r.stderr[-2000:]
+    lines = [l for l in r.stdout.splitlines() if l.startswith("{")]
+    assert len(lines) == 1
+    d = json.loads(lines[0])
+    assert d["impl"] == "reference" and d["n_gpus"] == 2
