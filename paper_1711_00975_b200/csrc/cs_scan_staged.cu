@@ -253,6 +253,7 @@ k_stage_first_cb(const __grid_constant__ PassParams P, const __grid_constant__ S
             c[1] = cell_of(q0.w, q1.x, q1.y, P.sc[0]);
             c[2] = cell_of(q1.z, q1.w, q2.x, P.sc[0]);
             c[3] = cell_of(q2.y, q2.z, q2.w, P.sc[0]);
+            uint32_t live4 = 0, fails4 = 0;
             /* two particles at a time (64 registers per thread at 1024 threads): hashes, coarse bits from shared
              * memory, then the fine words of the undecided rows, all in flight together */
 #pragma unroll
@@ -282,15 +283,25 @@ k_stage_first_cb(const __grid_constant__ PassParams P, const __grid_constant__ S
                     uint32_t fails = 0;
 #pragma unroll
                     for (int j = 0; j < FIRST; ++j) fails += 1u - ((wd[q][j] >> (h[q][j] & 31u)) & 1u);
-                    const bool live = keep[2 * half + q] && fails < (uint32_t)FIRST;  // FIRST = rank + 1 fails reject
-                    const uint32_t mask = __ballot_sync(0xFFFFFFFFu, live);
-                    if (mask) {
-                        const int leader = __ffs(mask) - 1;
-                        uint32_t base = 0;
-                        if ((int)lane == leader) base = atomicAdd(&s_cnt, (uint32_t)__popc(mask));
-                        base = __shfl_sync(0xFFFFFFFFu, base, leader);
-                        if (live) out[base + __popc(mask & below)] = c[2 * half + q] | ((uint64_t)fails << FAIL_SHIFT);
+                    if (keep[2 * half + q] && fails < (uint32_t)FIRST) {              // FIRST = rank + 1 fails reject
+                        live4 |= 1u << (2 * half + q);
+                        fails4 |= fails << (8 * (2 * half + q));
                     }
+                }
+            }
+            /* one reservation in the segment for the survivors among this warp's 128 particles */
+            uint32_t m[4], tot = 0;
+#pragma unroll
+            for (int q = 0; q < 4; ++q) { m[q] = __ballot_sync(0xFFFFFFFFu, (live4 >> q) & 1u); tot += __popc(m[q]); }
+            if (tot) {
+                uint32_t base = 0;
+                if (lane == 0) base = atomicAdd(&s_cnt, tot);
+                base = __shfl_sync(0xFFFFFFFFu, base, 0);
+#pragma unroll
+                for (int q = 0; q < 4; ++q) {
+                    if ((live4 >> q) & 1u)
+                        out[base + __popc(m[q] & below)] = c[q] | ((uint64_t)((fails4 >> (8 * q)) & 0xFFu) << FAIL_SHIFT);
+                    base += __popc(m[q]);
                 }
             }
         }
