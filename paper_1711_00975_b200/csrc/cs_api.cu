@@ -203,9 +203,13 @@ int read_states(cs_sketch* s) {
 
 /* Sort + dedupe + cut the candidate list of one scale (device side only; caller reads the states back). */
 int compact_scale(cs_sketch* s, int i) {
+    const uint32_t n = s->st_host[i].count < s->cap ? s->st_host[i].count : s->cap;
+    cudaError_t e = launch_est_range(s->sb[i].ek[s->cur[i]], n, s->st_dev + i, s->stream);
+    if (e != cudaSuccess) return fail(CS_ERR_CUDA, "range kernel: %s", cudaGetErrorString(e));
+    s->launches += n ? 2 : 1;
+    int rc = read_states(s);          /* the number of radix passes over the estimate depends on its range */
+    if (rc) return rc;
     const ScanState& h = s->st_host[i];
-    const uint32_t n = h.count < s->cap ? h.count : s->cap;
-    cudaError_t e;
     s->cur[i] = select_compact(s->sb[i], s->cur[i], n, s->id_bits[i], h.est_min, h.est_max, s->st_dev + i, s->k_max,
                                s->thr_min, s->stream, &s->launches, &e);
     if (e != cudaSuccess) return fail(CS_ERR_CUDA, "select_compact: %s", cudaGetErrorString(e));

@@ -134,6 +134,8 @@ struct SelectBuffers {
     uint32_t* scratch;
 };
 uint64_t select_scratch_words(uint64_t n);
+/* st->est_min / est_max = range of the estimates of the first n (unsorted) entries */
+cudaError_t launch_est_range(const uint32_t* ek, uint32_t n, ScanState* st_dev, cudaStream_t st);
 /* returns the index (0/1) of the half that holds the result; *launches += kernels launched */
 int select_compact(const SelectBuffers& B, int src, uint32_t n, int id_bits, int32_t est_min, int32_t est_max,
                    ScanState* st_dev, uint64_t k_max, int32_t thr_min, cudaStream_t stream, uint64_t* launches,

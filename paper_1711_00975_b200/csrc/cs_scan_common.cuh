@@ -57,20 +57,17 @@ __device__ __forceinline__ int32_t estimate_full(const PassParams& P, int s, uin
     return est;
 }
 
-/* Warp-aggregated append of (c, est) to the candidate list of one scale.  Must be reached by all 32 lanes. */
+/* Warp-aggregated append of (c, est) to the candidate list of one scale.  Must be reached by all 32 lanes.
+ * One global atomic per warp that has something to append; the estimate range of the list (which bounds the radix
+ * passes of the selector) is computed when the list is compacted (k_est_range), not here: three atomics per append on
+ * the one sector that holds the ScanState serialise at the L2 when many cells qualify (cfg 5: 3e5 appends per launch). */
 __device__ __forceinline__ void append_candidate(const ScanTarget& tg, bool emit, uint64_t c, int32_t est) {
     const uint32_t mask = __ballot_sync(0xFFFFFFFFu, emit);
     if (mask == 0) return;
     const uint32_t lane = threadIdx.x & 31u;
     const int leader = __ffs(mask) - 1;
-    int32_t lo = __reduce_min_sync(0xFFFFFFFFu, emit ? est : INT32_MAX);
-    int32_t hi = __reduce_max_sync(0xFFFFFFFFu, emit ? est : INT32_MIN);
     uint32_t base = 0;
-    if ((int)lane == leader) {
-        base = atomicAdd(&tg.st->count, (uint32_t)__popc(mask));
-        atomicMin(&tg.st->est_min, lo);
-        atomicMax(&tg.st->est_max, hi);
-    }
+    if ((int)lane == leader) base = atomicAdd(&tg.st->count, (uint32_t)__popc(mask));
     base = __shfl_sync(0xFFFFFFFFu, base, leader);
     if (emit) {
         uint64_t pos = (uint64_t)base + __popc(mask & ((1u << lane) - 1u));

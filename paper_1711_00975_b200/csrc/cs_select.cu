@@ -165,6 +165,38 @@ k_scatter(const uint64_t* __restrict__ sid, const uint32_t* __restrict__ sek, ui
     }
 }
 
+/* ---- estimate range of an unsorted list (bounds the radix passes over the estimate key) -------------------------- */
+
+__global__ void k_est_range_init(ScanState* st) {
+    st->est_min = INT32_MAX;
+    st->est_max = INT32_MIN;
+}
+
+__global__ void __launch_bounds__(256) k_est_range(const uint32_t* __restrict__ ek, uint32_t n, ScanState* st) {
+    uint32_t lo = 0xFFFFFFFFu, hi = 0;                     // keys: ascending key = descending estimate
+    const uint32_t stride = gridDim.x * 256;
+    for (uint32_t i = blockIdx.x * 256 + threadIdx.x; i < n; i += stride) {
+        const uint32_t k = ek[i];
+        lo = min(lo, k); hi = max(hi, k);
+    }
+    lo = __reduce_min_sync(0xFFFFFFFFu, lo);
+    hi = __reduce_max_sync(0xFFFFFFFFu, hi);
+    if ((threadIdx.x & 31) == 0 && lo <= hi) {
+        atomicMax(&st->est_max, key_to_est(lo));
+        atomicMin(&st->est_min, key_to_est(hi));
+    }
+}
+
+cudaError_t launch_est_range(const uint32_t* ek, uint32_t n, ScanState* st_dev, cudaStream_t st) {
+    k_est_range_init<<<1, 1, 0, st>>>(st_dev);
+    if (n) {
+        uint32_t blocks = (n + 255) / 256;
+        if (blocks > 148 * 4) blocks = 148 * 4;
+        k_est_range<<<blocks, 256, 0, st>>>(ek, n, st_dev);
+    }
+    return cudaGetLastError();
+}
+
 /* ---- duplicate removal on the sorted list --------------------------------------------------------------- */
 
 __device__ __forceinline__ bool is_first(const uint64_t* id, uint32_t i) { return i == 0 || id[i] != id[i - 1]; }
