@@ -17,10 +17,12 @@
  *   - The caller owns every input / output buffer.  The handle owns the counter tables, the candidate buffers,
  *     the staging ring and all scratch; cs_destroy frees them.
  *   - All device work is enqueued on the handle's stream (cs_set_stream; default: the legacy default stream).
- *     cs_update / cs_estimate / cs_sketch_add / cs_reset do not synchronise.  cs_update_host returns after the
- *     last host->device copy has been issued and waited for (the host buffer may then be reused); cs_scan*,
- *     cs_topk, cs_excursion, cs_sketch_read, cs_scan_stats synchronise the stream because they hand
- *     host-visible results or sizes back.
+ *     cs_estimate / cs_sketch_add / cs_reset do not synchronise.  cs_update is asynchronous except that it waits for
+ *     the stream when it (re)allocates its record scratch (first large call) and, for sample_p < 0.5, once per 2^28
+ *     particles to read back the number of kept particles.  cs_update_host returns after the last host->device copy
+ *     has been issued and waited for (the host buffer may then be reused); cs_scan*, cs_topk, cs_excursion,
+ *     cs_recount, cs_sketch_read, cs_scan_stats synchronise the stream because they hand host-visible results or
+ *     sizes back.
  *   - Positions are an array of structures: float32 x,y,z per particle, 12 bytes per particle, at least
  *     4-byte aligned (16-byte aligned input takes the fully vectorised path from its first particle).
  *   - There is no CPU fallback: every step below runs in CUDA kernels of this library; without a usable
