@@ -600,6 +600,39 @@ def test_recount_and_membership_filter(cs):
     g.close()
 
 
+# ---- randomised sweep over shapes, modes and call splits --------------------------------------------------------------
+
+@pytest.mark.parametrize("seed", [101, 102])
+def test_randomised_shapes_modes_and_splits(cs, seed):
+    """40 random cases per seed: d, w (power of two or not), 1-3 nested or unrelated meshes, n, sample_p, k, thresholds,
+    update mode / direct rows, scan mode, Count-Min, candidate capacity, table budget, a random split of the stream into
+    two calls.  (2100 cases of the same generator ran clean during round 1.)"""
+    from paper_1711_00975_b200 import synth
+    rng = np.random.default_rng(seed)
+    for case in range(40):
+        d = int(rng.integers(1, 11))
+        w = int(2 ** rng.integers(8, 21)) if rng.random() < 0.8 else int(rng.integers(300, 100000))
+        ns = int(rng.integers(1, 4)) if d <= 8 else 1
+        base = int(rng.choice([1, 3, 8, 33, 64, 250, 1024, 4000, 4642, 30000, 1 << 17]))
+        G = tuple(sorted({max(1, min(base * m, 1 << 20)) for m in rng.choice([1, 2, 4, 8], size=ns)}))
+        n = int(rng.choice([1, 5, 1000, 40001, 150000, 300003, 1200001], p=[.1, .1, .15, .25, .2, .15, .05]))
+        p = float(rng.choice([1.0, 1.0, 0.7, 0.3, 0.05]))
+        k = int(rng.choice([0, 1, 10, 500, 5000]))
+        thr = tuple(int(x) for x in rng.choice([-2, 0, 1, 2, 3, 5, 9], size=int(rng.integers(0, 3)), replace=False))
+        if k == 0 and not thr:
+            thr = (2,)
+        wl = synth.Workload("rs", N=n, G=G, d=d, w=w, k=max(k, 1), H=int(rng.choice([1, 8, 64])),
+                            f_bg=float(rng.choice([0.0, 0.3, 1.0])), m_min=0, L=100.0, seed=int(rng.integers(0, 2 ** 40)),
+                            gen_seed=seed * 1000 + case, sigma_mult=float(rng.choice([1.0, 0.05])))
+        xyz = synth.generate(wl, device="cuda")
+        _check_all(cs, wl, xyz, sample_p=p, k=k, thresholds=thr, probe_cells=64,
+                   split=[int(rng.integers(0, n + 1))] if rng.random() < 0.7 else None,
+                   cap=1024 if rng.random() < 0.3 else None,
+                   budget=int(rng.integers(1, d + 1)) * w * 4 if rng.random() < 0.3 else None,
+                   mode=(int(rng.integers(0, 3)), int(rng.integers(-1, 4))), scan_mode=int(rng.integers(0, 4)),
+                   counting=int(rng.random() < 0.25))
+
+
 # ---- BASELINE.json full size (cfg 3: 2^30 particles), in the launch configuration bench.py times ------------------
 
 def test_cfg3_full_size_properties(cs):
