@@ -11,7 +11,8 @@
  * Conventions for every call
  *   - extern "C", returns an int status: CS_OK (0) or a negative CS_ERR_* code.  Nothing throws, aborts or
  *     prints.  cs_last_error() returns a thread-local, NUL-terminated message for the last failing call.
- *   - "dev" pointers are CUDA device memory on the current device; "host" pointers are host memory (pinned
+ *   - "dev" pointers are CUDA device memory on the handle's device (the device that was current at cs_create; every
+ *     call switches to it for its duration and restores the caller's current device); "host" pointers are host memory (pinned
  *     memory makes the host-streamed calls asynchronous, pageable memory is accepted and slower); "any"
  *     pointers may be either (the library copies with cudaMemcpyDefault).
  *   - The caller owns every input / output buffer.  The handle owns the counter tables, the candidate buffers,
@@ -109,6 +110,28 @@ int cs_set_stream(cs_sketch* s, void* cuda_stream);
  * that the red.global.add traffic of each pass stays L2-resident.  The result does not depend on it. */
 int cs_set_table_budget(cs_sketch* s, uint64_t bytes);
 
+/* How the passes cut one call into launches (0 = keep the current value); the result never depends on it.
+ *   stage_particles  particles per batch of the host-streamed calls = size of one slot of the device staging ring
+ *                    (default 2^24: 3 slots x 192 MiB); changing it frees the ring, which is re-allocated on use
+ *   update_chunk     particles per scatter/apply pair of the binned update (default 2^27; record scratch ~ 8 B each)
+ *   scan_chunk       most particles one re-scan launch covers (default 2^27)
+ *   compact_chunk    particles per sampling-compaction launch when sample_p < 0.5 (default 2^28)
+ * Each a multiple of 4 in [64, 2^30].  Small values make short streams take the multi-batch paths (tests do). */
+int cs_set_chunk_sizes(cs_sketch* s, uint64_t stage_particles, uint64_t update_chunk, uint64_t scan_chunk,
+                       uint64_t compact_chunk);
+
+/* Replay cache (default 0 = off).  With bytes > 0 the handle may hold up to that much device memory with what the last
+ * cs_update* calls read, so that the re-scan of the SAME buffer does not fetch it again:
+ *   - cs_update_host / cs_update_records_host of a buffer of at most `bytes` copy it into one device buffer instead of
+ *     the staging ring; a following cs_scan_host / cs_scan_records_host with the same host address and length reads
+ *     that copy: the stream crosses PCIe once per update + re-scan instead of twice;
+ *   - for sample_p < 0.5 the kept particles that cs_update* compacted stay on the device (12 B each); a cs_scan* call
+ *     with the same address, length, sample_p and running index re-scans them without a second sampling pass.
+ * The caller promises that such a buffer still holds the same particles when it is passed to cs_scan*.  Every
+ * cs_update* call refreshes what is held for its buffer; cs_reset drops the kept particles.  Synchronises; frees what
+ * was held. */
+int cs_set_replay_cache(cs_sketch* s, uint64_t bytes);
+
 /* How cs_update applies the counter updates.  The result never depends on it.
  *   mode 1 "direct": one red.global.add.s32 per (particle, row) into L2-resident row groups (table budget above).
  *   mode 2 "binned": updates are first written as 2-byte records partitioned by table slice, then applied slice by
@@ -179,9 +202,9 @@ int cs_estimate(cs_sketch* s, int scale, const uint64_t* cells_dev, uint64_t m, 
  * cs_update): every kept particle's cell is estimated against the CURRENT tables; cells whose estimate can
  * still matter are collected, deduplicated and kept ordered by (estimate descending, cell id ascending).
  * The tables must not change between cs_scan_begin and the last cs_topk / cs_excursion. */
-int cs_scan_begin(cs_sketch* s, uint64_t k_max, int32_t thr_min);
+int cs_scan_begin(cs_sketch* s, uint64_t k_max, int32_t thr_min);   /* k_max <= 2^26, else CS_ERR_ARG */
 /* Initial capacity (entries per scale, a power of two in [2^10, 2^30]; default 2^22) of the candidate list the
- * next cs_scan_begin allocates: max(entries, 16*k_max rounded up to a power of two).  The list still grows by
+ * next cs_scan_begin allocates: max(entries, 16*k_max rounded up to a power of two) <= 2^30.  The list still grows by
  * doubling when the cells that must be kept do not fit; a small value only costs more compactions. */
 int cs_set_candidate_capacity(cs_sketch* s, uint64_t entries);
 int cs_scan(cs_sketch* s, const float* xyz_dev, uint64_t n, double sample_p);
@@ -223,6 +246,13 @@ int cs_excursion(cs_sketch* s, int scale, int32_t thr, uint64_t cap, uint64_t* i
 int cs_recount(cs_sketch* s, int scale, const uint64_t* ids_dev, uint64_t m, const float* xyz_dev, uint64_t n,
                uint32_t* counts_dev, float* xyz_out_dev, uint64_t cap, uint64_t* n_out);
 
+/* 26-neighbour shell of m cells of `scale` on the periodic mesh (Fig. 14: keep the particles of the
+ * heavy cells AND THEIR SURROUNDINGS for an offline halo finder): ids_out_dev[27*i + t], t = (dx+1) + 3*(dy+1) + 9*(dz+1)
+ * with dx, dy, dz in {-1, 0, 1}, = the cell at that offset from ids_dev[i], coordinates wrapped modulo G (t = 13 is the
+ * cell itself).  Feed the result to cs_recount (duplicates are harmless there).  Device pointers; ids < G^3;
+ * m <= 2^32; asynchronous on the handle's stream. */
+int cs_expand_neighbours(cs_sketch* s, int scale, const uint64_t* ids_dev, uint64_t m, uint64_t* ids_out_dev);
+
 /* out4[0] = candidates currently held, out4[1] = current collection threshold tau as (uint64)(int64)tau,
  * out4[2] = compactions run since cs_scan_begin, out4[3] = scan kernel launches since cs_scan_begin. */
 int cs_scan_stats(cs_sketch* s, int scale, uint64_t* out4_host);
@@ -236,7 +266,9 @@ int cs_coeffs(cs_sketch* s, int scale, uint64_t* out_4d_host, uint64_t* K_out_ho
 /* Number of kernels this handle has launched since create (bench.py's gpu_launches). */
 int cs_launch_count(cs_sketch* s, uint64_t* n_out);
 
-/* ---- measurement probes (the roofline denominators are measured, not assumed) ------------- */
+/* ---- measurement probes (the roofline denominators are measured, not assumed) -------------
+ * NOT part of the product path: no other call of this library uses them; bench.py calls them to measure the peaks
+ * its roofline fractions are quoted against.  They take no handle and run on the current device. */
 
 /* Issues n_ops red.global.add.s32 (mode 0), returning atom.global.add.s32 (mode 1) or 4-byte ld.global
  * gathers (mode 2) to addresses generated in registers, uniform over a table of table_bytes, from all SMs,

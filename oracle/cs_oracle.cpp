@@ -20,6 +20,8 @@
  *                                 (R10), selection made deterministic
  *                                 (R9), excursion set = all cells with
  *                                 estimate >= threshold (R8)
+ *   ora_select_streaming          the same selection over one shard of the stream in O(k) memory (full-size
+ *                                 parity by shards; mergeability PAPER.md:578)
  *   ora_full_search_topk          Alg. 1 l.7-13 (CSFS query: Estimate every j in [n])
  *   ora_exact_counts              exact counting, PAPER.md:398-402 (the brute-force pin)
  *   ora_update_records / ora_scan_records / ora_cells_of_records
@@ -383,6 +385,41 @@ int ora_topk_streaming(Oracle* o, int scale, const float* xyz, uint64_t n, doubl
     uint64_t m = 0;
     for (const auto& e : best) { ids_out[m] = e.second; est_out[m] = e.first; ++m; }
     *n_out = m;
+    return ORA_OK;
+}
+
+/* Streaming selection over ONE SHARD of a replayed stream (full-size parity runs the oracle over disjoint
+ * index ranges and merges the results with the same rule): the particles xyz[0..n) carry the running indices
+ * index0 .. index0 + n - 1.  One replayed particle at a time, against the tables as they stand (a shard run first sums
+ * the tables of all shards with ora_sketch_add), it keeps
+ *   (a) the k best distinct cells seen, in (est desc, id asc) order -- what ora_scan + ora_topk give on this shard;
+ *   (b) every distinct cell with estimate >= thr, same order       -- what ora_scan + ora_excursion give on this shard;
+ * in O(k + |b|) memory instead of the set of all scanned cells.  thr = INT32_MAX asks for no excursion set. */
+int ora_select_streaming(Oracle* o, int scale, const float* xyz, uint64_t n, uint64_t index0, double sample_p, uint64_t k,
+                         int32_t thr, uint64_t cap_x, uint64_t* ids_k, int32_t* est_k, uint64_t* n_k, uint64_t* ids_x,
+                         int32_t* est_x, uint64_t* n_x) {
+    if (!o || scale < 0 || scale >= (int)o->sc.size() || bad_p(sample_p) || !n_k || !n_x || (!xyz && n)) return ORA_ERR_ARG;
+    const Scale& S = o->sc[(size_t)scale];
+    std::set<std::pair<int32_t, uint64_t>, Better> best, above;
+    for (uint64_t i = 0; i < n; ++i) {
+        if (!keep_particle(o->K, index0 + i, sample_p)) continue;
+        uint64_t c = cell_of(xyz + 3 * i, S.scale, S.G);
+        int32_t e = estimate_cell(o, S, c);
+        if (k) {
+            best.insert(std::make_pair(e, c));
+            if (best.size() > k) best.erase(std::prev(best.end()));
+        }
+        if (thr != INT32_MAX && e >= thr) above.insert(std::make_pair(e, c));
+    }
+    uint64_t m = 0;
+    for (const auto& e : best) { ids_k[m] = e.second; est_k[m] = e.first; ++m; }
+    *n_k = m;
+    m = 0;
+    for (const auto& e : above) {
+        if (m < cap_x) { ids_x[m] = e.second; est_x[m] = e.first; }
+        ++m;
+    }
+    *n_x = m;
     return ORA_OK;
 }
 

@@ -68,6 +68,7 @@ def lib():
             "ora_topk": (ci, [vp, ci, u64, vp, vp, vp]),
             "ora_excursion": (ci, [vp, ci, i32, u64, vp, vp, vp]),
             "ora_topk_streaming": (ci, [vp, ci, vp, u64, dbl, u64, vp, vp, vp]),
+            "ora_select_streaming": (ci, [vp, ci, vp, u64, u64, dbl, u64, i32, u64, vp, vp, vp, vp, vp, vp]),
             "ora_full_search_topk": (ci, [vp, ci, u64, vp, vp, vp]),
             "ora_sketch_read": (ci, [vp, ci, vp]),
             "ora_sketch_add": (ci, [vp, ci, vp]),
@@ -259,6 +260,24 @@ class OracleSketch:
         _chk(lib().ora_topk_streaming(self._h, scale, _ptr(p), p.shape[0], sample_p, k, _ptr(ids), _ptr(est),
                                       C.byref(n)), "topk_streaming")
         return ids[: n.value].copy(), est[: n.value].copy()
+
+    def select_streaming(self, xyz, index0: int, k: int, thr: int = INT32_MAX, sample_p: float = 1.0, scale: int = 0):
+        """One shard of a replayed stream (running indices index0 ..): (top-k ids, est), (excursion ids, est) of the
+        shard against the tables as they stand, in O(k + excursion) memory."""
+        p = _xyz(xyz)
+        ids = np.empty(max(k, 1), dtype=np.uint64)
+        est = np.empty(max(k, 1), dtype=np.int32)
+        nk, nx = C.c_uint64(0), C.c_uint64(0)
+        cap = 1 << 16
+        while True:
+            xi = np.empty(cap, dtype=np.uint64)
+            xe = np.empty(cap, dtype=np.int32)
+            _chk(lib().ora_select_streaming(self._h, scale, _ptr(p), p.shape[0], index0, sample_p, k, thr, cap, _ptr(ids),
+                                            _ptr(est), C.byref(nk), _ptr(xi), _ptr(xe), C.byref(nx)), "select_streaming")
+            if nx.value <= cap:
+                break
+            cap = int(nx.value)
+        return (ids[: nk.value].copy(), est[: nk.value].copy()), (xi[: nx.value].copy(), xe[: nx.value].copy())
 
     def full_search_topk(self, k: int, scale: int = 0):
         ids = np.empty(max(k, 1), dtype=np.uint64)

@@ -30,6 +30,8 @@ SIGNATURES = {
     "cs_reset": (ci, [vp]),
     "cs_set_stream": (ci, [vp, vp]),
     "cs_set_table_budget": (ci, [vp, u64]),
+    "cs_set_chunk_sizes": (ci, [vp, u64, u64, u64, u64]),
+    "cs_set_replay_cache": (ci, [vp, u64]),
     "cs_set_update_mode": (ci, [vp, ci, ci]),
     "cs_set_counting_mode": (ci, [vp, ci]),
     "cs_set_scan_mode": (ci, [vp, ci]),
@@ -54,6 +56,7 @@ SIGNATURES = {
     "cs_topk": (ci, [vp, ci, u64, vp, vp, vp]),
     "cs_excursion": (ci, [vp, ci, i32, u64, vp, vp, vp]),
     "cs_recount": (ci, [vp, ci, vp, u64, vp, u64, vp, vp, u64, vp]),
+    "cs_expand_neighbours": (ci, [vp, ci, vp, u64, vp]),
     "cs_scan_stats": (ci, [vp, ci, vp]),
     "cs_sketch_read": (ci, [vp, ci, vp]),
     "cs_sketch_add": (ci, [vp, ci, vp]),
@@ -164,6 +167,12 @@ class CountSketch:
 
     def set_table_budget(self, nbytes: int):
         _chk(lib().cs_set_table_budget(self._h, nbytes), "cs_set_table_budget")
+
+    def set_chunk_sizes(self, stage_particles: int = 0, update_chunk: int = 0, scan_chunk: int = 0, compact_chunk: int = 0):
+        _chk(lib().cs_set_chunk_sizes(self._h, stage_particles, update_chunk, scan_chunk, compact_chunk), "cs_set_chunk_sizes")
+
+    def set_replay_cache(self, nbytes: int):
+        _chk(lib().cs_set_replay_cache(self._h, nbytes), "cs_set_replay_cache")
 
     def set_update_mode(self, mode: int, rows_direct: int = -1):
         _chk(lib().cs_set_update_mode(self._h, mode, rows_direct), "cs_set_update_mode")
@@ -293,6 +302,15 @@ class CountSketch:
                               vp(out.data_ptr()) if out is not None else None, extract_cap, C.byref(nm)), "cs_recount")
         k = min(int(nm.value), extract_cap)
         return counts[:m], (out[:k] if out is not None else None), int(nm.value)
+
+    def expand_neighbours(self, ids: torch.Tensor, scale: int = 0) -> torch.Tensor:
+        """(m, 27) tensor: the 26-neighbour shell (periodic) of each cell, column 13 = the cell itself."""
+        if not ids.is_cuda or ids.dtype not in (torch.int64, torch.uint64) or not ids.is_contiguous():
+            raise ValueError("ids must be a contiguous CUDA int64/uint64 tensor")
+        out = torch.empty((ids.numel(), 27), dtype=torch.int64, device=ids.device)
+        _chk(lib().cs_expand_neighbours(self._h, scale, vp(ids.data_ptr()), ids.numel(), vp(out.data_ptr())),
+             "cs_expand_neighbours")
+        return out
 
     def scan_stats(self, scale: int = 0) -> dict:
         out = (u64 * 4)()

@@ -9,6 +9,7 @@
 #include <cstdio>
 #include <cstring>
 #include <new>
+#include <vector>
 
 #include "cs_internal.h"
 
@@ -67,9 +68,11 @@ int bit_length(uint64_t v) {
 }
 
 constexpr int STAGE_SLOTS = 3;
-constexpr uint64_t STAGE_PARTICLES = 1ull << 24;      /* 192 MiB per staging slot */
-constexpr uint64_t MAX_CHUNK = 1ull << 27;            /* particles per scan launch */
+constexpr uint64_t STAGE_PARTICLES = 1ull << 24;      /* default particles per staging slot (192 MiB) */
+constexpr uint64_t MAX_CHUNK = 1ull << 27;            /* default particles per scan launch */
 constexpr uint32_t MIN_CAP = 1u << 22;                /* candidate entries per scale */
+constexpr uint64_t BIN_CHUNK = 1ull << 27;            /* default particles per scatter/apply pair of the binned update */
+constexpr uint64_t COMPACT_CHUNK = 1ull << 28;        /* default particles per sampling-compaction launch */
 
 }  // namespace
 
@@ -85,6 +88,8 @@ struct cs_sketch {
     cudaStream_t stream = nullptr;
     uint64_t upd_index = 0, scan_index = 0, launches = 0;
     uint64_t table_budget = 64ull << 20;   /* bytes of counters one update pass may touch (cs_set_table_budget) */
+    /* cs_set_chunk_sizes: how the passes cut a call into launches (the result never depends on them) */
+    uint64_t stage_particles = STAGE_PARTICLES, bin_chunk = BIN_CHUNK, scan_chunk = MAX_CHUNK, compact_chunk = COMPACT_CHUNK;
 
     /* candidate collection */
     bool scanning = false;
@@ -128,16 +133,60 @@ struct cs_sketch {
     uint64_t kept_cap = 0;             /* particles */
 
     /* packed records: positions of one batch unpacked to cell centres of the finest mesh */
-    float* unpacked = nullptr;         /* STAGE_PARTICLES particles */
+    float* unpacked = nullptr;
+    uint64_t unpacked_alloc = 0;       /* particles */
+
+    /* scratch kept between calls: hash table of cs_recount, id expansion of cs_scan_children / cs_expand_neighbours */
+    uint64_t* ht_keys = nullptr;
+    uint32_t* ht_vals = nullptr;
+    uint64_t ht_size = 0;              /* slots allocated */
+    uint64_t* ids_scratch = nullptr;
+    uint64_t ids_scratch_cap = 0;      /* ids */
 
     /* survivor lists of the row-partitioned scan */
     StageBuffers stb = {};
 
     /* host streaming */
     float* stage[STAGE_SLOTS] = {};
+    uint64_t stage_alloc = 0;          /* particles each allocated slot holds */
     cudaStream_t copy_stream = nullptr;
     cudaEvent_t ev_full[STAGE_SLOTS] = {}, ev_free[STAGE_SLOTS] = {};
+
+    /* replay cache (cs_set_replay_cache): what the last update call read, kept for the re-scan of the same buffer */
+    uint64_t replay_limit = 0;         /* bytes of device memory the handle may hold for it; 0 = off */
+    unsigned char* host_cache = nullptr;   /* raw batches of the last host-streamed update call */
+    uint64_t host_cache_bytes = 0;     /* allocated */
+    const void* hc_host = nullptr;     /* key: host address, items, bytes per item */
+    uint64_t hc_n = 0;
+    size_t hc_bpp = 0;
+    bool hc_valid = false;
+    float* kept_arena = nullptr;       /* kept particles of sampled update calls, segment after segment */
+    uint64_t kept_arena_cap = 0, kept_arena_used = 0;   /* particles */
+    struct KeptSeg { const float* src; uint64_t n, index0; double p; uint64_t off, cnt; };
+    std::vector<KeptSeg> kept_segs;
 };
+
+/* Every entry point that takes a handle runs on the handle's device, whatever device is current (and restores it). */
+struct DeviceGuard {
+    int prev = -1;
+    bool switched = false;
+    cudaError_t err = cudaSuccess;
+    explicit DeviceGuard(const cs_sketch* s) {
+        err = cudaGetDevice(&prev);
+        if (err == cudaSuccess && s && prev != s->device) {
+            err = cudaSetDevice(s->device);
+            switched = err == cudaSuccess;
+        }
+    }
+    ~DeviceGuard() { if (switched) cudaSetDevice(prev); }
+    DeviceGuard(const DeviceGuard&) = delete;
+    DeviceGuard& operator=(const DeviceGuard&) = delete;
+};
+#define CS_ENTER(s)                                                                                    \
+    if (!(s)) return fail(CS_ERR_ARG, "null handle");                                                  \
+    DeviceGuard guard_(s);                                                                             \
+    if (guard_.err != cudaSuccess) return fail(CS_ERR_CUDA, "cannot switch to the handle's device %d: %s", \
+                                                (s)->device, cudaGetErrorString(guard_.err))
 
 namespace {
 
@@ -241,7 +290,6 @@ bool bad_p(double p) { return !(p > 0.0) || p > 1.0; }
 /* ---- binned update: plan + passes (kernels in cs_update_binned.cu) -------------------- */
 
 constexpr uint32_t BIN_MAX = 4096;                    /* bins per pass (words of `cursor`) */
-constexpr uint64_t BIN_CHUNK = 1ull << 27;            /* particles per scatter/apply pair */
 constexpr uint64_t BIN_MIN_N = 1ull << 22;            /* auto mode: below this the direct kernel is as fast */
 constexpr size_t BIN_SMEM = 200 * 1024;               /* shared memory of one scatter CTA */
 
@@ -303,7 +351,8 @@ bool bin_plan(const cs_sketch* s, BinPlan* pl) {
 int update_binned(cs_sketch* s, const BinPlan& pl, const float* xyz, uint64_t n, uint64_t index0, double sample_p) {
     const PassParams full = pass_params(s, index0, sample_p);
     const int each = pl.rows_per_pass;
-    const uint64_t chunk_max = n < BIN_CHUNK ? n : BIN_CHUNK;
+    const uint64_t BC = s->bin_chunk;
+    const uint64_t chunk_max = n < BC ? n : BC;
     const double keep = sample_p < 1.0 ? sample_p : 1.0;
     uint64_t cap = (uint64_t)((double)chunk_max * keep / pl.SL * 1.04) + 2048;
     cap = (cap + 31) & ~(uint64_t)31;
@@ -316,8 +365,8 @@ int update_binned(cs_sketch* s, const BinPlan& pl, const float* xyz, uint64_t n,
         CS_CUDA(cudaMalloc(&s->bins, need * sizeof(uint16_t)));
         s->bins_records = need;
     }
-    for (uint64_t off = 0; off < n; off += BIN_CHUNK) {
-        uint64_t m = n - off < BIN_CHUNK ? n - off : BIN_CHUNK;
+    for (uint64_t off = 0; off < n; off += BC) {
+        uint64_t m = n - off < BC ? n - off : BC;
         for (int i = 0; i < s->n_scales; ++i)
             for (int j0 = 0; j0 < s->d; j0 += each) {
                 const int nr = j0 + each <= s->d ? each : s->d - j0;
@@ -547,7 +596,7 @@ int scan_device_raw(cs_sketch* s, const float* xyz, uint64_t n, double sample_p)
         }
         /* optimistic chunk: expect at most rate * chunk new entries per scale, keep a factor 2 of slack */
         double want = (double)free_min / (2.0 * (s->rate > 1e-9 ? s->rate : 1e-9));
-        uint64_t chunk = want >= (double)MAX_CHUNK ? MAX_CHUNK : (uint64_t)want;
+        uint64_t chunk = want >= (double)s->scan_chunk ? s->scan_chunk : (uint64_t)want;
         if (s->first_chunk && s->k_max) {                /* a small first chunk fixes a first tau cheaply */
             uint64_t c0 = 8 * s->k_max > (1u << 18) ? 8 * s->k_max : (1u << 18);
             if (chunk > c0) chunk = c0;
@@ -625,53 +674,114 @@ int scan_device_raw(cs_sketch* s, const float* xyz, uint64_t n, double sample_p)
 
 constexpr double COMPACT_BELOW_P = 0.5;               /* sample_p below which compaction pays */
 constexpr uint64_t COMPACT_MIN_N = 1ull << 20;
-constexpr uint64_t COMPACT_CHUNK = 1ull << 28;
 
-/* Kept particles of xyz[0..m) (running index index0) -> s->kept; *cnt = their number, or UINT64_MAX if they did not
- * fit (the caller then takes the sampling-in-kernel path for this chunk). */
-int compact_chunk(cs_sketch* s, const float* xyz, uint64_t m, uint64_t index0, double sample_p, uint64_t* cnt) {
-    const uint64_t want = (uint64_t)((double)(m < COMPACT_CHUNK ? m : COMPACT_CHUNK) * sample_p * 1.05) + 65536;
-    if (s->kept_cap < want) {
-        CS_CUDA(cudaStreamSynchronize(s->stream));
-        if (s->kept) cudaFree(s->kept);
-        s->kept = nullptr; s->kept_cap = 0;
-        CS_CUDA(cudaMalloc(&s->kept, want * 12));
-        s->kept_cap = want;
-    }
+/* Kept particles of xyz[0..m) (running index index0) -> dst (room for cap particles); *cnt = their number, or
+ * UINT64_MAX if they did not fit (the caller then takes another route for this chunk). */
+int compact_chunk(cs_sketch* s, const float* xyz, uint64_t m, uint64_t index0, double sample_p, float* dst, uint64_t cap,
+                  uint64_t* cnt) {
     CS_CUDA(cudaMemsetAsync(s->word_dev, 0, 4, s->stream));
-    cudaError_t e = launch_compact_kept(xyz, m, index0, s->K, sample_threshold(sample_p), s->kept, s->word_dev,
-                                        (uint32_t)(s->kept_cap < 0xFFFFFFFFull ? s->kept_cap : 0xFFFFFFFFull), s->sm_count,
-                                        s->stream);
+    cudaError_t e = launch_compact_kept(xyz, m, index0, s->K, sample_threshold(sample_p), dst, s->word_dev,
+                                        (uint32_t)(cap < 0xFFFFFFFFull ? cap : 0xFFFFFFFFull), s->sm_count, s->stream);
     if (e != cudaSuccess) return fail(CS_ERR_CUDA, "compaction kernel: %s", cudaGetErrorString(e));
     s->launches += 1;
     CS_CUDA(cudaMemcpyAsync(s->word_host, s->word_dev, 4, cudaMemcpyDeviceToHost, s->stream));
     CS_CUDA(cudaStreamSynchronize(s->stream));
-    *cnt = *s->word_host <= s->kept_cap ? *s->word_host : UINT64_MAX;
+    *cnt = *s->word_host <= cap ? *s->word_host : UINT64_MAX;
+    return CS_OK;
+}
+
+/* scratch buffer for the kept particles of one chunk (no replay cache, or the cache is full) */
+int ensure_kept(cs_sketch* s, uint64_t m, double sample_p) {
+    const uint64_t want = (uint64_t)((double)(m < s->compact_chunk ? m : s->compact_chunk) * sample_p * 1.05) + 65536;
+    if (s->kept_cap >= want) return CS_OK;
+    CS_CUDA(cudaStreamSynchronize(s->stream));
+    if (s->kept) cudaFree(s->kept);
+    s->kept = nullptr; s->kept_cap = 0;
+    CS_CUDA(cudaMalloc(&s->kept, want * 12));
+    s->kept_cap = want;
     return CS_OK;
 }
 
 bool wants_compaction_of_stream(uint64_t n, double sample_p) { return sample_p < COMPACT_BELOW_P && n >= COMPACT_MIN_N; }
 
+/* Replay cache, sampled streams: reserve room for the kept particles of an update call over (xyz, n, index0, p) in the
+ * arena.  Returns the index of the new segment, or -1 (cache off / no room: the caller uses the scratch buffer). */
+int kept_seg_begin(cs_sketch* s, const float* xyz, uint64_t n, uint64_t index0, double p) {
+    if (!s->replay_limit) return -1;
+    for (size_t i = 0; i < s->kept_segs.size(); ++i)       /* the same buffer again: its old copy is stale */
+        if (s->kept_segs[i].src == xyz && s->kept_segs[i].index0 == index0) s->kept_segs[i].n = 0;
+    const uint64_t want = (uint64_t)((double)n * p * 1.05) + 65536;
+    if (s->kept_arena_cap - s->kept_arena_used < want) {       /* grow (geometrically, within the budget), keeping what is held */
+        const uint64_t room = s->replay_limit > s->host_cache_bytes ? (s->replay_limit - s->host_cache_bytes) / 12 : 0;
+        uint64_t cap = 2 * s->kept_arena_cap > s->kept_arena_used + 2 * want ? 2 * s->kept_arena_cap : s->kept_arena_used + 2 * want;
+        if (cap > room) cap = room;
+        if (cap < s->kept_arena_used + want) return -1;
+        float* grown = nullptr;
+        if (cudaMalloc(&grown, cap * 12) != cudaSuccess) { cudaGetLastError(); return -1; }
+        if (s->kept_arena) {
+            if (cudaMemcpyAsync(grown, s->kept_arena, s->kept_arena_used * 12, cudaMemcpyDeviceToDevice, s->stream) != cudaSuccess ||
+                cudaStreamSynchronize(s->stream) != cudaSuccess) { cudaGetLastError(); cudaFree(grown); return -1; }
+            cudaFree(s->kept_arena);
+        }
+        s->kept_arena = grown;
+        s->kept_arena_cap = cap;
+    }
+    if (s->kept_segs.size() >= 4096) return -1;
+    cs_sketch::KeptSeg g = {xyz, n, index0, p, s->kept_arena_used, 0};
+    s->kept_segs.push_back(g);
+    return (int)s->kept_segs.size() - 1;
+}
+
+void kept_cache_clear(cs_sketch* s) { s->kept_segs.clear(); s->kept_arena_used = 0; }
+
 int update_passes(cs_sketch* s, const float* xyz, uint64_t n, uint64_t index0, double sample_p) {
     if (!wants_compaction_of_stream(n, sample_p)) return update_passes_raw(s, xyz, n, index0, sample_p);
-    for (uint64_t off = 0; off < n; off += COMPACT_CHUNK) {
-        const uint64_t m = n - off < COMPACT_CHUNK ? n - off : COMPACT_CHUNK;
-        uint64_t cnt = 0;
-        int rc = compact_chunk(s, xyz + 3 * off, m, index0 + off, sample_p, &cnt);
-        if (rc) return rc;
+    int seg = kept_seg_begin(s, xyz, n, index0, sample_p);
+    for (uint64_t off = 0; off < n; off += s->compact_chunk) {
+        const uint64_t m = n - off < s->compact_chunk ? n - off : s->compact_chunk;
+        uint64_t cnt = UINT64_MAX;
+        const float* kept = nullptr;
+        int rc = CS_OK;
+        if (seg >= 0) {
+            cs_sketch::KeptSeg& g = s->kept_segs[seg];
+            float* dst = s->kept_arena + 3 * (g.off + g.cnt);
+            rc = compact_chunk(s, xyz + 3 * off, m, index0 + off, sample_p, dst, s->kept_arena_cap - (g.off + g.cnt), &cnt);
+            if (rc) return rc;
+            if (cnt == UINT64_MAX) { s->kept_segs.pop_back(); seg = -1; }   /* does not fit after all: no cache entry */
+            else { kept = dst; g.cnt += cnt; }
+        }
+        if (seg < 0) {
+            rc = ensure_kept(s, m, sample_p);
+            if (rc) return rc;
+            rc = compact_chunk(s, xyz + 3 * off, m, index0 + off, sample_p, s->kept, s->kept_cap, &cnt);
+            if (rc) return rc;
+            kept = s->kept;
+        }
         if (cnt == UINT64_MAX) rc = update_passes_raw(s, xyz + 3 * off, m, index0 + off, sample_p);
-        else if (cnt)          rc = update_passes_raw(s, s->kept, cnt, 0, 1.0);
+        else if (cnt)          rc = update_passes_raw(s, kept, cnt, 0, 1.0);
         if (rc) return rc;
     }
+    if (seg >= 0) s->kept_arena_used = s->kept_segs[seg].off + s->kept_segs[seg].cnt;
     return CS_OK;
 }
 
 int scan_device(cs_sketch* s, const float* xyz, uint64_t n, double sample_p) {
     if (!wants_compaction_of_stream(n, sample_p)) return scan_device_raw(s, xyz, n, sample_p);
-    for (uint64_t off = 0; off < n; off += COMPACT_CHUNK) {
-        const uint64_t m = n - off < COMPACT_CHUNK ? n - off : COMPACT_CHUNK;
+    for (size_t i = 0; i < s->kept_segs.size(); ++i) {       /* replay of a buffer whose kept particles are still held */
+        const cs_sketch::KeptSeg& g = s->kept_segs[i];
+        if (g.src == xyz && g.n == n && g.index0 == s->scan_index && g.p == sample_p) {
+            const uint64_t next = s->scan_index + n;
+            int rc = g.cnt ? scan_device_raw(s, s->kept_arena + 3 * g.off, g.cnt, 1.0) : CS_OK;
+            s->scan_index = next;
+            return rc;
+        }
+    }
+    for (uint64_t off = 0; off < n; off += s->compact_chunk) {
+        const uint64_t m = n - off < s->compact_chunk ? n - off : s->compact_chunk;
         uint64_t cnt = 0;
-        int rc = compact_chunk(s, xyz + 3 * off, m, s->scan_index, sample_p, &cnt);
+        int rc = ensure_kept(s, m, sample_p);
+        if (rc) return rc;
+        rc = compact_chunk(s, xyz + 3 * off, m, s->scan_index, sample_p, s->kept, s->kept_cap, &cnt);
         if (rc) return rc;
         if (cnt == UINT64_MAX) {
             rc = scan_device_raw(s, xyz + 3 * off, m, sample_p);       /* advances scan_index by m itself */
@@ -722,24 +832,115 @@ int emit_prefix(cs_sketch* s, int i, uint32_t n, uint64_t* ids_out, int32_t* est
 }
 
 int ensure_staging(cs_sketch* s) {
-    if (s->stage[0]) return CS_OK;
-    CS_CUDA(cudaStreamCreateWithFlags(&s->copy_stream, cudaStreamNonBlocking));
-    for (int k = 0; k < STAGE_SLOTS; ++k) {
-        CS_CUDA(cudaMalloc(&s->stage[k], STAGE_PARTICLES * 12));
-        CS_CUDA(cudaEventCreateWithFlags(&s->ev_full[k], cudaEventDisableTiming));
-        CS_CUDA(cudaEventCreateWithFlags(&s->ev_free[k], cudaEventDisableTiming));
+    if (!s->copy_stream) {
+        CS_CUDA(cudaStreamCreateWithFlags(&s->copy_stream, cudaStreamNonBlocking));
+        for (int k = 0; k < STAGE_SLOTS; ++k) {
+            CS_CUDA(cudaEventCreateWithFlags(&s->ev_full[k], cudaEventDisableTiming));
+            CS_CUDA(cudaEventCreateWithFlags(&s->ev_free[k], cudaEventDisableTiming));
+        }
     }
     return CS_OK;
 }
 
-/* Issue the host->device copy of batch b into its ring slot (waits for the kernel that last used the slot). */
-int stage_batch(cs_sketch* s, const float* xyz_host, uint64_t n, uint64_t b) {
-    const int slot = (int)(b % STAGE_SLOTS);
-    const uint64_t off = b * STAGE_PARTICLES;
-    const uint64_t m = n - off < STAGE_PARTICLES ? n - off : STAGE_PARTICLES;
-    CS_CUDA(cudaStreamWaitEvent(s->copy_stream, s->ev_free[slot], 0));
-    CS_CUDA(cudaMemcpyAsync(s->stage[slot], xyz_host + 3 * off, m * 12, cudaMemcpyHostToDevice, s->copy_stream));
-    CS_CUDA(cudaEventRecord(s->ev_full[slot], s->copy_stream));
+void free_stage_slots(cs_sketch* s) {
+    for (int k = 0; k < STAGE_SLOTS; ++k) {
+        if (s->stage[k]) cudaFree(s->stage[k]);
+        s->stage[k] = nullptr;
+    }
+    s->stage_alloc = 0;
+}
+
+int ensure_stage_slots(cs_sketch* s) {
+    if (s->stage[0] && s->stage_alloc == s->stage_particles) return CS_OK;
+    CS_CUDA(cudaStreamSynchronize(s->stream));
+    free_stage_slots(s);
+    for (int k = 0; k < STAGE_SLOTS; ++k) CS_CUDA(cudaMalloc(&s->stage[k], s->stage_particles * 12));
+    s->stage_alloc = s->stage_particles;
+    return CS_OK;
+}
+
+void free_host_cache(cs_sketch* s) {
+    if (s->host_cache) cudaFree(s->host_cache);
+    s->host_cache = nullptr; s->host_cache_bytes = 0; s->hc_valid = false;
+}
+
+/* Host-streamed pass (SURVEY 8.a a8; PAPER.md:295-298 batch flow, :570 I/O overlapped with compute): n items of bpp
+ * bytes in host memory are cut into batches of stage_particles items; batch b is copied with cudaMemcpyAsync on the
+ * copy stream into ring slot b mod 3 (after the kernels that last read the slot, ev_free) while the kernels of batch
+ * b-1 run on the handle's stream; body(dev_ptr, items, first_item) enqueues the work of one batch.
+ * Replay cache: when the handle may hold the whole buffer (cs_set_replay_cache), an update call copies the batches
+ * into one device buffer instead of the ring (fill), and a following scan call of the same host buffer (replay) finds
+ * them there: the stream crosses PCIe once. */
+template <class Body>
+int stream_host(cs_sketch* s, const void* host, size_t bpp, uint64_t n, bool fill_allowed, bool replay_allowed, Body body) {
+    const uint64_t B = s->stage_particles;
+    const uint64_t batches = (n + B - 1) / B;
+    if (replay_allowed && s->hc_valid && s->hc_host == host && s->hc_n == n && s->hc_bpp == bpp) {
+        for (uint64_t b = 0; b < batches; ++b) {
+            const uint64_t off = b * B, m = n - off < B ? n - off : B;
+            int rc = body(s->host_cache + off * bpp, m, off);
+            if (rc) return rc;
+        }
+        return CS_OK;
+    }
+    int rc = ensure_staging(s);
+    if (rc) return rc;
+    bool fill = false;
+    if (fill_allowed) {
+        s->hc_valid = false;                               /* whatever was cached belongs to an older update call */
+        const uint64_t kept_bytes = s->kept_arena_cap * 12;
+        if (s->replay_limit >= kept_bytes && s->replay_limit - kept_bytes >= n * bpp) {
+            if (s->host_cache_bytes < n * bpp) {
+                CS_CUDA(cudaStreamSynchronize(s->stream));
+                free_host_cache(s);
+                if (cudaMalloc(&s->host_cache, n * bpp) == cudaSuccess) s->host_cache_bytes = n * bpp;
+                else { cudaGetLastError(); s->host_cache = nullptr; }
+            }
+            fill = s->host_cache != nullptr;
+        }
+    }
+    if (!fill) {
+        rc = ensure_stage_slots(s);
+        if (rc) return rc;
+    }
+    auto slot_ptr = [&](uint64_t b) -> unsigned char* {
+        return fill ? s->host_cache + b * B * bpp : reinterpret_cast<unsigned char*>(s->stage[b % STAGE_SLOTS]);
+    };
+    auto copy_in = [&](uint64_t b) -> int {
+        const int slot = (int)(b % STAGE_SLOTS);
+        const uint64_t off = b * B, m = n - off < B ? n - off : B;
+        if (!fill) CS_CUDA(cudaStreamWaitEvent(s->copy_stream, s->ev_free[slot], 0));
+        CS_CUDA(cudaMemcpyAsync(slot_ptr(b), static_cast<const unsigned char*>(host) + off * bpp, m * bpp,
+                                cudaMemcpyHostToDevice, s->copy_stream));
+        CS_CUDA(cudaEventRecord(s->ev_full[slot], s->copy_stream));
+        return CS_OK;
+    };
+    rc = copy_in(0);
+    if (rc) return rc;
+    for (uint64_t b = 0; b < batches; ++b) {
+        if (b + 1 < batches) {                               /* the next copy runs while this batch is processed */
+            rc = copy_in(b + 1);
+            if (rc) return rc;
+        }
+        const int slot = (int)(b % STAGE_SLOTS);
+        const uint64_t off = b * B, m = n - off < B ? n - off : B;
+        CS_CUDA(cudaStreamWaitEvent(s->stream, s->ev_full[slot], 0));
+        rc = body(slot_ptr(b), m, off);
+        if (rc) return rc;
+        CS_CUDA(cudaEventRecord(s->ev_free[slot], s->stream));
+    }
+    CS_CUDA(cudaStreamSynchronize(s->copy_stream));          /* the host buffer may be reused on return */
+    if (fill) { s->hc_host = host; s->hc_n = n; s->hc_bpp = bpp; s->hc_valid = true; }
+    return CS_OK;
+}
+
+int ensure_ids_scratch(cs_sketch* s, uint64_t ids) {
+    if (s->ids_scratch_cap >= ids) return CS_OK;
+    CS_CUDA(cudaStreamSynchronize(s->stream));
+    if (s->ids_scratch) cudaFree(s->ids_scratch);
+    s->ids_scratch = nullptr; s->ids_scratch_cap = 0;
+    CS_CUDA(cudaMalloc(&s->ids_scratch, ids * sizeof(uint64_t)));
+    s->ids_scratch_cap = ids;
     return CS_OK;
 }
 
@@ -772,9 +973,16 @@ int check_records(const cs_sketch* s, const uint64_t* recs, uint64_t n, double s
     return CS_OK;
 }
 
-/* m <= STAGE_PARTICLES device records -> s->unpacked -> the ordinary update / scan passes */
+/* m <= stage_particles device records -> s->unpacked -> the ordinary update / scan passes */
 int records_batch(cs_sketch* s, const uint64_t* recs_dev, uint64_t m, uint64_t index0, double sample_p, bool scan) {
-    if (!s->unpacked) CS_CUDA(cudaMalloc(&s->unpacked, STAGE_PARTICLES * 12));
+    if (s->unpacked_alloc < m) {
+        CS_CUDA(cudaStreamSynchronize(s->stream));
+        if (s->unpacked) cudaFree(s->unpacked);
+        s->unpacked = nullptr; s->unpacked_alloc = 0;
+        const uint64_t want = m > s->stage_particles ? m : s->stage_particles;
+        CS_CUDA(cudaMalloc(&s->unpacked, want * 12));
+        s->unpacked_alloc = want;
+    }
     const uint32_t gf = finest_nested_mesh(s);
     cudaError_t e = launch_unpack_centres(recs_dev, m, gf, (float)(s->L / (double)gf), s->unpacked, s->stream);
     if (e != cudaSuccess) return fail(CS_ERR_CUDA, "unpack kernel: %s", cudaGetErrorString(e));
@@ -783,8 +991,9 @@ int records_batch(cs_sketch* s, const uint64_t* recs_dev, uint64_t m, uint64_t i
 }
 
 int records_device(cs_sketch* s, const uint64_t* recs_dev, uint64_t n, double sample_p, bool scan) {
-    for (uint64_t off = 0; off < n; off += STAGE_PARTICLES) {
-        const uint64_t m = n - off < STAGE_PARTICLES ? n - off : STAGE_PARTICLES;
+    const uint64_t B = s->stage_particles;
+    for (uint64_t off = 0; off < n; off += B) {
+        const uint64_t m = n - off < B ? n - off : B;
         int rc = records_batch(s, recs_dev + off, m, s->upd_index + off, sample_p, scan);
         if (rc) return rc;
     }
@@ -794,34 +1003,10 @@ int records_device(cs_sketch* s, const uint64_t* recs_dev, uint64_t n, double sa
 
 /* records in host memory: 8 B per particle over PCIe through the same ring of staging slots */
 int records_host(cs_sketch* s, const uint64_t* recs_host, uint64_t n, double sample_p, bool scan) {
-    int rc = ensure_staging(s);
+    int rc = stream_host(s, recs_host, 8, n, !scan, scan, [&](const void* dev, uint64_t m, uint64_t off) -> int {
+        return records_batch(s, static_cast<const uint64_t*>(dev), m, s->upd_index + off, sample_p, scan);
+    });
     if (rc) return rc;
-    const uint64_t batches = (n + STAGE_PARTICLES - 1) / STAGE_PARTICLES;
-    auto stage = [&](uint64_t b) -> int {
-        const int slot = (int)(b % STAGE_SLOTS);
-        const uint64_t off = b * STAGE_PARTICLES;
-        const uint64_t m = n - off < STAGE_PARTICLES ? n - off : STAGE_PARTICLES;
-        CS_CUDA(cudaStreamWaitEvent(s->copy_stream, s->ev_free[slot], 0));
-        CS_CUDA(cudaMemcpyAsync(s->stage[slot], recs_host + off, m * 8, cudaMemcpyHostToDevice, s->copy_stream));
-        CS_CUDA(cudaEventRecord(s->ev_full[slot], s->copy_stream));
-        return CS_OK;
-    };
-    rc = stage(0);
-    if (rc) return rc;
-    for (uint64_t b = 0; b < batches; ++b) {
-        if (b + 1 < batches) {
-            rc = stage(b + 1);
-            if (rc) return rc;
-        }
-        const int slot = (int)(b % STAGE_SLOTS);
-        const uint64_t off = b * STAGE_PARTICLES;
-        const uint64_t m = n - off < STAGE_PARTICLES ? n - off : STAGE_PARTICLES;
-        CS_CUDA(cudaStreamWaitEvent(s->stream, s->ev_full[slot], 0));
-        rc = records_batch(s, reinterpret_cast<const uint64_t*>(s->stage[slot]), m, s->upd_index + off, sample_p, scan);
-        if (rc) return rc;
-        CS_CUDA(cudaEventRecord(s->ev_free[slot], s->stream));
-    }
-    CS_CUDA(cudaStreamSynchronize(s->copy_stream));
     if (!scan) s->upd_index += n;
     return CS_OK;
 }
@@ -853,9 +1038,9 @@ int cs_hash_cell(uint64_t a, uint64_t b, uint64_t c, int big, uint64_t* r_out, u
         return fail(CS_ERR_ARG, "cs_hash_cell: c out of range for this form");
     const HashCoef k = split_coef(a, b);
     if (big == 2) {
-        const uint64_t tb = affine_mod_p<true>(k, 0u, cell_c1(c));      /* the table entry the kernels look up */
-        *low32_out = affine_low32_tb(k, cell_c0(c), tb + 1);
-        *r_out = (affine_partial_tb(k, cell_c0(c), tb) + 0) % P61;      /* s mod p, for the comparison only */
+        const uint64_t tb = affine_mod_p<true>(k, 0u, cell_c1(c));      /* the table entry: (A*c1 + b) mod p */
+        *low32_out = affine_low32_tb(k, cell_c0(c), tb);
+        *r_out = affine_mod_p_tb(k, cell_c0(c), tb);
     } else if (big) {
         *r_out = affine_mod_p<true>(k, cell_c0(c), cell_c1(c));
         *low32_out = affine_low32<true>(k, cell_c0(c), cell_c1(c));
@@ -932,6 +1117,7 @@ int cs_create(cs_sketch** out, int d, uint64_t w, uint32_t G, double L, uint64_t
 
 int cs_destroy(cs_sketch* s) {
     if (!s) return CS_OK;
+    DeviceGuard guard_(s);
     if (s->stream || s->T[0]) cudaStreamSynchronize(s->stream);
     if (s->copy_stream) cudaStreamSynchronize(s->copy_stream);
     free_candidates(s);
@@ -955,36 +1141,73 @@ int cs_destroy(cs_sketch* s) {
         if (s->ev_free[k]) cudaEventDestroy(s->ev_free[k]);
     }
     if (s->copy_stream) cudaStreamDestroy(s->copy_stream);
+    if (s->host_cache) cudaFree(s->host_cache);
+    if (s->kept_arena) cudaFree(s->kept_arena);
+    if (s->ht_keys) cudaFree(s->ht_keys);
+    if (s->ht_vals) cudaFree(s->ht_vals);
+    if (s->ids_scratch) cudaFree(s->ids_scratch);
     delete s;
     return CS_OK;
 }
 
 int cs_reset(cs_sketch* s) {
-    if (!s) return fail(CS_ERR_ARG, "null handle");
+    CS_ENTER(s);
     for (int i = 0; i < s->n_scales; ++i)
         CS_CUDA(cudaMemsetAsync(s->T[i], 0, (size_t)s->d * s->w * sizeof(int32_t), s->stream));
     s->upd_index = 0; s->scan_index = 0; s->scanning = false;
+    kept_cache_clear(s);
     for (int i = 0; i < CS_MAX_SCALES; ++i) { s->dirty[i] = false; s->last_compact[i] = 0; }
     memset(s->st_host, 0, sizeof(ScanState) * CS_MAX_SCALES);
     return CS_OK;
 }
 
 int cs_set_stream(cs_sketch* s, void* cuda_stream) {
-    if (!s) return fail(CS_ERR_ARG, "null handle");
+    CS_ENTER(s);
     CS_CUDA(cudaStreamSynchronize(s->stream));           /* work already queued finishes on the old stream */
     s->stream = (cudaStream_t)cuda_stream;
     return CS_OK;
 }
 
 int cs_set_table_budget(cs_sketch* s, uint64_t bytes) {
-    if (!s) return fail(CS_ERR_ARG, "null handle");
+    CS_ENTER(s);
     if (bytes < 4) return fail(CS_ERR_ARG, "budget must be at least one counter");
     s->table_budget = bytes;
     return CS_OK;
 }
 
+int cs_set_chunk_sizes(cs_sketch* s, uint64_t stage_particles, uint64_t update_chunk, uint64_t scan_chunk,
+                       uint64_t compact_chunk) {
+    CS_ENTER(s);
+    const uint64_t v[4] = {stage_particles, update_chunk, scan_chunk, compact_chunk};
+    for (int i = 0; i < 4; ++i)
+        if (v[i] && (v[i] < 64 || v[i] > (1ull << 30) || (v[i] & 3u)))
+            return fail(CS_ERR_ARG, "chunk sizes must be multiples of 4 in [64, 2^30] (0 = keep)");
+    if (stage_particles && stage_particles != s->stage_particles) {
+        CS_CUDA(cudaStreamSynchronize(s->stream));
+        if (s->copy_stream) CS_CUDA(cudaStreamSynchronize(s->copy_stream));
+        free_stage_slots(s);
+        s->stage_particles = stage_particles;
+    }
+    if (update_chunk) s->bin_chunk = update_chunk;
+    if (scan_chunk) s->scan_chunk = scan_chunk;
+    if (compact_chunk) s->compact_chunk = compact_chunk;
+    return CS_OK;
+}
+
+int cs_set_replay_cache(cs_sketch* s, uint64_t bytes) {
+    CS_ENTER(s);
+    CS_CUDA(cudaStreamSynchronize(s->stream));
+    if (s->copy_stream) CS_CUDA(cudaStreamSynchronize(s->copy_stream));
+    free_host_cache(s);
+    if (s->kept_arena) cudaFree(s->kept_arena);
+    s->kept_arena = nullptr; s->kept_arena_cap = 0;
+    kept_cache_clear(s);
+    s->replay_limit = bytes;
+    return CS_OK;
+}
+
 int cs_set_update_mode(cs_sketch* s, int mode, int rows_direct) {
-    if (!s) return fail(CS_ERR_ARG, "null handle");
+    CS_ENTER(s);
     if (mode < 0 || mode > 2 || rows_direct < -1 || rows_direct > CS_MAX_ROWS)
         return fail(CS_ERR_ARG, "mode must be 0 (auto), 1 (direct) or 2 (binned); rows_direct in [-1, 32]");
     s->update_mode = mode;
@@ -993,7 +1216,7 @@ int cs_set_update_mode(cs_sketch* s, int mode, int rows_direct) {
 }
 
 int cs_set_counting_mode(cs_sketch* s, int mode) {
-    if (!s) return fail(CS_ERR_ARG, "null handle");
+    CS_ENTER(s);
     if (mode < 0 || mode > 1) return fail(CS_ERR_ARG, "mode must be 0 (Count Sketch) or 1 (Count-Min)");
     if (s->upd_index != 0 || s->scanning) return fail(CS_ERR_STATE, "the counting mode can only change on an empty sketch");
     for (int i = 0; i < s->n_scales; ++i)
@@ -1012,20 +1235,20 @@ int cs_set_counting_mode(cs_sketch* s, int mode) {
 }
 
 int cs_set_scan_mode(cs_sketch* s, int mode) {
-    if (!s) return fail(CS_ERR_ARG, "null handle");
+    CS_ENTER(s);
     if (mode < 0 || mode > 3) return fail(CS_ERR_ARG, "mode must be 0 (auto), 1 (plain), 2 (bitmap) or 3 (bitmap stages)");
     s->scan_mode = mode;
     return CS_OK;
 }
 
 int cs_set_update_index(cs_sketch* s, uint64_t index) {
-    if (!s) return fail(CS_ERR_ARG, "null handle");
+    CS_ENTER(s);
     s->upd_index = index;
     return CS_OK;
 }
 
 int cs_set_scan_index(cs_sketch* s, uint64_t index) {
-    if (!s) return fail(CS_ERR_ARG, "null handle");
+    CS_ENTER(s);
     s->scan_index = index;
     return CS_OK;
 }
@@ -1040,6 +1263,7 @@ int cs_update(cs_sketch* s, const float* xyz_dev, uint64_t n, double sample_p) {
     int rc = check_xyz(s, xyz_dev, n, sample_p);
     if (rc) return rc;
     if (!n) return CS_OK;
+    DeviceGuard guard_(s);
     rc = update_passes(s, xyz_dev, n, s->upd_index, sample_p);
     if (rc) return rc;
     s->upd_index += n;
@@ -1050,27 +1274,17 @@ int cs_update_host(cs_sketch* s, const float* xyz_host, uint64_t n, double sampl
     int rc = check_xyz(s, xyz_host, n, sample_p);
     if (rc) return rc;
     if (!n) return CS_OK;
-    rc = ensure_staging(s);
+    DeviceGuard guard_(s);
+    rc = stream_host(s, xyz_host, 12, n, true, false, [&](const void* dev, uint64_t m, uint64_t off) -> int {
+        return update_passes(s, static_cast<const float*>(dev), m, s->upd_index + off, sample_p);
+    });
     if (rc) return rc;
-    const uint64_t batches = (n + STAGE_PARTICLES - 1) / STAGE_PARTICLES;
-    for (uint64_t b = 0; b < batches; ++b) {
-        rc = stage_batch(s, xyz_host, n, b);
-        if (rc) return rc;
-        const int slot = (int)(b % STAGE_SLOTS);
-        const uint64_t off = b * STAGE_PARTICLES;
-        const uint64_t m = n - off < STAGE_PARTICLES ? n - off : STAGE_PARTICLES;
-        CS_CUDA(cudaStreamWaitEvent(s->stream, s->ev_full[slot], 0));
-        rc = update_passes(s, s->stage[slot], m, s->upd_index + off, sample_p);
-        if (rc) return rc;
-        CS_CUDA(cudaEventRecord(s->ev_free[slot], s->stream));
-    }
-    CS_CUDA(cudaStreamSynchronize(s->copy_stream));      /* the host buffer may be reused on return */
     s->upd_index += n;
     return CS_OK;
 }
 
 int cs_pack_records(cs_sketch* s, const float* xyz_dev, uint64_t n, uint64_t* recs_dev) {
-    if (!s) return fail(CS_ERR_ARG, "null handle");
+    CS_ENTER(s);
     if (n && (!xyz_dev || !recs_dev)) return fail(CS_ERR_ARG, "null buffer with n > 0");
     if ((reinterpret_cast<uintptr_t>(xyz_dev) & 3u) || (reinterpret_cast<uintptr_t>(recs_dev) & 7u))
         return fail(CS_ERR_ARG, "positions must be 4-byte aligned, records 8-byte aligned");
@@ -1083,12 +1297,14 @@ int cs_pack_records(cs_sketch* s, const float* xyz_dev, uint64_t n, uint64_t* re
 int cs_update_records(cs_sketch* s, const uint64_t* recs_dev, uint64_t n, double sample_p) {
     int rc = check_records(s, recs_dev, n, sample_p);
     if (rc || !n) return rc;
+    DeviceGuard guard_(s);
     return records_device(s, recs_dev, n, sample_p, false);
 }
 
 int cs_update_records_host(cs_sketch* s, const uint64_t* recs_host, uint64_t n, double sample_p) {
     int rc = check_records(s, recs_host, n, sample_p);
     if (rc || !n) return rc;
+    DeviceGuard guard_(s);
     return records_host(s, recs_host, n, sample_p, false);
 }
 
@@ -1097,6 +1313,7 @@ int cs_scan_records(cs_sketch* s, const uint64_t* recs_dev, uint64_t n, double s
     if (rc) return rc;
     if (!s->scanning) return fail(CS_ERR_STATE, "cs_scan_records before cs_scan_begin");
     if (!n) return CS_OK;
+    DeviceGuard guard_(s);
     return records_device(s, recs_dev, n, sample_p, true);
 }
 
@@ -1105,11 +1322,12 @@ int cs_scan_records_host(cs_sketch* s, const uint64_t* recs_host, uint64_t n, do
     if (rc) return rc;
     if (!s->scanning) return fail(CS_ERR_STATE, "cs_scan_records_host before cs_scan_begin");
     if (!n) return CS_OK;
+    DeviceGuard guard_(s);
     return records_host(s, recs_host, n, sample_p, true);
 }
 
 int cs_estimate(cs_sketch* s, int scale, const uint64_t* cells_dev, uint64_t m, int32_t* est_dev) {
-    if (!s) return fail(CS_ERR_ARG, "null handle");
+    CS_ENTER(s);
     if (scale < 0 || scale >= s->n_scales) return fail(CS_ERR_ARG, "scale out of range");
     if (m && (!cells_dev || !est_dev)) return fail(CS_ERR_ARG, "null buffer with m > 0");
     if (!m) return CS_OK;
@@ -1121,14 +1339,14 @@ int cs_estimate(cs_sketch* s, int scale, const uint64_t* cells_dev, uint64_t m, 
 }
 
 int cs_scan_begin(cs_sketch* s, uint64_t k_max, int32_t thr_min) {
-    if (!s) return fail(CS_ERR_ARG, "null handle");
-    if (k_max > (1ull << 28)) return fail(CS_ERR_ARG, "k_max must be <= 2^28");
-    uint64_t want = 16 * k_max;
+    CS_ENTER(s);
+    if (k_max > (1ull << 26)) return fail(CS_ERR_ARG, "k_max must be <= 2^26");
+    uint64_t want = 16 * k_max;                          /* <= 2^30, the limit of the list (grow_candidates) */
     if (want < s->cap_min) want = s->cap_min;
-    uint32_t cap = s->cap_min;
+    uint64_t cap = s->cap_min;
     while (cap < want) cap *= 2;
     if (s->cap != cap) {
-        int rc = alloc_candidates(s, cap);
+        int rc = alloc_candidates(s, (uint32_t)cap);
         if (rc) return rc;
     }
     s->k_max = k_max; s->thr_min = thr_min;
@@ -1149,7 +1367,7 @@ int cs_scan_begin(cs_sketch* s, uint64_t k_max, int32_t thr_min) {
 }
 
 int cs_set_candidate_capacity(cs_sketch* s, uint64_t entries) {
-    if (!s) return fail(CS_ERR_ARG, "null handle");
+    CS_ENTER(s);
     if (entries < 1024 || entries > (1ull << 30) || (entries & (entries - 1)))
         return fail(CS_ERR_ARG, "capacity must be a power of two in [2^10, 2^30]");
     s->cap_min = (uint32_t)entries;
@@ -1161,6 +1379,7 @@ int cs_scan(cs_sketch* s, const float* xyz_dev, uint64_t n, double sample_p) {
     if (rc) return rc;
     if (!s->scanning) return fail(CS_ERR_STATE, "cs_scan before cs_scan_begin");
     if (!n) return CS_OK;
+    DeviceGuard guard_(s);
     return scan_device(s, xyz_dev, n, sample_p);
 }
 
@@ -1169,30 +1388,14 @@ int cs_scan_host(cs_sketch* s, const float* xyz_host, uint64_t n, double sample_
     if (rc) return rc;
     if (!s->scanning) return fail(CS_ERR_STATE, "cs_scan_host before cs_scan_begin");
     if (!n) return CS_OK;
-    rc = ensure_staging(s);
-    if (rc) return rc;
-    const uint64_t batches = (n + STAGE_PARTICLES - 1) / STAGE_PARTICLES;
-    rc = stage_batch(s, xyz_host, n, 0);
-    if (rc) return rc;
-    for (uint64_t b = 0; b < batches; ++b) {
-        if (b + 1 < batches) {                           /* next copy runs while this batch is scanned */
-            rc = stage_batch(s, xyz_host, n, b + 1);
-            if (rc) return rc;
-        }
-        const int slot = (int)(b % STAGE_SLOTS);
-        const uint64_t off = b * STAGE_PARTICLES;
-        const uint64_t m = n - off < STAGE_PARTICLES ? n - off : STAGE_PARTICLES;
-        CS_CUDA(cudaStreamWaitEvent(s->stream, s->ev_full[slot], 0));
-        rc = scan_device(s, s->stage[slot], m, sample_p);
-        if (rc) return rc;
-        CS_CUDA(cudaEventRecord(s->ev_free[slot], s->stream));
-    }
-    CS_CUDA(cudaStreamSynchronize(s->copy_stream));
-    return CS_OK;
+    DeviceGuard guard_(s);
+    return stream_host(s, xyz_host, 12, n, false, true, [&](const void* dev, uint64_t m, uint64_t) -> int {
+        return scan_device(s, static_cast<const float*>(dev), m, sample_p);
+    });
 }
 
 int cs_scan_cells(cs_sketch* s, int scale, const uint64_t* cells_dev, uint64_t m) {
-    if (!s) return fail(CS_ERR_ARG, "null handle");
+    CS_ENTER(s);
     if (scale < 0 || scale >= s->n_scales) return fail(CS_ERR_ARG, "scale out of range");
     if (m && !cells_dev) return fail(CS_ERR_ARG, "null cells with m > 0");
     if (!s->scanning) return fail(CS_ERR_STATE, "cs_scan_cells before cs_scan_begin");
@@ -1226,7 +1429,7 @@ int cs_scan_cells(cs_sketch* s, int scale, const uint64_t* cells_dev, uint64_t m
 }
 
 int cs_scan_children(cs_sketch* s, int parent_scale, int child_scale, const uint64_t* parent_ids_dev, uint64_t m) {
-    if (!s) return fail(CS_ERR_ARG, "null handle");
+    CS_ENTER(s);
     if (parent_scale < 0 || parent_scale >= s->n_scales || child_scale < 0 || child_scale >= s->n_scales)
         return fail(CS_ERR_ARG, "scale out of range");
     if (m && !parent_ids_dev) return fail(CS_ERR_ARG, "null parents with m > 0");
@@ -1236,23 +1439,20 @@ int cs_scan_children(cs_sketch* s, int parent_scale, int child_scale, const uint
     const uint32_t r = Gc / Gp;
     const uint64_t r3 = (uint64_t)r * r * r;
     const uint64_t per = (1ull << 21) / r3 ? (1ull << 21) / r3 : 1;      /* parents per expansion: <= 2^21 ids (16 MiB) */
-    uint64_t* ids = nullptr;
-    CS_CUDA(cudaMalloc(&ids, per * r3 * sizeof(uint64_t)));
-    int rc = CS_OK;
+    int rc = ensure_ids_scratch(s, per * r3);
+    if (rc) return rc;
     for (uint64_t off = 0; off < m && rc == CS_OK; off += per) {
         const uint64_t mm = m - off < per ? m - off : per;
-        cudaError_t e = launch_expand_children(parent_ids_dev + off, mm, Gp, Gc, r, ids, s->stream);
+        cudaError_t e = launch_expand_children(parent_ids_dev + off, mm, Gp, Gc, r, s->ids_scratch, s->stream);
         if (e != cudaSuccess) { rc = fail(CS_ERR_CUDA, "expand kernel: %s", cudaGetErrorString(e)); break; }
         s->launches += 1;
-        rc = cs_scan_cells(s, child_scale, ids, mm * r3);
+        rc = cs_scan_cells(s, child_scale, s->ids_scratch, mm * r3);
     }
-    cudaStreamSynchronize(s->stream);
-    cudaFree(ids);
     return rc;
 }
 
 int cs_scan_all(cs_sketch* s, int scale) {
-    if (!s) return fail(CS_ERR_ARG, "null handle");
+    CS_ENTER(s);
     if (scale < 0 || scale >= s->n_scales) return fail(CS_ERR_ARG, "scale out of range");
     if (!s->scanning) return fail(CS_ERR_STATE, "cs_scan_all before cs_scan_begin");
     const uint64_t m = (uint64_t)s->G[scale] * s->G[scale] * s->G[scale];
@@ -1307,6 +1507,7 @@ int cs_scan_all(cs_sketch* s, int scale) {
 
 int cs_topk(cs_sketch* s, int scale, uint64_t k, uint64_t* ids_out, int32_t* est_out, uint64_t* n_out) {
     if (!s || !n_out) return fail(CS_ERR_ARG, "null argument");
+    DeviceGuard guard_(s);
     if (scale < 0 || scale >= s->n_scales) return fail(CS_ERR_ARG, "scale out of range");
     if (k && (!ids_out || !est_out)) return fail(CS_ERR_ARG, "null output with k > 0");
     if (!s->scanning) return fail(CS_ERR_STATE, "cs_topk before cs_scan_begin");
@@ -1324,6 +1525,7 @@ int cs_topk(cs_sketch* s, int scale, uint64_t k, uint64_t* ids_out, int32_t* est
 int cs_excursion(cs_sketch* s, int scale, int32_t thr, uint64_t cap, uint64_t* ids_out, int32_t* est_out,
                  uint64_t* n_total) {
     if (!s || !n_total) return fail(CS_ERR_ARG, "null argument");
+    DeviceGuard guard_(s);
     if (scale < 0 || scale >= s->n_scales) return fail(CS_ERR_ARG, "scale out of range");
     if (cap && (!ids_out || !est_out)) return fail(CS_ERR_ARG, "null output with cap > 0");
     if (!s->scanning) return fail(CS_ERR_STATE, "cs_excursion before cs_scan_begin");
@@ -1346,7 +1548,7 @@ int cs_excursion(cs_sketch* s, int scale, int32_t thr, uint64_t cap, uint64_t* i
 
 int cs_recount(cs_sketch* s, int scale, const uint64_t* ids_dev, uint64_t m, const float* xyz_dev, uint64_t n,
                uint32_t* counts_dev, float* xyz_out_dev, uint64_t cap, uint64_t* n_out) {
-    if (!s) return fail(CS_ERR_ARG, "null handle");
+    CS_ENTER(s);
     if (scale < 0 || scale >= s->n_scales) return fail(CS_ERR_ARG, "scale out of range");
     if (m > (1ull << 28)) return fail(CS_ERR_ARG, "at most 2^28 cells");
     if ((m && (!ids_dev || !counts_dev)) || (n && !xyz_dev)) return fail(CS_ERR_ARG, "null buffer with a non-zero size");
@@ -1356,29 +1558,48 @@ int cs_recount(cs_sketch* s, int scale, const uint64_t* ids_dev, uint64_t m, con
     if (!m || !n) return CS_OK;
     uint64_t size = 1024;
     while (size < 4 * m) size *= 2;                                   /* load factor <= 1/4 */
-    uint64_t* keys = nullptr;
-    uint32_t* vals = nullptr;
-    CS_CUDA(cudaMalloc(&keys, size * sizeof(uint64_t)));
-    cudaError_t e = cudaMalloc(&vals, size * sizeof(uint32_t));
-    if (e == cudaSuccess) e = cudaMemsetAsync(keys, 0xFF, size * sizeof(uint64_t), s->stream);
-    if (e == cudaSuccess) e = cudaMemsetAsync(vals, 0xFF, size * sizeof(uint32_t), s->stream);
-    if (e == cudaSuccess) e = cudaMemsetAsync(s->word_dev, 0, 4, s->stream);
-    if (e == cudaSuccess) e = launch_ht_build(ids_dev, (uint32_t)m, keys, vals, (uint32_t)(size - 1), s->stream);
+    if (s->ht_size < size) {
+        CS_CUDA(cudaStreamSynchronize(s->stream));
+        if (s->ht_keys) cudaFree(s->ht_keys);
+        if (s->ht_vals) cudaFree(s->ht_vals);
+        s->ht_keys = nullptr; s->ht_vals = nullptr; s->ht_size = 0;
+        CS_CUDA(cudaMalloc(&s->ht_keys, size * sizeof(uint64_t)));
+        CS_CUDA(cudaMalloc(&s->ht_vals, size * sizeof(uint32_t)));
+        s->ht_size = size;
+    }
+    CS_CUDA(cudaMemsetAsync(s->ht_keys, 0xFF, size * sizeof(uint64_t), s->stream));
+    CS_CUDA(cudaMemsetAsync(s->ht_vals, 0xFF, size * sizeof(uint32_t), s->stream));
+    CS_CUDA(cudaMemsetAsync(s->word_dev, 0, 4, s->stream));
+    cudaError_t e = launch_ht_build(ids_dev, (uint32_t)m, s->ht_keys, s->ht_vals, (uint32_t)(size - 1), s->stream);
     if (e == cudaSuccess)
-        e = launch_recount(s->P.sc[scale], xyz_dev, n, keys, vals, (uint32_t)(size - 1), counts_dev, xyz_out_dev, s->word_dev,
-                           cap, s->sm_count, s->stream);
-    if (e == cudaSuccess) e = cudaMemcpyAsync(s->word_host, s->word_dev, 4, cudaMemcpyDeviceToHost, s->stream);
-    if (e == cudaSuccess) e = cudaStreamSynchronize(s->stream);
-    cudaFree(keys);
-    if (vals) cudaFree(vals);
-    if (e != cudaSuccess) return fail(e == cudaErrorMemoryAllocation ? CS_ERR_NOMEM : CS_ERR_CUDA, "cs_recount: %s", cudaGetErrorString(e));
+        e = launch_recount(s->P.sc[scale], xyz_dev, n, s->ht_keys, s->ht_vals, (uint32_t)(size - 1), counts_dev, xyz_out_dev,
+                           s->word_dev, cap, s->sm_count, s->stream);
+    if (e != cudaSuccess) return fail(CS_ERR_CUDA, "cs_recount: %s", cudaGetErrorString(e));
     s->launches += 2;
+    CS_CUDA(cudaMemcpyAsync(s->word_host, s->word_dev, 4, cudaMemcpyDeviceToHost, s->stream));
+    CS_CUDA(cudaStreamSynchronize(s->stream));
     if (n_out) *n_out = *s->word_host;
+    return CS_OK;
+}
+
+/* 26-neighbour shell (Fig. 14: the heavy cells "and their surroundings"): ids_out[27*i + t], t =
+ * (dx+1) + 3*(dy+1) + 9*(dz+1), = the cell at offset (dx, dy, dz) from ids_dev[i] on the mesh of `scale`, wrapped
+ * periodically (the box is periodic, BASELINE.json configs); t = 13 is the cell itself. */
+int cs_expand_neighbours(cs_sketch* s, int scale, const uint64_t* ids_dev, uint64_t m, uint64_t* ids_out_dev) {
+    CS_ENTER(s);
+    if (scale < 0 || scale >= s->n_scales) return fail(CS_ERR_ARG, "scale out of range");
+    if (m && (!ids_dev || !ids_out_dev)) return fail(CS_ERR_ARG, "null buffer with m > 0");
+    if (m > (1ull << 32)) return fail(CS_ERR_ARG, "at most 2^32 cells");
+    if (!m) return CS_OK;
+    cudaError_t e = launch_expand_neighbours(ids_dev, m, s->G[scale], ids_out_dev, s->stream);
+    if (e != cudaSuccess) return fail(CS_ERR_CUDA, "neighbour kernel: %s", cudaGetErrorString(e));
+    s->launches += 1;
     return CS_OK;
 }
 
 int cs_scan_stats(cs_sketch* s, int scale, uint64_t* out4_host) {
     if (!s || !out4_host) return fail(CS_ERR_ARG, "null argument");
+    DeviceGuard guard_(s);
     if (scale < 0 || scale >= s->n_scales) return fail(CS_ERR_ARG, "scale out of range");
     if (!s->scanning) return fail(CS_ERR_STATE, "cs_scan_stats before cs_scan_begin");
     int rc = read_states(s);
@@ -1392,6 +1613,7 @@ int cs_scan_stats(cs_sketch* s, int scale, uint64_t* out4_host) {
 
 int cs_sketch_read(cs_sketch* s, int scale, int32_t* out_d_by_w) {
     if (!s || !out_d_by_w) return fail(CS_ERR_ARG, "null argument");
+    DeviceGuard guard_(s);
     if (scale < 0 || scale >= s->n_scales) return fail(CS_ERR_ARG, "scale out of range");
     CS_CUDA(cudaMemcpyAsync(out_d_by_w, s->T[scale], (size_t)s->d * s->w * sizeof(int32_t), cudaMemcpyDefault, s->stream));
     CS_CUDA(cudaStreamSynchronize(s->stream));
@@ -1400,6 +1622,7 @@ int cs_sketch_read(cs_sketch* s, int scale, int32_t* out_d_by_w) {
 
 int cs_sketch_add(cs_sketch* s, int scale, const int32_t* in_d_by_w) {
     if (!s || !in_d_by_w) return fail(CS_ERR_ARG, "null argument");
+    DeviceGuard guard_(s);
     if (scale < 0 || scale >= s->n_scales) return fail(CS_ERR_ARG, "scale out of range");
     const uint64_t n = (uint64_t)s->d * s->w;
     cudaPointerAttributes at;
@@ -1433,6 +1656,7 @@ int cs_coeffs(cs_sketch* s, int scale, uint64_t* out_4d_host, uint64_t* K_out_ho
 
 int cs_launch_count(cs_sketch* s, uint64_t* n_out) {
     if (!s || !n_out) return fail(CS_ERR_ARG, "null argument");
+    DeviceGuard guard_(s);
     *n_out = s->launches;
     return CS_OK;
 }

@@ -115,6 +115,7 @@ cudaError_t launch_scan_range(const PassParams& P, const ScanParams& S, int scal
                               cudaStream_t st);
 cudaError_t launch_expand_children(const uint64_t* parents, uint64_t m, uint32_t Gp, uint32_t Gc, uint32_t r, uint64_t* out,
                                    cudaStream_t st);
+cudaError_t launch_expand_neighbours(const uint64_t* ids, uint64_t m, uint32_t G, uint64_t* out, cudaStream_t st);
 cudaError_t launch_estimate(const PassParams& P, int scale, const uint64_t* cells, uint64_t m, int32_t* est,
                             cudaStream_t st);
 cudaError_t launch_table_add(int32_t* T, const int32_t* in, uint64_t n, cudaStream_t st);

@@ -24,8 +24,7 @@ k_ht_build(const uint64_t* __restrict__ ids, uint32_t m, unsigned long long* __r
     uint32_t s = ht_slot(c, mask);
     for (;;) {
         const unsigned long long old = atomicCAS(&keys[s], (unsigned long long)HT_EMPTY, (unsigned long long)c);
-        if (old == HT_EMPTY) { vals[s] = i; return; }
-        if (old == c) { atomicMin(&vals[s], i); return; }             // duplicate id: the first occurrence counts
+        if (old == HT_EMPTY || old == c) { atomicMin(&vals[s], i); return; }   // vals start at ~0u; duplicate id: the first occurrence counts
         s = (s + 1) & mask;
     }
 }

@@ -159,6 +159,29 @@ cudaError_t launch_expand_children(const uint64_t* parents, uint64_t m, uint32_t
     return cudaGetLastError();
 }
 
+/* 26-neighbour shell of mesh cells, periodic (Fig. 14: the particles of the heavy cells "and their
+ * surroundings" go to the offline halo finder): out[27*i + t], t = (dx+1) + 3*(dy+1) + 9*(dz+1). */
+__global__ void __launch_bounds__(256)
+k_expand_neighbours(const uint64_t* __restrict__ ids, uint64_t m, uint32_t G, uint64_t* __restrict__ out) {
+    const uint64_t total = m * 27;
+    const uint64_t stride = (uint64_t)gridDim.x * blockDim.x;
+    for (uint64_t i = (uint64_t)blockIdx.x * blockDim.x + threadIdx.x; i < total; i += stride) {
+        const uint64_t c = ids[i / 27];
+        const uint32_t t = (uint32_t)(i % 27);
+        const uint32_t x = (uint32_t)(c % G), y = (uint32_t)((c / G) % G), z = (uint32_t)(c / ((uint64_t)G * G));
+        const uint32_t nx = (x + G + t % 3 - 1) % G, ny = (y + G + (t / 3) % 3 - 1) % G, nz = (z + G + t / 9 - 1) % G;
+        out[i] = (uint64_t)nx + (uint64_t)G * ((uint64_t)ny + (uint64_t)G * nz);
+    }
+}
+
+cudaError_t launch_expand_neighbours(const uint64_t* ids, uint64_t m, uint32_t G, uint64_t* out, cudaStream_t st) {
+    if (!m) return cudaSuccess;
+    uint64_t blocks = (m * 27 + 255) / 256;
+    if (blocks > 148 * 8) blocks = 148 * 8;
+    k_expand_neighbours<<<(int)blocks, 256, 0, st>>>(ids, m, G, out);
+    return cudaGetLastError();
+}
+
 /* ---- dispatch on (d, w power of two) ------------------------------------------------------------------ */
 
 template <bool POW2>

@@ -50,9 +50,9 @@ k_build_bitmap(const int32_t* __restrict__ T, uint64_t n, int32_t tau, uint32_t*
 }
 
 /* true iff at most (d-1)/2 rows of cell c are clear in the bitmap of scale s */
-template <int D, int HM>
+template <int D, bool BIG>
 __device__ __forceinline__ bool bitmap_survives(const PassParams& P, int s, const uint32_t* __restrict__ bm, uint32_t c0,
-                                                uint32_t c1, uint32_t tb_addr) {
+                                                uint32_t c1) {
     const int d = D ? D : P.d;
     const int max_fail = P.rank;
     const uint32_t wmask = (uint32_t)(P.w - 1);
@@ -63,7 +63,7 @@ __device__ __forceinline__ bool bitmap_survives(const PassParams& P, int s, cons
         uint32_t wd[FIRST], h[FIRST];
 #pragma unroll
         for (int j = 0; j < FIRST; ++j) {
-            h[j] = bucket_of<HM>(rows[j], c0, c1, tb_addr + j * 8, wmask);
+            h[j] = bucket_of<BIG>(rows[j], c0, c1, wmask);
             wd[j] = ld_bits(bm + (((uint64_t)j * P.w + h[j]) >> 5));
         }
 #pragma unroll
@@ -71,14 +71,14 @@ __device__ __forceinline__ bool bitmap_survives(const PassParams& P, int s, cons
 #pragma unroll
         for (int j = FIRST; j < D; ++j) {
             if (fails <= max_fail) {
-                const uint32_t hj = bucket_of<HM>(rows[j], c0, c1, tb_addr + j * 8, wmask);
+                const uint32_t hj = bucket_of<BIG>(rows[j], c0, c1, wmask);
                 const uint32_t w = ld_bits(bm + (((uint64_t)j * P.w + hj) >> 5));
                 fails += 1 - (int)((w >> (hj & 31u)) & 1u);
             }
         }
     } else {
         for (int j = 0; j < d && fails <= max_fail; ++j) {
-            const uint32_t hj = bucket_of<HM>(rows[j], c0, c1, tb_addr + j * 8, wmask);
+            const uint32_t hj = bucket_of<BIG>(rows[j], c0, c1, wmask);
             const uint32_t w = ld_bits(bm + (((uint64_t)j * P.w + hj) >> 5));
             fails += 1 - (int)((w >> (hj & 31u)) & 1u);
         }
@@ -88,14 +88,11 @@ __device__ __forceinline__ bool bitmap_survives(const PassParams& P, int s, cons
 
 struct BitmapParams {
     const uint32_t* bm[CS_MAX_SCALES];
-    uint8_t hm[CS_MAX_SCALES];          // hash mode per scale
 };
 
 template <int D>
 __device__ __forceinline__ void scan_particle_bm(const PassParams& P, const ScanParams& S, const BitmapParams& Bm,
-                                                 const int32_t* tau, uint32_t tb_base, bool keep, float x, float y,
-                                                 float z) {
-    const int d = D ? D : P.d;
+                                                 const int32_t* tau, bool keep, float x, float y, float z) {
     for (int s = 0; s < P.n_scales; ++s) {
         uint64_t c = 0;
         int32_t est = 0;
@@ -103,11 +100,8 @@ __device__ __forceinline__ void scan_particle_bm(const PassParams& P, const Scan
         if (keep) {
             c = cell_of(x, y, z, P.sc[s]);
             const uint32_t c0 = cell_c0(c), c1 = cell_c1(c);
-            const uint32_t tb_addr = tb_base + (uint32_t)((s * HASH_TB + c1) * d) * 8u;     // tb[s][c1][j]
-            bool live;
-            if (Bm.hm[s] == 0)      live = bitmap_survives<D, 0>(P, s, Bm.bm[s], c0, c1, tb_addr);
-            else if (Bm.hm[s] == 1) live = bitmap_survives<D, 1>(P, s, Bm.bm[s], c0, c1, tb_addr);
-            else                    live = bitmap_survives<D, 2>(P, s, Bm.bm[s], c0, c1, tb_addr);
+            const bool live = P.sc[s].big ? bitmap_survives<D, true>(P, s, Bm.bm[s], c0, c1)
+                                          : bitmap_survives<D, false>(P, s, Bm.bm[s], c0, c1);
             if (live) {                                  // rare: exact estimate from the counters
                 emit = P.sc[s].big ? estimate_ge<D, true, true>(P, s, c, tau[s], est)
                                    : estimate_ge<D, true, false>(P, s, c, tau[s], est);
@@ -122,14 +116,6 @@ __global__ void __launch_bounds__(PASS_THREADS)
 k_scan_bitmap(const __grid_constant__ PassParams P, const __grid_constant__ ScanParams S,
               const __grid_constant__ BitmapParams Bm, const float* __restrict__ xyz, uint64_t n, uint32_t head,
               uint64_t groups) {
-    extern __shared__ __align__(16) uint64_t tb[];       // tb[s][c1][j] = 1 + (A_j*c1 + b_j) mod p (bucket hashes)
-    const int d = D ? D : P.d;
-    for (uint32_t i = threadIdx.x; i < (uint32_t)(P.n_scales * HASH_TB * d); i += PASS_THREADS) {
-        const uint32_t j = i % d, c1 = (i / d) % HASH_TB, s = i / (d * HASH_TB);
-        tb[i] = Bm.hm[s] == 1 ? affine_mod_p<true>(P.rows[s * d + j].h, 0u, c1) + 1 : 0;
-    }
-    __syncthreads();
-    const uint32_t tb_base = (uint32_t)__cvta_generic_to_shared(tb);
     int32_t tau[CS_MAX_SCALES];
 #pragma unroll
     for (int s = 0; s < CS_MAX_SCALES; ++s) tau[s] = s < P.n_scales ? S.tg[s].st->tau : 0;
@@ -154,10 +140,10 @@ k_scan_bitmap(const __grid_constant__ PassParams P, const __grid_constant__ Scan
             k2 = keep_particle(P.K, i0 + 2, P.Tp);
             k3 = keep_particle(P.K, i0 + 3, P.Tp);
         }
-        scan_particle_bm<D>(P, S, Bm, tau, tb_base, k0, q0.x, q0.y, q0.z);
-        scan_particle_bm<D>(P, S, Bm, tau, tb_base, k1, q0.w, q1.x, q1.y);
-        scan_particle_bm<D>(P, S, Bm, tau, tb_base, k2, q1.z, q1.w, q2.x);
-        scan_particle_bm<D>(P, S, Bm, tau, tb_base, k3, q2.y, q2.z, q2.w);
+        scan_particle_bm<D>(P, S, Bm, tau, k0, q0.x, q0.y, q0.z);
+        scan_particle_bm<D>(P, S, Bm, tau, k1, q0.w, q1.x, q1.y);
+        scan_particle_bm<D>(P, S, Bm, tau, k2, q1.z, q1.w, q2.x);
+        scan_particle_bm<D>(P, S, Bm, tau, k3, q2.y, q2.z, q2.w);
     }
     if (blockIdx.x == 0 && threadIdx.x < 32) {        // warp 0: the <= 6 edge particles
         const uint64_t tail0 = (uint64_t)head + 4 * groups;
@@ -171,7 +157,7 @@ k_scan_bitmap(const __grid_constant__ PassParams P, const __grid_constant__ Scan
             const float* p = xyz + 3 * i;
             x = ld_stream4(p); y = ld_stream4(p + 1); z = ld_stream4(p + 2);
         }
-        scan_particle_bm<D>(P, S, Bm, tau, tb_base, keep, x, y, z);
+        scan_particle_bm<D>(P, S, Bm, tau, keep, x, y, z);
     }
 }
 
@@ -190,20 +176,13 @@ cudaError_t launch_build_bitmap(const int32_t* T, uint64_t n_counters, int32_t t
 cudaError_t launch_scan_bitmap(const PassParams& P, const ScanParams& S, const uint32_t* const* bm, const float* xyz,
                                uint64_t n, int sm_count, cudaStream_t st) {
     BitmapParams Bm = {};
-    for (int s = 0; s < P.n_scales; ++s) {
-        Bm.bm[s] = bm[s];
-        const uint64_t cells = (uint64_t)P.sc[s].G * P.sc[s].G * P.sc[s].G;
-        Bm.hm[s] = !P.sc[s].big ? 0 : (((cells - 1) >> 31) < HASH_TB ? 1 : 2);
-    }
+    for (int s = 0; s < P.n_scales; ++s) Bm.bm[s] = bm[s];
     uint32_t head;
     uint64_t groups;
     split_aligned(xyz, n, &head, &groups);
-    const size_t smem = (size_t)P.n_scales * HASH_TB * P.d * sizeof(uint64_t);
-    cudaError_t e = cudaSuccess;
+    const size_t smem = 0;
 #define CS_CALL(DD)                                                                                               \
     {                                                                                                             \
-        e = cudaFuncSetAttribute(k_scan_bitmap<DD>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);       \
-        if (e != cudaSuccess) return e;                                                                           \
         int per_sm = 0;                                                                                           \
         cudaOccupancyMaxActiveBlocksPerMultiprocessor(&per_sm, k_scan_bitmap<DD>, PASS_THREADS, smem);            \
         if (per_sm < 1) per_sm = 1;                                                                               \

@@ -102,23 +102,16 @@ __device__ __forceinline__ uint32_t ld_bits(const uint32_t* p) {
     asm volatile("ld.global.relaxed.gpu.u32 %0, [%1];" : "=r"(v) : "l"(p));
     return v;
 }
-__device__ __forceinline__ uint64_t lds_u64s(uint32_t addr) {
-    uint64_t v;
-    asm volatile("ld.shared.u64 %0, [%1];" : "=l"(v) : "r"(addr));
-    return v;
-}
-
 __device__ __forceinline__ uint32_t lds_u32s(uint32_t addr) {
     uint32_t v;
     asm volatile("ld.shared.u32 %0, [%1];" : "=r"(v) : "r"(addr));
     return v;
 }
 
-/* bucket hash of row rc under hash mode HM (0: c < 2^31; 1: table in shared memory; 2: general two-limb form) */
-template <int HM>
-__device__ __forceinline__ uint32_t bucket_of(const RowCoef& rc, uint32_t c0, uint32_t c1, uint32_t tb_addr, uint32_t wmask) {
-    if (HM == 1) return affine_low32_tb(rc.h, c0, lds_u64s(tb_addr)) & wmask;
-    return affine_low32<HM == 2>(rc.h, c0, c1) & wmask;
+/* bucket hash of row rc (w a power of two); BIG: cell ids of this mesh can exceed 2^31 */
+template <bool BIG>
+__device__ __forceinline__ uint32_t bucket_of(const RowCoef& rc, uint32_t c0, uint32_t c1, uint32_t wmask) {
+    return affine_low32<BIG>(rc.h, c0, c1) & wmask;
 }
 
 #define CS_DISPATCH_D(CALL)                                    \

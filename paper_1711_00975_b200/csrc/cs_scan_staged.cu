@@ -187,19 +187,17 @@ struct CoarseParams {
     const uint32_t* coarse;    // rows 0 .. FIRST-1, row_words words each
     uint32_t g;                // log2 counters per coarse bit
     uint32_t row_words;        // (w >> g) / 32
-    uint32_t hm;               // hash mode (0 one limb, 1 table, 2 general)
+    uint32_t big;              // cell ids of the mesh can exceed 2^31
     uint32_t nseg;             // segments = grid size of the following stages
 };
 
-template <int FIRST, int HM>
-__device__ __forceinline__ void cb_hashes(const PassParams& P, uint32_t tb_base, uint32_t wmask, const uint64_t* c,
-                                          uint32_t (&h)[2][FIRST]) {
+template <int FIRST, bool BIG>
+__device__ __forceinline__ void cb_hashes(const PassParams& P, uint32_t wmask, const uint64_t* c, uint32_t (&h)[2][FIRST]) {
 #pragma unroll
     for (int q = 0; q < 2; ++q) {
         const uint32_t c0 = cell_c0(c[q]), c1 = cell_c1(c[q]);
-        const uint32_t tb_addr = tb_base + c1 * (uint32_t)(P.d * 8);                  // tb[c1][j], j < d
 #pragma unroll
-        for (int j = 0; j < FIRST; ++j) h[q][j] = bucket_of<HM>(P.rows[j], c0, c1, tb_addr + j * 8, wmask);
+        for (int j = 0; j < FIRST; ++j) h[q][j] = bucket_of<BIG>(P.rows[j], c0, c1, wmask);
     }
 }
 
@@ -216,12 +214,8 @@ k_stage_first_cb(const __grid_constant__ PassParams P, const __grid_constant__ S
         uint4* dst = reinterpret_cast<uint4*>(cb_smem);
         for (uint32_t i = threadIdx.x; i < cwords / 4; i += CB_THREADS) dst[i] = src[i];
     }
-    uint64_t* tb = reinterpret_cast<uint64_t*>(cb_smem + cwords);
-    for (uint32_t i = threadIdx.x; i < (uint32_t)(HASH_TB * P.d); i += CB_THREADS)
-        tb[i] = C.hm == 1 ? affine_mod_p<true>(P.rows[i % P.d].h, 0u, i / P.d) + 1 : 0;
     __syncthreads();
     const uint32_t cs_addr = (uint32_t)__cvta_generic_to_shared(cb_smem);
-    const uint32_t tb_base = (uint32_t)__cvta_generic_to_shared(tb);
     const uint32_t wmask = (uint32_t)(P.w - 1);
     const float4* body = reinterpret_cast<const float4*>(xyz + 3 * (uint64_t)head);
     const uint32_t lane = threadIdx.x & 31u;
@@ -259,9 +253,8 @@ k_stage_first_cb(const __grid_constant__ PassParams P, const __grid_constant__ S
 #pragma unroll
             for (int half = 0; half < 2; ++half) {
                 uint32_t h[2][FIRST];
-                if (C.hm == 0)      cb_hashes<FIRST, 0>(P, tb_base, wmask, c + 2 * half, h);
-                else if (C.hm == 1) cb_hashes<FIRST, 1>(P, tb_base, wmask, c + 2 * half, h);
-                else                cb_hashes<FIRST, 2>(P, tb_base, wmask, c + 2 * half, h);
+                if (C.big) cb_hashes<FIRST, true>(P, wmask, c + 2 * half, h);
+                else       cb_hashes<FIRST, false>(P, wmask, c + 2 * half, h);
                 uint32_t wd[2][FIRST];
 #pragma unroll
                 for (int q = 0; q < 2; ++q)
@@ -464,9 +457,8 @@ cudaError_t launch_scan_staged_cb(const PassParams& P, const ScanTarget& tg, con
     Q.seg_cap = seg_cap; Q.row0 = 0; Q.d_all = P.d; Q.pad = 0;
     CoarseParams C;
     C.fine = fine; C.coarse = coarse; C.g = g; C.row_words = row_words; C.nseg = (uint32_t)blocks;
-    const uint64_t cells = (uint64_t)P.sc[0].G * P.sc[0].G * P.sc[0].G;
-    C.hm = !P.sc[0].big ? 0 : (((cells - 1) >> 31) < HASH_TB ? 1 : 2);
-    const size_t smem = (size_t)first * row_words * 4 + (size_t)HASH_TB * P.d * sizeof(uint64_t);
+    C.big = P.sc[0].big;
+    const size_t smem = (size_t)first * row_words * 4;
     cudaError_t e = cudaSuccess;
 #define CS_CB(F)                                                                                              \
     case F:                                                                                                   \

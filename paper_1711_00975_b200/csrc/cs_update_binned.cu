@@ -48,12 +48,11 @@ __device__ __forceinline__ void st_stream16u(uint4* p, const uint4& v) {
 }
 
 /* Shared-memory layout of k_bin_scatter (dynamic):
- *   cnt[NB] | qlen | pad | queue[NB] (u16) | buf[NB*C] (u16) | 64 B pad | tb[64][2R] (u64, hash tables, HM == 1)
+ *   cnt[NB] | qlen | pad | queue[NB] (u16) | buf[NB*C] (u16) | 64 B pad
  * All accesses of the hot loop use 32-bit shared-space addresses (no generic-to-shared conversion per access). */
 __host__ __device__ inline size_t smem_off_queue(uint32_t nb) { return (((size_t)nb + 2) * 4 + 15) & ~(size_t)15; }
 __host__ __device__ inline size_t smem_off_buf(uint32_t nb) { return (smem_off_queue(nb) + (size_t)nb * 2 + 15) & ~(size_t)15; }
-__host__ __device__ inline size_t smem_off_tb(uint32_t nb, uint32_t C) { return smem_off_buf(nb) + (size_t)nb * C * 2 + 64; }
-size_t scatter_smem_bytes(uint32_t nb, uint32_t C) { return smem_off_tb(nb, C) + (size_t)HASH_TB * 2 * 8 * 8; }
+size_t scatter_smem_bytes(uint32_t nb, uint32_t C) { return smem_off_buf(nb) + (size_t)nb * C * 2 + 64; }
 
 __device__ __forceinline__ uint32_t atoms_inc(uint32_t addr) {
     uint32_t old;
@@ -62,11 +61,6 @@ __device__ __forceinline__ uint32_t atoms_inc(uint32_t addr) {
 }
 __device__ __forceinline__ void sts_u16(uint32_t addr, uint32_t v) {
     asm volatile("st.shared.u16 [%0], %1;" :: "r"(addr), "h"((unsigned short)v) : "memory");
-}
-__device__ __forceinline__ uint64_t lds_u64(uint32_t addr) {
-    uint64_t v;
-    asm volatile("ld.shared.u64 %0, [%1];" : "=l"(v) : "r"(addr));
-    return v;
 }
 
 /* Apply one record directly (fallback path and the partial buffers at the end of the kernel). */
@@ -78,31 +72,20 @@ __device__ __forceinline__ void apply_direct(int32_t* T, uint32_t bin, uint32_t 
 struct InsertCtx {
     uint32_t cnt_addr;     // shared address of cnt[0]
     uint32_t buf_addr;     // shared address of buf[0]
-    uint32_t tb_addr;      // shared address of tb[0][0]
     uint32_t C, C2;        // staging capacity in records / bytes
     uint32_t log2S, smask; // slice shift, (1 << log2S) - 1
     uint32_t log2w, wmask;
     int32_t rows_direct;
 };
 
-/* Hash mode HM: 0 = cell ids < 2^31 (one limb), 1 = high limb < 64 through the shared-memory table
- * (cs_hash.h affine_partial_tb), 2 = general two-limb form. */
-template <int HM>
-__device__ __forceinline__ void row_hashes(const RowCoef& rc, uint32_t c0, uint32_t c1, uint32_t tb_row_addr,
-                                           uint32_t& h, uint32_t& sb) {
-    if (HM == 1) {
-        uint64_t th, ts;                                  // both table entries of the row with one 16-byte load
-        asm volatile("ld.shared.v2.u64 {%0, %1}, [%2];" : "=l"(th), "=l"(ts) : "r"(tb_row_addr));
-        h = affine_low32_tb(rc.h, c0, th);
-        sb = affine_low32_tb(rc.s, c0, ts) & 1u;
-    } else {
-        h = affine_low32<HM == 2>(rc.h, c0, c1);
-        sb = affine_low32<HM == 2>(rc.s, c0, c1) & 1u;
-    }
+/* BIG: cell ids of the mesh can exceed 2^31 (two-limb form of cs_hash.h). */
+template <bool BIG>
+__device__ __forceinline__ void row_hashes(const RowCoef& rc, uint32_t c0, uint32_t c1, uint32_t& h, uint32_t& sb) {
+    h = affine_low32<BIG>(rc.h, c0, c1);
+    sb = affine_low32<BIG>(rc.s, c0, c1) & 1u;
 }
 
 /* Rare path: rows of one particle whose staging buffer was full are applied with red.global. */
-template <int HM>
 __device__ __noinline__ void apply_rows_direct(const PassParams& P, uint32_t wmask, uint32_t c0, uint32_t c1, uint32_t ovf) {
     while (ovf) {
         const int j = __ffs(ovf) - 1;
@@ -113,17 +96,16 @@ __device__ __noinline__ void apply_rows_direct(const PassParams& P, uint32_t wma
     }
 }
 
-template <int R, int HM>
+template <int R, bool BIG>
 __device__ __forceinline__ void bin_particle(const PassParams& P, const InsertCtx& X, float x, float y, float z) {
     const uint64_t c = cell_of(x, y, z, P.sc[0]);
     const uint32_t c0 = cell_c0(c), c1 = cell_c1(c);
-    const uint32_t tb_addr = X.tb_addr + c1 * (uint32_t)(R * 16);
     int32_t* T = P.sc[0].T;
     uint32_t ovf = 0;
 #pragma unroll
     for (int j = 0; j < R; ++j) {
         uint32_t h, sb;
-        row_hashes<HM>(P.rows[j], c0, c1, tb_addr + j * 16, h, sb);
+        row_hashes<BIG>(P.rows[j], c0, c1, h, sb);
         if (j < X.rows_direct) {
             red_add(T + (((uint32_t)j << X.log2w) | (h & X.wmask)), 1 - 2 * (int32_t)sb);
             continue;
@@ -135,13 +117,13 @@ __device__ __forceinline__ void bin_particle(const PassParams& P, const InsertCt
         if (slot < X.C) sts_u16(X.buf_addr + bin * X.C2 + slot * 2u, ((key & X.smask) << 1) + sb);
         else            ovf |= 1u << j;                                 // staging buffer full
     }
-    if (ovf) apply_rows_direct<HM>(P, X.wmask, c0, c1, ovf);
+    if (ovf) apply_rows_direct(P, X.wmask, c0, c1, ovf);
 }
 
 /* Particles [head, head + 2*pairs) are read as pairs (3 x 8 B per thread, 8-byte aligned); the <= 1 particle
  * before and the <= 1 after are applied directly by block 0.
  * One round = every thread bins one pair; then the bins holding >= 32 records are queued and flushed. */
-template <int R, int HM>
+template <int R, bool BIG>
 __global__ void __launch_bounds__(BIN_THREADS, 1)
 k_bin_scatter(const __grid_constant__ PassParams P, const __grid_constant__ BinParams B,
               const float* __restrict__ xyz, uint64_t n, uint32_t head, uint64_t pairs) {
@@ -151,22 +133,12 @@ k_bin_scatter(const __grid_constant__ PassParams P, const __grid_constant__ BinP
     uint32_t* qlen = cnt + B.nb;
     uint16_t* queue = reinterpret_cast<uint16_t*>(smem_raw + smem_off_queue(B.nb));
     uint16_t* buf = reinterpret_cast<uint16_t*>(smem_raw + smem_off_buf(B.nb));
-    uint64_t* tb = reinterpret_cast<uint64_t*>(smem_raw + smem_off_tb(B.nb, B.C));
     for (uint32_t i = threadIdx.x; i < B.nb + 1; i += NT) cnt[i] = 0;          // cnt and qlen
-    if (HM == 1) {
-        /* tb[c1][2j + {0,1}] = 1 + (A*c1 + b) mod p = 1 + (a*(c1*2^31) + b) mod p for the bucket / sign hash of row j */
-        for (uint32_t i = threadIdx.x; i < HASH_TB * 2 * R; i += NT) {
-            const uint32_t c1 = i / (2 * R), hs = i % (2 * R);
-            const RowCoef& rc = P.rows[hs >> 1];
-            tb[i] = affine_mod_p<true>((hs & 1) ? rc.s : rc.h, 0u, c1) + 1;          // tb + 1, see affine_low32_tb
-        }
-    }
     __syncthreads();
 
     InsertCtx X;
     X.cnt_addr = (uint32_t)__cvta_generic_to_shared(cnt);
     X.buf_addr = (uint32_t)__cvta_generic_to_shared(buf);
-    X.tb_addr = (uint32_t)__cvta_generic_to_shared(tb);
     X.C = B.C; X.C2 = B.C * 2u;
     X.log2S = B.log2S; X.smask = (1u << B.log2S) - 1u;
     X.log2w = B.log2w; X.wmask = (uint32_t)(P.w - 1);
@@ -190,8 +162,8 @@ k_bin_scatter(const __grid_constant__ PassParams P, const __grid_constant__ BinP
                 const float2 q1 = ld_stream8(body + 3 * g + 1);
                 const float2 q2 = ld_stream8(body + 3 * g + 2);
                 const uint64_t i0 = P.index0 + head + 2 * g;
-                if (!P.sample || keep_particle(P.K, i0, P.Tp)) bin_particle<R, HM>(P, X, q0.x, q0.y, q1.x);
-                if (!P.sample || keep_particle(P.K, i0 + 1, P.Tp)) bin_particle<R, HM>(P, X, q1.y, q2.x, q2.y);
+                if (!P.sample || keep_particle(P.K, i0, P.Tp)) bin_particle<R, BIG>(P, X, q0.x, q0.y, q1.x);
+                if (!P.sample || keep_particle(P.K, i0 + 1, P.Tp)) bin_particle<R, BIG>(P, X, q1.y, q2.x, q2.y);
             }
         }
         __syncthreads();
@@ -260,7 +232,7 @@ k_bin_scatter(const __grid_constant__ PassParams P, const __grid_constant__ BinP
         if (i != ~0ull && (!P.sample || keep_particle(P.K, P.index0 + i, P.Tp))) {
             const float* p = xyz + 3 * i;
             const uint64_t c = cell_of(ld_stream4(p), ld_stream4(p + 1), ld_stream4(p + 2), P.sc[0]);
-            apply_rows_direct<HM>(P, X.wmask, cell_c0(c), cell_c1(c), (1u << R) - 1u);
+            apply_rows_direct(P, X.wmask, cell_c0(c), cell_c1(c), (1u << R) - 1u);
         }
     }
 }
@@ -305,16 +277,14 @@ static cudaError_t launch_scatter_r(const PassParams& P, const BinParams& B, con
     const uint64_t pairs = (n - head) / 2;
     const size_t smem = scatter_smem_bytes(B.nb, B.C);
     cudaError_t e;
-    const uint64_t cells = (uint64_t)P.sc[0].G * P.sc[0].G * P.sc[0].G;
-    const int hm = !P.sc[0].big ? 0 : (((cells - 1) >> 31) < HASH_TB ? 1 : 2);
-#define CS_SCATTER(HM)                                                                                          \
-    e = cudaFuncSetAttribute(k_bin_scatter<R, HM>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);     \
+#define CS_SCATTER(BIG)                                                                                         \
+    e = cudaFuncSetAttribute(k_bin_scatter<R, BIG>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);    \
     if (e != cudaSuccess) return e;                                                                             \
     { int per_sm = 0;                                                                                         \
-      cudaOccupancyMaxActiveBlocksPerMultiprocessor(&per_sm, k_bin_scatter<R, HM>, (int)B.threads, smem);       \
+      cudaOccupancyMaxActiveBlocksPerMultiprocessor(&per_sm, k_bin_scatter<R, BIG>, (int)B.threads, smem);      \
       if (per_sm < 1) per_sm = 1;                                                                               \
-      k_bin_scatter<R, HM><<<sm_count * per_sm, B.threads, smem, st>>>(P, B, xyz, n, head, pairs); }
-    if (hm == 0) { CS_SCATTER(0) } else if (hm == 1) { CS_SCATTER(1) } else { CS_SCATTER(2) }
+      k_bin_scatter<R, BIG><<<sm_count * per_sm, B.threads, smem, st>>>(P, B, xyz, n, head, pairs); }
+    if (P.sc[0].big) { CS_SCATTER(true) } else { CS_SCATTER(false) }
 #undef CS_SCATTER
     return cudaGetLastError();
 }

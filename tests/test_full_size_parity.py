@@ -1,0 +1,160 @@
+"""Full-size parity against the oracle (SURVEY section 4 tier T3, 8.d.4), in the launch configuration bench.py times:
+cfg 3 and cfg 5 at N = 2^30 device-resident (automatic update / scan modes, 8 binned chunks, ~12 scan chunks) and three
+2^28-particle batches of cfg 4 through the host-streamed calls with the default 2^24-particle staging ring (48 batches:
+every slot is reused 16 times).  The oracle side is tests/sharded_oracle.py: the plain oracle over P disjoint index
+ranges, tables summed, lists merged by its own rule (valid by PAPER.md:578; pinned in tests/test_oracle_pins.py).
+
+Compared elementwise: the whole int32 table of every scale, 10^5 estimates (occupied + random cells), the full top-k ids
+and values, and (cfg 5) the excursion sets at every threshold.
+
+Opt-in: minutes of host time and ~40 GB of host memory.  CS_FULL_PARITY=1 python -m pytest tests/test_full_size_parity.py -m gpu
+(CS_FULL_PARITY_THREADS overrides the number of oracle threads, default = all cores).  Each test appends a line to
+gpurun_out/full_parity.log when it passes.
+"""
+import os
+import time
+
+import numpy as np
+import pytest
+import torch
+
+from oracle import cs_oracle as ora
+from sharded_oracle import ShardedOracle, _merge
+
+pytestmark = [pytest.mark.gpu, pytest.mark.slow,
+              pytest.mark.skipif(os.environ.get("CS_FULL_PARITY") != "1", reason="full-size parity is opt-in: CS_FULL_PARITY=1")]
+
+THREADS = int(os.environ.get("CS_FULL_PARITY_THREADS", "0")) or (os.cpu_count() or 8)
+
+
+@pytest.fixture(scope="module")
+def cs():
+    if not torch.cuda.is_available():
+        pytest.skip("no CUDA device")
+    from paper_1711_00975_b200 import build, binding
+    build.build_libcs()
+    binding.lib()
+    return binding
+
+
+def _ids(t):
+    return t.cpu().numpy().view(np.uint64)
+
+
+def _log(line):
+    os.makedirs("gpurun_out", exist_ok=True)
+    with open("gpurun_out/full_parity.log", "a") as f:
+        f.write(line + "\n")
+    print(line)
+
+
+def _first_diff(a, b):
+    a, b = np.asarray(a).ravel(), np.asarray(b).ravel()
+    if a.shape != b.shape:
+        return f"shapes {a.shape} vs {b.shape}"
+    i = np.flatnonzero(a != b)
+    return "equal" if len(i) == 0 else f"{len(i)} differences, first at flat index {int(i[0])}: {a[i[0]]} vs {b[i[0]]}"
+
+
+def _estimates_agree(g, so, wl, host_np, rng, m=100_000):
+    for s, G in enumerate(wl.G):
+        take = rng.integers(0, host_np.shape[0], size=m // 2)
+        take.sort()
+        occ = ora.quantise(host_np[take], G, wl.L)
+        cells = np.concatenate([occ, rng.integers(0, G ** 3, size=m // 2, dtype=np.uint64)])
+        ge = g.estimate(torch.from_numpy(cells.view(np.int64)).cuda(), s).cpu().numpy()
+        oe = so.estimate(cells, s)
+        assert np.array_equal(ge, oe), f"estimates differ at scale {s}: {_first_diff(ge, oe)}"
+
+
+def _device_resident(cs, name):
+    from paper_1711_00975_b200 import synth
+    wl = synth.CONFIGS[name]
+    t0 = time.perf_counter()
+    xyz = synth.generate(wl, device="cuda")
+    host_np = xyz.cpu().numpy()
+    p, k = wl.sample_p, wl.k
+    thr_min = min(wl.thresholds) if wl.thresholds else ora.INT32_MAX
+    t_gen = time.perf_counter() - t0
+
+    g = cs.CountSketch(wl.d, wl.w, list(wl.G), wl.L, wl.seed)
+    g.update(xyz, p)                                       # automatic modes, default chunking: what bench.py times
+    g.scan_begin(k, thr_min)
+    g.scan(xyz, p)
+    stats = g.scan_stats(0)
+
+    t0 = time.perf_counter()
+    so = ShardedOracle(wl.d, wl.w, wl.G, wl.L, wl.seed, THREADS)
+    so.update(host_np, p, 0)
+    t_upd = time.perf_counter() - t0
+    for s in range(len(wl.G)):
+        gt = g.sketch(s).cpu().numpy()
+        assert np.array_equal(gt, so.sketch(s)), f"table differs at scale {s}: {_first_diff(gt, so.sketch(s))}"
+    _estimates_agree(g, so, wl, host_np, np.random.default_rng(11))
+    t0 = time.perf_counter()
+    sel = so.select(host_np, k, thr_min, p, 0)
+    t_sel = time.perf_counter() - t0
+    n_exc = []
+    for s in range(len(wl.G)):
+        (ti, te), (xi, xe) = sel[s]
+        gi, gv = g.topk(k, s)
+        assert len(ti) == k
+        assert np.array_equal(_ids(gi), ti), f"top-k ids differ at scale {s}: {_first_diff(_ids(gi), ti)}"
+        assert np.array_equal(gv.cpu().numpy(), te), f"top-k values differ at scale {s}: {_first_diff(gv.cpu().numpy(), te)}"
+        for thr in wl.thresholds:
+            yi, ye, yt = g.excursion(thr, s)
+            keep = xe >= thr
+            assert yt == int(keep.sum()), f"excursion size differs at scale {s}, thr {thr}: {yt} vs {int(keep.sum())}"
+            assert np.array_equal(_ids(yi), xi[keep]) and np.array_equal(ye.cpu().numpy(), xe[keep]), (s, thr)
+            n_exc.append(yt)
+    _log(f"PASS {name}: N={wl.N} d={wl.d} w={wl.w} G={list(wl.G)} p={p} k={k} thresholds={list(wl.thresholds)}: int32 tables "
+         f"({len(wl.G)} x {wl.d * wl.w} counters), 1e5 estimates per scale, top-{k} ids+values per scale"
+         f"{', excursion sets ' + str(n_exc) if n_exc else ''} bit-exact to the oracle over {THREADS} index ranges; "
+         f"scan: {stats}; generate {t_gen:.0f} s, oracle update {t_upd:.0f} s, oracle select {t_sel:.0f} s")
+    g.close(); so.close()
+
+
+def test_cfg3_full_size_against_the_oracle(cs):
+    _device_resident(cs, "cfg3")
+
+
+def test_cfg5_full_size_against_the_oracle(cs):
+    _device_resident(cs, "cfg5")
+
+
+def test_cfg4_three_batches_host_streamed_against_the_oracle(cs):
+    """3 x 2^28 particles of cfg 4 (per-batch generator keys, G = 4642, d = 7, w = 2^24, k = 3e5) from pinned host memory
+    through cs_update_host / cs_scan_host: 48 staging batches of 2^24 particles, three host calls."""
+    from paper_1711_00975_b200 import synth
+    wl = synth.CONFIGS["cfg4"]
+    B, nb = wl.batch, 3
+    cat = synth.Catalogue(wl, "cuda")
+    host = torch.empty((nb * B, 3), dtype=torch.float32, pin_memory=True)
+    for b in range(nb):
+        host[b * B:(b + 1) * B].copy_(synth.generate(wl, device="cuda", batch=b, n=B, catalogue=cat))
+    torch.cuda.synchronize()
+    host_np = host.numpy()
+    k = wl.k
+    g = cs.CountSketch(wl.d, wl.w, list(wl.G), wl.L, wl.seed)
+    for b in range(nb):
+        g.update_host(host[b * B:(b + 1) * B])
+    g.scan_begin(k)
+    for b in range(nb):
+        g.scan_host(host[b * B:(b + 1) * B])
+    stats = g.scan_stats(0)
+    t0 = time.perf_counter()
+    so = ShardedOracle(wl.d, wl.w, wl.G, wl.L, wl.seed, THREADS)
+    for b in range(nb):
+        so.update(host_np[b * B:(b + 1) * B], 1.0, b * B)
+    gt = g.sketch(0).cpu().numpy()
+    assert np.array_equal(gt, so.sketch(0)), f"table differs: {_first_diff(gt, so.sketch(0))}"
+    _estimates_agree(g, so, wl, host_np, np.random.default_rng(12))
+    tops = [so.select(host_np[b * B:(b + 1) * B], k, ora.INT32_MAX, 1.0, b * B)[0][0] for b in range(nb)]
+    ti, te = _merge(tops, k)
+    gi, gv = g.topk(k, 0, device="cpu")
+    assert np.array_equal(_ids(gi), ti), f"top-k ids differ: {_first_diff(_ids(gi), ti)}"
+    assert np.array_equal(gv.numpy(), te), f"top-k values differ: {_first_diff(gv.numpy(), te)}"
+    _log(f"PASS cfg4 x {nb} batches: N={nb * B} host-streamed (48 staging batches) d={wl.d} w={wl.w} G={list(wl.G)} k={k}: "
+         f"int32 table, 1e5 estimates, top-{k} ids+values bit-exact to the oracle over {THREADS} index ranges; scan: {stats}; "
+         f"oracle {time.perf_counter() - t0:.0f} s")
+    g.close(); so.close()

@@ -562,3 +562,35 @@ def test_argument_errors():
             o.update(np.zeros((1, 3), dtype=np.float32), p)
     with pytest.raises(RuntimeError):
         o.topk(3)                                                           # before scan_begin
+
+
+# ---- full-size parity device: the oracle over disjoint index ranges --------------------
+
+@pytest.mark.parametrize("p,G,parts", [(1.0, (32,), 3), (0.6, (16, 32, 64), 4), (0.3, (48,), 7)])
+def test_sharded_oracle_equals_single_oracle(p, G, parts):
+    """ora_select_streaming over P shards (each with the running index of its first particle), tables summed, lists
+    merged by (est desc, id asc, unique), against the plain single-stream oracle: tables, top-k, excursion sets."""
+    from sharded_oracle import ShardedOracle
+    X = _stream(30001, 21, L=64.0)
+    L = 64.0
+    o = ora.OracleSketch(5, 1024, G, L, 9)
+    o.update(X[:12345], p); o.update(X[12345:], p)
+    o.scan_begin(); o.scan(X, p)
+    so = ShardedOracle(5, 1024, G, L, 9, parts)
+    so.update(X[:12345], p, 0)
+    so.update(X[12345:], p, 12345)                         # a second batch continues the running index
+    for k, thr in ((50, 3), (100000, -100)):
+        sel = so.select(X, k, thr, p, 0)
+        for s in range(len(G)):
+            assert np.array_equal(so.sketch(s), o.sketch(s))
+            (ti, te), (xi, xe) = sel[s]
+            oi, oe = o.topk(k, s)
+            assert np.array_equal(ti, oi) and np.array_equal(te, oe)
+            yi, ye, yn = o.excursion(thr, s)
+            assert yn == len(xi) and np.array_equal(xi, yi) and np.array_equal(xe, ye)
+    # one shard alone, no excursion set asked: the streaming selection is ora_scan + ora_topk of that shard
+    (ti, te), (xi, xe) = so.o[0].select_streaming(X[100:9000], 100, 40, sample_p=p)
+    o.scan_begin(); o.set_scan_index(100); o.scan(X[100:9000], p)
+    oi, oe = o.topk(40)
+    assert np.array_equal(ti, oi) and np.array_equal(te, oe) and len(xi) == 0
+    so.close(); o.close()
