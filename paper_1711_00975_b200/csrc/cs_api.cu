@@ -101,6 +101,7 @@ struct cs_sketch {
     int cur[CS_MAX_SCALES] = {};
     bool dirty[CS_MAX_SCALES] = {};
     uint32_t last_compact[CS_MAX_SCALES] = {};
+    uint32_t epoch[CS_MAX_SCALES] = {};   /* look-back epochs of the selector (cs_select.cu), one counter per scale */
     uint64_t n_compactions[CS_MAX_SCALES] = {};
     uint64_t n_scan_launches = 0;
     double rate = 1.0;
@@ -212,6 +213,7 @@ int alloc_candidates(cs_sketch* s, uint32_t cap) {
             CS_CUDA(cudaMalloc(&s->sb[i].ek[h], (size_t)cap * sizeof(uint32_t)));
         }
         CS_CUDA(cudaMalloc(&s->sb[i].scratch, (size_t)select_scratch_words(cap) * sizeof(uint32_t)));
+        CS_CUDA(cudaMemsetAsync(s->sb[i].scratch, 0, (size_t)select_scratch_words(cap) * sizeof(uint32_t), s->stream));
         s->cur[i] = 0;
     }
     s->cap = cap;
@@ -230,15 +232,15 @@ int grow_candidates(cs_sketch* s) {
             CS_CUDA(cudaMalloc(&nb.ek[h], (size_t)cap * sizeof(uint32_t)));
         }
         CS_CUDA(cudaMalloc(&nb.scratch, (size_t)select_scratch_words(cap) * sizeof(uint32_t)));
+        CS_CUDA(cudaMemsetAsync(nb.scratch, 0, (size_t)select_scratch_words(cap) * sizeof(uint32_t), s->stream));
         const uint32_t held = s->st_host[i].count < s->cap ? s->st_host[i].count : s->cap;
-        const int c = s->cur[i];
-        CS_CUDA(cudaMemcpyAsync(nb.id[0], s->sb[i].id[c], (size_t)held * 8, cudaMemcpyDeviceToDevice, s->stream));
-        CS_CUDA(cudaMemcpyAsync(nb.ek[0], s->sb[i].ek[c], (size_t)held * 4, cudaMemcpyDeviceToDevice, s->stream));
+        const int c = s->cur[i];                             /* the list stays in the same half: the device names it too */
+        CS_CUDA(cudaMemcpyAsync(nb.id[c], s->sb[i].id[c], (size_t)held * 8, cudaMemcpyDeviceToDevice, s->stream));
+        CS_CUDA(cudaMemcpyAsync(nb.ek[c], s->sb[i].ek[c], (size_t)held * 4, cudaMemcpyDeviceToDevice, s->stream));
         CS_CUDA(cudaStreamSynchronize(s->stream));
         for (int h = 0; h < 2; ++h) { cudaFree(s->sb[i].id[h]); cudaFree(s->sb[i].ek[h]); }
         cudaFree(s->sb[i].scratch);
         s->sb[i] = nb;
-        s->cur[i] = 0;
     }
     s->cap = cap;
     return CS_OK;
@@ -247,20 +249,16 @@ int grow_candidates(cs_sketch* s) {
 int read_states(cs_sketch* s) {
     CS_CUDA(cudaMemcpyAsync(s->st_host, s->st_dev, sizeof(ScanState) * s->n_scales, cudaMemcpyDeviceToHost, s->stream));
     CS_CUDA(cudaStreamSynchronize(s->stream));
+    for (int i = 0; i < s->n_scales; ++i) s->cur[i] = (int)(s->st_host[i].half & 1u);   /* compactions move the list */
     return CS_OK;
 }
 
-/* Sort + dedupe + cut the candidate list of one scale (device side only; caller reads the states back). */
+/* Sort + dedupe + cut the candidate list of one scale: enqueued only, no synchronisation.  The list may end up in the
+ * other half of its ping-pong buffers: the caller reads the states back (read_states) before it uses s->cur again. */
 int compact_scale(cs_sketch* s, int i) {
     const uint32_t n = s->st_host[i].count < s->cap ? s->st_host[i].count : s->cap;
-    cudaError_t e = launch_est_range(s->sb[i].ek[s->cur[i]], n, s->st_dev + i, s->stream);
-    if (e != cudaSuccess) return fail(CS_ERR_CUDA, "range kernel: %s", cudaGetErrorString(e));
-    s->launches += n ? 2 : 1;
-    int rc = read_states(s);          /* the number of radix passes over the estimate depends on its range */
-    if (rc) return rc;
-    const ScanState& h = s->st_host[i];
-    s->cur[i] = select_compact(s->sb[i], s->cur[i], n, s->id_bits[i], h.est_min, h.est_max, s->st_dev + i, s->k_max,
-                               s->thr_min, s->stream, &s->launches, &e);
+    cudaError_t e = select_compact(s->sb[i], s->cap, s->cur[i], n, s->id_bits[i], s->st_dev + i, s->k_max, s->thr_min, s->stream,
+                                   &s->launches, &s->epoch[i]);
     if (e != cudaSuccess) return fail(CS_ERR_CUDA, "select_compact: %s", cudaGetErrorString(e));
     s->dirty[i] = false;
     s->n_compactions[i] += 1;
@@ -1358,6 +1356,8 @@ int cs_scan_begin(cs_sketch* s, uint64_t k_max, int32_t thr_min) {
         s->st_host[i].est_min = INT32_MAX;
         s->st_host[i].est_max = INT32_MIN;
         s->st_host[i].uniq = 0;
+        s->st_host[i].half = 0;
+        s->cur[i] = 0;
         s->dirty[i] = false; s->last_compact[i] = 0; s->n_compactions[i] = 0;
     }
     CS_CUDA(cudaMemcpyAsync(s->st_dev, s->st_host, sizeof(ScanState) * s->n_scales, cudaMemcpyHostToDevice, s->stream));

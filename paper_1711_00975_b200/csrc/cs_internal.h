@@ -34,8 +34,9 @@ struct ScanState {
     int32_t tau;       // current collection threshold: only estimates >= tau are collected
     int32_t est_min;   // min / max estimate among the entries held (bounds the radix passes over the estimate)
     int32_t est_max;
-    uint32_t uniq;     // scratch: number of unique entries after the last compaction, before the cut
-    uint32_t pad[3];
+    uint32_t uniq;     // number of unique entries after the last compaction, before the cut
+    uint32_t half;     // which half of the ping-pong candidate buffers holds the list (set by every compaction)
+    uint32_t pad[2];
 };
 
 struct ScanTarget {
@@ -126,21 +127,19 @@ cudaError_t launch_recount(const ScaleParams& sp, const float* xyz, uint64_t n, 
                            uint32_t mask, uint32_t* counts, float* out, uint32_t* out_count, uint64_t cap, int sm_count,
                            cudaStream_t st);
 
-/* selection (cs_select.cu): sort the first n candidates of `src` by (ek ascending, id ascending), drop
- * duplicate ids, cut to the entries that can still matter and update *st (count, tau, est_min, est_max).
- * The result is left in `dst`.  scratch: at least select_scratch_words(n) uint32 words. */
+/* selection (cs_select.cu): sort the first n candidates of one half by (ek ascending, id ascending), drop
+ * duplicate ids, cut to the entries that can still matter and update *st (count, tau, est_min, est_max, half).
+ * scratch: at least select_scratch_words(cap) uint32 words. */
 struct SelectBuffers {
     uint64_t* id[2];
     uint32_t* ek[2];
     uint32_t* scratch;
 };
-uint64_t select_scratch_words(uint64_t n);
-/* st->est_min / est_max = range of the estimates of the first n (unsorted) entries */
-cudaError_t launch_est_range(const uint32_t* ek, uint32_t n, ScanState* st_dev, cudaStream_t st);
-/* returns the index (0/1) of the half that holds the result; *launches += kernels launched */
-int select_compact(const SelectBuffers& B, int src, uint32_t n, int id_bits, int32_t est_min, int32_t est_max,
-                   ScanState* st_dev, uint64_t k_max, int32_t thr_min, cudaStream_t stream, uint64_t* launches,
-                   cudaError_t* err);
+uint64_t select_scratch_words(uint64_t cap);      /* scratch must be zeroed once after allocation */
+/* Enqueues one compaction of the first n entries of half `src` of buffers with room for `cap` entries: no host round
+ * trip inside; st_dev->half / count / tau describe the result.  *launches += kernels launched; *epoch: per-buffer counter. */
+cudaError_t select_compact(const SelectBuffers& B, uint32_t cap, int src, uint32_t n, int id_bits, ScanState* st_dev,
+                           uint64_t k_max, int32_t thr_min, cudaStream_t stream, uint64_t* launches, uint32_t* epoch);
 cudaError_t launch_emit_prefix(const uint64_t* id, const uint32_t* ek, uint32_t n, uint64_t* ids_out,
                                int32_t* est_out, cudaStream_t st);
 /* number of leading entries (sorted by ek ascending) with estimate >= thr, written to *n_out_dev */

@@ -12,8 +12,16 @@
  * (no cell with a smaller estimate can enter the top k_max or an excursion set with thr >= thr_min).
  * Top-k for any k <= k_max and the excursion set for any thr >= thr_min are then prefixes of the list.
  *
- * Kernels: k_hist (per-tile digit counts), k_exscan (single-block exclusive scan), k_scatter (stable
- * scatter: warp match.any ranks + per-warp digit counters), k_uniq_count / k_uniq_scatter, k_cut, k_emit.
+ * One compaction = a fixed sequence of launches, with no host round trip in it:
+ *   k_radix_hist   digit histograms of ALL passes in one sweep over the list
+ *   k_radix_plan   one block: which passes are needed (a digit that is the same in every entry is skipped on the device:
+ *                  the high bytes of the estimate key almost always are), exclusive digit bases, ping-pong plan
+ *   k_radix_pass   one launch per digit: every tile ranks its entries (warp match.any + per-warp digit counters, stable),
+ *                  publishes its digit counts and obtains its offsets from the tiles before it by decoupled look-back
+ *                  (tiles take tickets in order, so a tile only ever waits for tiles that already run)
+ *   k_uniq         drops duplicate ids, again with a look-back over tile totals
+ *   k_cut          fixes the new tau and the number of entries kept, records which half of the ping-pong buffers holds
+ *                  the list (the host learns it when it next reads the scan states)
  */
 #include "cs_device.cuh"
 
@@ -24,55 +32,71 @@ constexpr int SORT_WARPS = SORT_THREADS / 32;
 constexpr int SORT_ITEMS = 8;                              // items per lane
 constexpr int SORT_TILE = SORT_THREADS * SORT_ITEMS;       // 2048 entries per block
 constexpr int SORT_SEG = 32 * SORT_ITEMS;                  // consecutive entries owned by one warp
+constexpr int MAX_PASSES = 12;                             // 8 id bytes (ids < 2^60 need 8) + 4 estimate-key bytes
 
-__device__ __forceinline__ uint32_t digit_of(uint64_t id, uint32_t ek, int from_ek, int shift, uint32_t ek_base) {
-    return from_ek ? (((ek - ek_base) >> shift) & 255u) : ((uint32_t)(id >> shift) & 255u);
+/* Device-side plan of one compaction; lives at the start of SelectBuffers::scratch, zeroed before every compaction. */
+struct SortPlan {
+    uint32_t hist[MAX_PASSES][256];    // digit counts; k_radix_plan turns them into exclusive bases
+    uint32_t active[MAX_PASSES];       // 0: every entry has the same digit in this pass -> nothing to do
+    uint32_t src_half[MAX_PASSES];     // which half (0/1) pass p reads
+    uint32_t ticket[MAX_PASSES + 1];   // tile tickets per pass, last = k_uniq
+    uint32_t sorted_half;              // half that holds the sorted list
+    uint32_t uniq_total;               // unique entries
+    uint32_t pad[2];
+};
+
+/* look-back status word: epoch << 34 | flag << 32 | count; a word of another epoch reads as "not published yet" */
+constexpr uint64_t FLAG_AGG = 1, FLAG_INC = 2;
+__device__ __forceinline__ uint64_t status_word(uint32_t epoch, uint64_t flag, uint32_t count) {
+    return ((uint64_t)epoch << 34) | (flag << 32) | count;
+}
+__device__ __forceinline__ uint64_t ld_status(const uint64_t* p) {
+    uint64_t v;
+    asm volatile("ld.global.relaxed.gpu.u64 %0, [%1];" : "=l"(v) : "l"(p));
+    return v;
+}
+__device__ __forceinline__ void st_status(uint64_t* p, uint64_t v) {
+    asm volatile("st.global.relaxed.gpu.u64 [%0], %1;" :: "l"(p), "l"(v) : "memory");
 }
 
-/* counts[digit * nblocks + block] = number of entries of this block's tile with that digit */
+struct HalfPtrs {
+    uint64_t* id[2];
+    uint32_t* ek[2];
+};
+
+__device__ __forceinline__ uint32_t digit_of(uint64_t id, uint32_t ek, int pass, int id_passes) {
+    return pass < id_passes ? ((uint32_t)(id >> (8 * pass)) & 255u) : ((ek >> (8 * (pass - id_passes))) & 255u);
+}
+
+/* hist[p][digit] += entries of the list with that digit in pass p, for all passes at once */
 __global__ void __launch_bounds__(SORT_THREADS)
-k_hist(const uint64_t* __restrict__ id, const uint32_t* __restrict__ ek, uint32_t n, int from_ek, int shift,
-       uint32_t ek_base, uint32_t* __restrict__ counts, uint32_t nblocks) {
-    __shared__ uint32_t h[256];
-    h[threadIdx.x] = 0;
+k_radix_hist(const uint64_t* __restrict__ id, const uint32_t* __restrict__ ek, uint32_t n, int id_passes, int passes,
+             SortPlan* plan) {
+    __shared__ uint32_t h[MAX_PASSES][256];
+    for (int i = threadIdx.x; i < passes * 256; i += SORT_THREADS) (&h[0][0])[i] = 0;
     __syncthreads();
-    const uint32_t t0 = blockIdx.x * SORT_TILE;
-    for (int r = 0; r < SORT_ITEMS; ++r) {
-        uint32_t i = t0 + r * SORT_THREADS + threadIdx.x;
-        if (i < n) atomicAdd(&h[digit_of(from_ek ? 0 : id[i], from_ek ? ek[i] : 0, from_ek, shift, ek_base)], 1u);
+    const uint32_t stride = gridDim.x * SORT_THREADS;
+    for (uint32_t i = blockIdx.x * SORT_THREADS + threadIdx.x; i < n; i += stride) {
+        const uint64_t c = id[i];
+        const uint32_t k = ek[i];
+        for (int p = 0; p < passes; ++p) atomicAdd(&h[p][digit_of(c, k, p, id_passes)], 1u);
     }
     __syncthreads();
-    counts[threadIdx.x * nblocks + blockIdx.x] = h[threadIdx.x];
+    for (int i = threadIdx.x; i < passes * 256; i += SORT_THREADS) {
+        const uint32_t v = (&h[0][0])[i];
+        if (v) atomicAdd(&plan->hist[0][0] + i, v);
+    }
 }
 
-/* In-place exclusive prefix sum of a[0..len) by one block of 1024 threads; *total_out (optional) = sum.
- * Tiles of 16384 words: 16 words per thread (four 16-byte accesses when aligned), warp-shuffle scans, a running carry
- * between tiles. */
-constexpr int EX_PER = 16;
-__global__ void __launch_bounds__(1024) k_exscan(uint32_t* __restrict__ a, uint32_t len, uint32_t* total_out) {
-    __shared__ uint32_t wsum[32];
-    __shared__ uint32_t s_carry;
-    const uint32_t lane = threadIdx.x & 31u, warp = threadIdx.x >> 5;
-    if (threadIdx.x == 0) s_carry = 0;
-    __syncthreads();
-    const bool vec = (reinterpret_cast<uintptr_t>(a) & 15u) == 0;
-    for (uint32_t t0 = 0; t0 < len; t0 += 1024 * EX_PER) {
-        const uint32_t i = t0 + threadIdx.x * EX_PER;
-        uint32_t v[EX_PER];
-        if (vec && i + EX_PER <= len) {
-#pragma unroll
-            for (int q = 0; q < EX_PER / 4; ++q) {
-                const uint4 u = reinterpret_cast<const uint4*>(a + i)[q];
-                v[4 * q] = u.x; v[4 * q + 1] = u.y; v[4 * q + 2] = u.z; v[4 * q + 3] = u.w;
-            }
-        } else {
-#pragma unroll
-            for (int k = 0; k < EX_PER; ++k) v[k] = i + k < len ? a[i + k] : 0;
-        }
-        uint32_t mine = 0;
-#pragma unroll
-        for (int k = 0; k < EX_PER; ++k) mine += v[k];
-        uint32_t incl = mine;
+/* One block of 256 threads: thread t = digit t. */
+__global__ void __launch_bounds__(256) k_radix_plan(SortPlan* plan, uint32_t n, int passes, uint32_t first_half) {
+    __shared__ uint32_t wsum[8];
+    __shared__ uint32_t s_active[MAX_PASSES];
+    const uint32_t t = threadIdx.x, lane = t & 31u, warp = t >> 5;
+    for (int p = 0; p < passes; ++p) {
+        const uint32_t c = plan->hist[p][t];
+        const int trivial = __syncthreads_or(c == n);
+        uint32_t incl = c;
 #pragma unroll
         for (int off = 1; off < 32; off <<= 1) {
             const uint32_t u = __shfl_up_sync(0xFFFFFFFFu, incl, off);
@@ -80,50 +104,43 @@ __global__ void __launch_bounds__(1024) k_exscan(uint32_t* __restrict__ a, uint3
         }
         if (lane == 31) wsum[warp] = incl;
         __syncthreads();
-        if (warp == 0) {
-            uint32_t w = wsum[lane], wi = w;
-#pragma unroll
-            for (int off = 1; off < 32; off <<= 1) {
-                const uint32_t u = __shfl_up_sync(0xFFFFFFFFu, wi, off);
-                if (lane >= off) wi += u;
-            }
-            wsum[lane] = wi - w;                                   // exclusive prefix of the warp totals
-        }
-        __syncthreads();
-        uint32_t run = s_carry + wsum[warp] + incl - mine;
-#pragma unroll
-        for (int k = 0; k < EX_PER; ++k) {
-            const uint32_t x = v[k];
-            v[k] = run;
-            run += x;
-        }
-        if (vec && i + EX_PER <= len) {
-#pragma unroll
-            for (int q = 0; q < EX_PER / 4; ++q)
-                reinterpret_cast<uint4*>(a + i)[q] = make_uint4(v[4 * q], v[4 * q + 1], v[4 * q + 2], v[4 * q + 3]);
-        } else {
-#pragma unroll
-            for (int k = 0; k < EX_PER; ++k)
-                if (i + k < len) a[i + k] = v[k];
-        }
-        __syncthreads();
-        if (threadIdx.x == 1023) s_carry = run;                    // total up to the end of this tile
+        uint32_t base = 0;
+        for (uint32_t q = 0; q < warp; ++q) base += wsum[q];
+        plan->hist[p][t] = base + incl - c;                    // exclusive base of digit t
+        if (t == 0) s_active[p] = trivial ? 0u : 1u;
         __syncthreads();
     }
-    if (total_out && threadIdx.x == 0) *total_out = s_carry;
+    if (t == 0) {
+        uint32_t half = first_half;
+        for (int p = 0; p < passes; ++p) {
+            plan->active[p] = s_active[p];
+            plan->src_half[p] = half;
+            if (s_active[p]) half ^= 1u;
+        }
+        plan->sorted_half = half;
+    }
 }
 
-/* Stable scatter of one radix pass.  Warp wq owns entries [t0 + wq*SORT_SEG, +SORT_SEG) in order; within a
- * round of 32 the rank among equal digits comes from match.any, across rounds from a per-warp counter. */
+/* One radix pass, stable.  Warp wq of a tile owns entries [t0 + wq*SORT_SEG, +SORT_SEG) in order; within a round of 32
+ * the rank among equal digits comes from match.any, across rounds from a per-warp counter.  status: tiles x 256 words. */
 __global__ void __launch_bounds__(SORT_THREADS)
-k_scatter(const uint64_t* __restrict__ sid, const uint32_t* __restrict__ sek, uint64_t* __restrict__ did,
-          uint32_t* __restrict__ dek, uint32_t n, int from_ek, int shift, uint32_t ek_base,
-          const uint32_t* __restrict__ offsets, uint32_t nblocks) {
+k_radix_pass(const __grid_constant__ HalfPtrs H, uint32_t n, int pass, int id_passes, SortPlan* plan,
+             uint64_t* __restrict__ status, uint32_t epoch) {
+    if (!plan->active[pass]) return;
     __shared__ uint32_t wcnt[SORT_WARPS][256];
+    __shared__ uint32_t s_tile;
     const uint32_t lane = threadIdx.x & 31u, wq = threadIdx.x >> 5;
+    if (threadIdx.x == 0) s_tile = atomicAdd(&plan->ticket[pass], 1u);
     for (int i = threadIdx.x; i < SORT_WARPS * 256; i += SORT_THREADS) (&wcnt[0][0])[i] = 0;
     __syncthreads();
-    const uint32_t base = blockIdx.x * SORT_TILE + wq * SORT_SEG;
+    const uint32_t tile = s_tile;
+    const uint32_t src = plan->src_half[pass];
+    const uint64_t* __restrict__ sid = H.id[src];
+    const uint32_t* __restrict__ sek = H.ek[src];
+    uint64_t* __restrict__ did = H.id[src ^ 1u];
+    uint32_t* __restrict__ dek = H.ek[src ^ 1u];
+
+    const uint32_t base = tile * SORT_TILE + wq * SORT_SEG;
     uint64_t kid[SORT_ITEMS];
     uint32_t kek[SORT_ITEMS], off[SORT_ITEMS];
     uint32_t* mine = wcnt[wq];
@@ -133,22 +150,41 @@ k_scatter(const uint64_t* __restrict__ sid, const uint32_t* __restrict__ sek, ui
         const bool valid = i < n;
         kid[r] = valid ? sid[i] : 0;
         kek[r] = valid ? sek[i] : 0;
-        const uint32_t dg = valid ? digit_of(kid[r], kek[r], from_ek, shift, ek_base) : 255u;
+        const uint32_t dg = valid ? digit_of(kid[r], kek[r], pass, id_passes) : 255u;
         const uint32_t peers = __match_any_sync(0xFFFFFFFFu, dg);
         const uint32_t rank = __popc(peers & ((1u << lane) - 1u));
         const uint32_t before = mine[dg];
         __syncwarp();
-        if (rank == 0) mine[dg] = before + __popc(peers);
-        __syncwarp();
+        if (rank == 0) mine[dg] = before + __popc(peers);       // invalid lanes inflate digit 255 of the last tile only:
+        __syncwarp();                                           // nothing is ranked after them
         off[r] = before + rank;
     }
     __syncthreads();
-    {   /* thread t = digit t: turn per-warp counts into per-warp bases (global offset of this block first) */
-        uint32_t run = offsets[threadIdx.x * nblocks + blockIdx.x];
+    {   /* thread t = digit t: tile count -> publish -> look back -> per-warp bases */
+        const uint32_t t = threadIdx.x;
+        uint32_t cnt = 0;
+#pragma unroll
+        for (int q = 0; q < SORT_WARPS; ++q) cnt += wcnt[q][t];
+        uint64_t* my = status + (uint64_t)tile * 256 + t;
+        uint32_t excl = 0;
+        if (tile == 0) {
+            st_status(my, status_word(epoch, FLAG_INC, cnt));
+        } else {
+            st_status(my, status_word(epoch, FLAG_AGG, cnt));
+            for (uint32_t j = tile; j-- > 0;) {
+                const uint64_t* theirs = status + (uint64_t)j * 256 + t;
+                uint64_t w;
+                do { w = ld_status(theirs); } while ((uint32_t)(w >> 34) != epoch || ((w >> 32) & 3u) == 0);
+                excl += (uint32_t)w;
+                if ((w >> 32) & FLAG_INC) break;
+            }
+            st_status(my, status_word(epoch, FLAG_INC, excl + cnt));
+        }
+        uint32_t run = plan->hist[pass][t] + excl;
 #pragma unroll
         for (int q = 0; q < SORT_WARPS; ++q) {
-            uint32_t c = wcnt[q][threadIdx.x];
-            wcnt[q][threadIdx.x] = run;
+            const uint32_t c = wcnt[q][t];
+            wcnt[q][t] = run;
             run += c;
         }
     }
@@ -157,7 +193,7 @@ k_scatter(const uint64_t* __restrict__ sid, const uint32_t* __restrict__ sek, ui
     for (int r = 0; r < SORT_ITEMS; ++r) {
         const uint32_t i = base + r * 32 + lane;
         if (i < n) {
-            const uint32_t dg = digit_of(kid[r], kek[r], from_ek, shift, ek_base);
+            const uint32_t dg = digit_of(kid[r], kek[r], pass, id_passes);
             const uint32_t dst = mine[dg] + off[r];
             did[dst] = kid[r];
             dek[dst] = kek[r];
@@ -165,99 +201,81 @@ k_scatter(const uint64_t* __restrict__ sid, const uint32_t* __restrict__ sek, ui
     }
 }
 
-/* ---- estimate range of an unsorted list (bounds the radix passes over the estimate key) -------------------------- */
+/* ---- duplicate removal on the sorted list ------------------------------------------------------------------------ */
 
-__global__ void k_est_range_init(ScanState* st) {
-    st->est_min = INT32_MAX;
-    st->est_max = INT32_MIN;
-}
-
-__global__ void __launch_bounds__(256) k_est_range(const uint32_t* __restrict__ ek, uint32_t n, ScanState* st) {
-    uint32_t lo = 0xFFFFFFFFu, hi = 0;                     // keys: ascending key = descending estimate
-    const uint32_t stride = gridDim.x * 256;
-    for (uint32_t i = blockIdx.x * 256 + threadIdx.x; i < n; i += stride) {
-        const uint32_t k = ek[i];
-        lo = min(lo, k); hi = max(hi, k);
-    }
-    lo = __reduce_min_sync(0xFFFFFFFFu, lo);
-    hi = __reduce_max_sync(0xFFFFFFFFu, hi);
-    if ((threadIdx.x & 31) == 0 && lo <= hi) {
-        atomicMax(&st->est_max, key_to_est(lo));
-        atomicMin(&st->est_min, key_to_est(hi));
-    }
-}
-
-cudaError_t launch_est_range(const uint32_t* ek, uint32_t n, ScanState* st_dev, cudaStream_t st) {
-    k_est_range_init<<<1, 1, 0, st>>>(st_dev);
-    if (n) {
-        uint32_t blocks = (n + 255) / 256;
-        if (blocks > 148 * 4) blocks = 148 * 4;
-        k_est_range<<<blocks, 256, 0, st>>>(ek, n, st_dev);
-    }
-    return cudaGetLastError();
-}
-
-/* ---- duplicate removal on the sorted list --------------------------------------------------------------- */
-
-__device__ __forceinline__ bool is_first(const uint64_t* id, uint32_t i) { return i == 0 || id[i] != id[i - 1]; }
-
+/* Each thread owns SORT_ITEMS consecutive entries; block scan of the per-thread counts of "first of its id" flags; the
+ * tile's offset comes from a look-back over the tile totals (ustatus: one word per tile). */
 __global__ void __launch_bounds__(SORT_THREADS)
-k_uniq_count(const uint64_t* __restrict__ id, uint32_t n, uint32_t* __restrict__ blockcnt) {
+k_uniq(const __grid_constant__ HalfPtrs H, uint32_t n, SortPlan* plan, uint64_t* __restrict__ ustatus, uint32_t epoch,
+       uint32_t tiles) {
     __shared__ uint32_t wsum[SORT_WARPS];
-    const uint32_t t0 = blockIdx.x * SORT_TILE;
-    uint32_t c = 0;
-    for (int r = 0; r < SORT_ITEMS; ++r) {
-        uint32_t i = t0 + r * SORT_THREADS + threadIdx.x;
-        if (i < n) c += is_first(id, i);
-    }
-    c = __reduce_add_sync(0xFFFFFFFFu, c);
-    if ((threadIdx.x & 31) == 0) wsum[threadIdx.x >> 5] = c;
+    __shared__ uint32_t s_tile, s_excl;
+    if (threadIdx.x == 0) s_tile = atomicAdd(&plan->ticket[MAX_PASSES], 1u);
     __syncthreads();
-    if (threadIdx.x == 0) {
-        uint32_t s = 0;
-        for (int q = 0; q < SORT_WARPS; ++q) s += wsum[q];
-        blockcnt[blockIdx.x] = s;
-    }
-}
-
-/* Each thread owns SORT_ITEMS consecutive entries; block-exclusive scan of the per-thread flag counts. */
-__global__ void __launch_bounds__(SORT_THREADS)
-k_uniq_scatter(const uint64_t* __restrict__ sid, const uint32_t* __restrict__ sek, uint64_t* __restrict__ did,
-               uint32_t* __restrict__ dek, uint32_t n, const uint32_t* __restrict__ blockoff) {
-    __shared__ uint32_t wsum[SORT_WARPS];
-    const uint32_t first = blockIdx.x * SORT_TILE + threadIdx.x * SORT_ITEMS;
+    const uint32_t tile = s_tile;
+    const uint32_t src = plan->sorted_half;
+    const uint64_t* __restrict__ sid = H.id[src];
+    const uint32_t* __restrict__ sek = H.ek[src];
+    uint64_t* __restrict__ did = H.id[src ^ 1u];
+    uint32_t* __restrict__ dek = H.ek[src ^ 1u];
+    const uint32_t first = tile * SORT_TILE + threadIdx.x * SORT_ITEMS;
+    uint64_t v[SORT_ITEMS];
+    uint64_t prev = (first > 0 && first <= n) ? sid[first - 1] : 0;
     uint32_t flags = 0, c = 0;
 #pragma unroll
     for (int r = 0; r < SORT_ITEMS; ++r) {
-        uint32_t i = first + r;
-        if (i < n && is_first(sid, i)) { flags |= 1u << r; ++c; }
+        const uint32_t i = first + r;
+        v[r] = i < n ? sid[i] : 0;
+        if (i < n && (i == 0 || v[r] != prev)) { flags |= 1u << r; ++c; }
+        prev = v[r];
     }
     const uint32_t lane = threadIdx.x & 31u, wq = threadIdx.x >> 5;
     uint32_t incl = c;
 #pragma unroll
     for (int off = 1; off < 32; off <<= 1) {
-        uint32_t v = __shfl_up_sync(0xFFFFFFFFu, incl, off);
-        if (lane >= off) incl += v;
+        const uint32_t u = __shfl_up_sync(0xFFFFFFFFu, incl, off);
+        if (lane >= off) incl += u;
     }
     if (lane == 31) wsum[wq] = incl;
     __syncthreads();
-    uint32_t wbase = 0;
-    for (uint32_t q = 0; q < wq; ++q) wbase += wsum[q];
-    uint32_t dst = blockoff[blockIdx.x] + wbase + incl - c;
+    uint32_t wbase = 0, total = 0;
+    for (uint32_t q = 0; q < SORT_WARPS; ++q) { if (q < wq) wbase += wsum[q]; total += wsum[q]; }
+    if (threadIdx.x == 0) {
+        uint32_t excl = 0;
+        if (tile == 0) {
+            st_status(ustatus, status_word(epoch, FLAG_INC, total));
+        } else {
+            st_status(ustatus + tile, status_word(epoch, FLAG_AGG, total));
+            for (uint32_t j = tile; j-- > 0;) {
+                uint64_t w;
+                do { w = ld_status(ustatus + j); } while ((uint32_t)(w >> 34) != epoch || ((w >> 32) & 3u) == 0);
+                excl += (uint32_t)w;
+                if ((w >> 32) & FLAG_INC) break;
+            }
+            st_status(ustatus + tile, status_word(epoch, FLAG_INC, excl + total));
+        }
+        s_excl = excl;
+        if (tile == tiles - 1) plan->uniq_total = excl + total;
+    }
+    __syncthreads();
+    uint32_t dst = s_excl + wbase + incl - c;
 #pragma unroll
     for (int r = 0; r < SORT_ITEMS; ++r) {
         if (flags & (1u << r)) {
-            did[dst] = sid[first + r];
+            did[dst] = v[r];
             dek[dst] = sek[first + r];
             ++dst;
         }
     }
 }
 
-/* One thread: m unique sorted entries in ek[0..m).  Fixes the new tau and the number of entries kept. */
-__global__ void k_cut(const uint32_t* __restrict__ ek, const uint32_t* __restrict__ m_ptr, uint32_t m_const,
-                      ScanState* st, uint64_t k_max, int32_t thr_min) {
-    const uint32_t m = m_ptr ? *m_ptr : m_const;
+/* One thread.  The m unique sorted entries are in half `half` (or, with plan != NULL, in the half k_uniq wrote: the one
+ * opposite to plan->sorted_half, m = plan->uniq_total).  Fixes the new tau and the number of entries kept. */
+__global__ void k_cut(const __grid_constant__ HalfPtrs H, const SortPlan* plan, uint32_t half_const, ScanState* st,
+                      uint64_t k_max, int32_t thr_min) {
+    const uint32_t half = plan ? (plan->sorted_half ^ 1u) : half_const;
+    const uint32_t m = plan ? plan->uniq_total : 0u;
+    const uint32_t* __restrict__ ek = H.ek[half];
     int32_t tau_k;
     if (k_max == 0) tau_k = INT32_MAX;                       // no top-k asked: only thr_min bounds tau
     else tau_k = (m >= k_max) ? key_to_est(ek[k_max - 1]) : INT32_MIN;
@@ -275,6 +293,7 @@ __global__ void k_cut(const uint32_t* __restrict__ ek, const uint32_t* __restric
     st->tau = tau;
     st->est_max = lo ? key_to_est(ek[0]) : INT32_MIN;
     st->est_min = lo ? key_to_est(ek[lo - 1]) : INT32_MAX;
+    st->half = half;
 }
 
 __global__ void __launch_bounds__(256)
@@ -302,53 +321,43 @@ __global__ void k_count_ge(const uint32_t* __restrict__ ek, uint32_t n, int32_t 
 
 static uint32_t tiles_of(uint64_t n) { return (uint32_t)((n + SORT_TILE - 1) / SORT_TILE); }
 
+/* scratch layout (uint32 words): SortPlan | status[tiles][256] (u64) | ustatus[tiles] (u64) */
+static uint64_t plan_words() { return (sizeof(SortPlan) + 15) / 16 * 4; }
 uint64_t select_scratch_words(uint64_t n) {
-    return (uint64_t)tiles_of(n) * 256 + tiles_of(n) + 64;
+    const uint64_t t = tiles_of(n) + 1;
+    return plan_words() + t * 256 * 2 + t * 2 + 16;
 }
 
-static int bits_of(uint64_t v) {
-    int b = 0;
-    while (v) { ++b; v >>= 1; }
-    return b;
-}
-
-int select_compact(const SelectBuffers& B, int src, uint32_t n, int id_bits, int32_t est_min, int32_t est_max,
-                   ScanState* st_dev, uint64_t k_max, int32_t thr_min, cudaStream_t stream, uint64_t* launches,
-                   cudaError_t* err) {
-    *err = cudaSuccess;
-    int cur = src;
+/* Enqueues one compaction of the first n entries of half `src` (all on `stream`, no synchronisation).  Afterwards
+ * st_dev->half names the half that holds the list and st_dev->count its length.  *epoch: per-buffer launch counter. */
+cudaError_t select_compact(const SelectBuffers& B, uint32_t cap, int src, uint32_t n, int id_bits, ScanState* st_dev,
+                           uint64_t k_max, int32_t thr_min, cudaStream_t stream, uint64_t* launches, uint32_t* epoch) {
+    HalfPtrs H;
+    for (int h = 0; h < 2; ++h) { H.id[h] = B.id[h]; H.ek[h] = B.ek[h]; }
     if (n == 0) {
-        k_cut<<<1, 1, 0, stream>>>(B.ek[cur], nullptr, 0, st_dev, k_max, thr_min);
+        k_cut<<<1, 1, 0, stream>>>(H, nullptr, (uint32_t)src, st_dev, k_max, thr_min);
         *launches += 1;
-        *err = cudaGetLastError();
-        return cur;
+        return cudaGetLastError();
     }
-    const uint32_t nb = tiles_of(n);
-    uint32_t* counts = B.scratch;                     // 256 * nb words
-    uint32_t* blockcnt = B.scratch + (uint64_t)256 * nb;   // nb words
-    uint32_t* total = blockcnt + nb;                  // 1 word
-    /* LSD passes: id bytes first (least significant key), then the estimate key relative to its minimum */
-    const uint32_t ek_base = est_to_key(est_max);                    // smallest key present
-    const uint32_t ek_span = est_to_key(est_min) - ek_base;          // largest key - smallest key
-    const int id_passes = (id_bits + 7) / 8, ek_passes = (bits_of(ek_span) + 7) / 8;
-    for (int p = 0; p < id_passes + ek_passes; ++p) {
-        const int from_ek = p >= id_passes;
-        const int shift = 8 * (from_ek ? p - id_passes : p);
-        k_hist<<<nb, SORT_THREADS, 0, stream>>>(B.id[cur], B.ek[cur], n, from_ek, shift, ek_base, counts, nb);
-        k_exscan<<<1, 1024, 0, stream>>>(counts, 256 * nb, nullptr);
-        k_scatter<<<nb, SORT_THREADS, 0, stream>>>(B.id[cur], B.ek[cur], B.id[cur ^ 1], B.ek[cur ^ 1], n, from_ek,
-                                                   shift, ek_base, counts, nb);
-        *launches += 3;
-        cur ^= 1;
+    SortPlan* plan = reinterpret_cast<SortPlan*>(B.scratch);
+    uint64_t* status = reinterpret_cast<uint64_t*>(B.scratch + plan_words());
+    uint64_t* ustatus = status + (uint64_t)(tiles_of(cap) + 1) * 256;
+    const uint32_t tiles = tiles_of(n);
+    const int id_passes = (id_bits + 7) / 8, passes = id_passes + 4;
+    cudaError_t e = cudaMemsetAsync(plan, 0, sizeof(SortPlan), stream);
+    if (e != cudaSuccess) return e;
+    uint32_t hb = tiles < 148u * 8u ? tiles : 148u * 8u;
+    k_radix_hist<<<hb, SORT_THREADS, 0, stream>>>(B.id[src], B.ek[src], n, id_passes, passes, plan);
+    k_radix_plan<<<1, 256, 0, stream>>>(plan, n, passes, (uint32_t)src);
+    for (int p = 0; p < passes; ++p) {
+        *epoch += 1;
+        k_radix_pass<<<tiles, SORT_THREADS, 0, stream>>>(H, n, p, id_passes, plan, status, *epoch & 0x3FFFFFFFu);
     }
-    k_uniq_count<<<nb, SORT_THREADS, 0, stream>>>(B.id[cur], n, blockcnt);
-    k_exscan<<<1, 1024, 0, stream>>>(blockcnt, nb, total);
-    k_uniq_scatter<<<nb, SORT_THREADS, 0, stream>>>(B.id[cur], B.ek[cur], B.id[cur ^ 1], B.ek[cur ^ 1], n, blockcnt);
-    cur ^= 1;
-    k_cut<<<1, 1, 0, stream>>>(B.ek[cur], total, 0, st_dev, k_max, thr_min);
-    *launches += 4;
-    *err = cudaGetLastError();
-    return cur;
+    *epoch += 1;
+    k_uniq<<<tiles, SORT_THREADS, 0, stream>>>(H, n, plan, ustatus, *epoch & 0x3FFFFFFFu, tiles);
+    k_cut<<<1, 1, 0, stream>>>(H, plan, 0u, st_dev, k_max, thr_min);
+    *launches += 4 + passes;
+    return cudaGetLastError();
 }
 
 cudaError_t launch_emit_prefix(const uint64_t* id, const uint32_t* ek, uint32_t n, uint64_t* ids_out,
