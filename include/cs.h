@@ -263,6 +263,28 @@ int cs_sketch_read(cs_sketch* s, int scale, int32_t* out_d_by_w);       /* any p
 int cs_sketch_add(cs_sketch* s, int scale, const int32_t* in_d_by_w);   /* any pointer; T += in, wraparound  */
 int cs_coeffs(cs_sketch* s, int scale, uint64_t* out_4d_host, uint64_t* K_out_host);
 
+/* Device address of the d*w int32 counters of `scale` (row-major, owned by the handle, valid until cs_destroy), so that
+ * a collective can sum the tables of several GPUs IN PLACE (ncclAllReduce(int32, sum) on this buffer: PAPER.md:578,
+ * SURVEY 8.e) instead of copying them out and adding them back.  The caller orders its accesses after the handle's
+ * stream (cs_set_stream) and must not touch the buffer while a cs_update* / cs_scan* call is in flight. */
+int cs_table_ptr(cs_sketch* s, int scale, int32_t** table_dev_out);
+
+/* Phase timing.  cs_set_timing(s, 1) makes the handle record CUDA events on its stream between the launches of its
+ * kernel classes (one event per class change: no synchronisation, microseconds of host time); cs_get_timing synchronises
+ * the stream, writes ms_out[p] = device time spent in phase p since the last call and spans_out[p] (may be NULL) = number
+ * of launch groups it was measured over, and forgets them.  Phases: 0 update scatter (k_bin_scatter, or k_update in
+ * direct mode), 1 update apply (k_bin_apply), 2 sampling compaction (k_compact_kept), 3 first scan stage / one-kernel
+ * scans, 4 later scan stages, 5 bitmap builds, 6 selection (sort + unique + cut), 7 unused. */
+#define CS_N_PHASES 8
+int cs_set_timing(cs_sketch* s, int on);
+int cs_get_timing(cs_sketch* s, double* ms_out, uint64_t* spans_out);
+
+/* Routes the counter updates of the binned cs_update took since the last call (then zeroed): out4[0] = applied with
+ * red.global because a shared-memory staging buffer was full, out4[1] = because a bin region was full (both only on
+ * heavily duplicated streams), out4[2] = leftovers of partial staging buffers at kernel end, out4[3] = written as
+ * binned records.  Synchronises. */
+int cs_update_stats(cs_sketch* s, uint64_t* out4_host);
+
 /* Number of kernels this handle has launched since create (bench.py's gpu_launches). */
 int cs_launch_count(cs_sketch* s, uint64_t* n_out);
 

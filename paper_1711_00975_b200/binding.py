@@ -61,6 +61,10 @@ SIGNATURES = {
     "cs_sketch_read": (ci, [vp, ci, vp]),
     "cs_sketch_add": (ci, [vp, ci, vp]),
     "cs_coeffs": (ci, [vp, ci, vp, vp]),
+    "cs_table_ptr": (ci, [vp, ci, vp]),
+    "cs_set_timing": (ci, [vp, ci]),
+    "cs_get_timing": (ci, [vp, vp, vp]),
+    "cs_update_stats": (ci, [vp, vp]),
     "cs_launch_count": (ci, [vp, vp]),
     "cs_probe_l2": (ci, [ci, u64, u64, ci, vp, vp]),
     "cs_probe_stream": (ci, [vp, u64, ci, vp, vp]),
@@ -330,12 +334,39 @@ class CountSketch:
             raise ValueError("table must be a contiguous int32 tensor with d*w entries")
         _chk(lib().cs_sketch_add(self._h, scale, vp(table.data_ptr())), "cs_sketch_add")
 
+    def table_view(self, scale: int = 0) -> torch.Tensor:
+        """(d, w) int32 tensor ALIASING the handle's counters (no copy): for in-place collectives over the table."""
+        ptr = vp(None)
+        _chk(lib().cs_table_ptr(self._h, scale, C.byref(ptr)), "cs_table_ptr")
+
+        class _Alias:
+            __cuda_array_interface__ = {"shape": (self.d, self.w), "typestr": "<i4", "data": (int(ptr.value), False),
+                                        "version": 3, "strides": None}
+        return torch.as_tensor(_Alias(), device=self.device)
+
     def coeffs(self, scale: int = 0):
         import numpy as np
         out = np.empty(4 * self.d, dtype=np.uint64)
         K = u64(0)
         _chk(lib().cs_coeffs(self._h, scale, out.ctypes.data_as(vp), C.byref(K)), "cs_coeffs")
         return out.reshape(self.d, 4), int(K.value)
+
+    PHASES = ("update_scatter", "update_apply", "compact_kept", "scan_first", "scan_next", "bitmap", "select", "other")
+
+    def set_timing(self, on: bool):
+        _chk(lib().cs_set_timing(self._h, int(on)), "cs_set_timing")
+
+    def get_timing(self) -> dict:
+        """{phase: (ms, launch groups)} since the last call."""
+        ms = (dbl * 8)()
+        sp = (u64 * 8)()
+        _chk(lib().cs_get_timing(self._h, ms, sp), "cs_get_timing")
+        return {n: (float(ms[i]), int(sp[i])) for i, n in enumerate(self.PHASES)}
+
+    def update_stats(self) -> dict:
+        out = (u64 * 4)()
+        _chk(lib().cs_update_stats(self._h, out), "cs_update_stats")
+        return {"staging_overflow": int(out[0]), "region_overflow": int(out[1]), "leftover": int(out[2]), "binned": int(out[3])}
 
     def launch_count(self) -> int:
         v = u64(0)

@@ -121,6 +121,8 @@ struct cs_sketch {
     uint16_t* bins = nullptr;          /* record regions */
     uint64_t bins_records = 0;         /* capacity of `bins` in records */
     uint32_t* cursor = nullptr;        /* BIN_MAX words */
+    unsigned long long* bin_stats = nullptr;   /* 4 device counters of the binned route (cs_update_stats) */
+    PhaseTimer tm;                     /* cs_set_timing / cs_get_timing */
 
     /* bitmap prefilter of the scan (cs_scan_bitmap.cu): B[j][b] = |T[j][b]| >= tau_bm, per scale */
     int scan_mode = 0;                 /* cs_set_scan_mode: 0 auto, 1 plain, 2 bitmap, 3 bitmap first stage */
@@ -257,8 +259,10 @@ int read_states(cs_sketch* s) {
  * other half of its ping-pong buffers: the caller reads the states back (read_states) before it uses s->cur again. */
 int compact_scale(cs_sketch* s, int i) {
     const uint32_t n = s->st_host[i].count < s->cap ? s->st_host[i].count : s->cap;
+    s->tm.mark(PH_SELECT, s->stream);
     cudaError_t e = select_compact(s->sb[i], s->cap, s->cur[i], n, s->id_bits[i], s->st_dev + i, s->k_max, s->thr_min, s->stream,
                                    &s->launches, &s->epoch[i]);
+    s->tm.stop(s->stream);
     if (e != cudaSuccess) return fail(CS_ERR_CUDA, "select_compact: %s", cudaGetErrorString(e));
     s->dirty[i] = false;
     s->n_compactions[i] += 1;
@@ -356,6 +360,10 @@ int update_binned(cs_sketch* s, const BinPlan& pl, const float* xyz, uint64_t n,
     cap = (cap + 31) & ~(uint64_t)31;
     const uint64_t need = cap * each * pl.SL;
     if (!s->cursor) CS_CUDA(cudaMalloc(&s->cursor, BIN_MAX * sizeof(uint32_t)));
+    if (!s->bin_stats) {
+        CS_CUDA(cudaMalloc(&s->bin_stats, 4 * sizeof(unsigned long long)));
+        CS_CUDA(cudaMemsetAsync(s->bin_stats, 0, 4 * sizeof(unsigned long long), s->stream));
+    }
     if (s->bins_records < need) {
         CS_CUDA(cudaStreamSynchronize(s->stream));
         if (s->bins) cudaFree(s->bins);
@@ -380,8 +388,10 @@ int update_binned(cs_sketch* s, const BinPlan& pl, const float* xyz, uint64_t n,
                 B.rows_direct = pl.rows_direct < nr ? pl.rows_direct : nr;
                 B.nb = (uint32_t)(nr - B.rows_direct) * pl.SL;
                 B.threads = pl.threads; B.C = pl.C; B.log2S = pl.log2S; B.log2w = pl.log2w;
+                B.stats = s->bin_stats;
                 if (B.nb) CS_CUDA(cudaMemsetAsync(s->cursor, 0, B.nb * sizeof(uint32_t), s->stream));
-                cudaError_t e = launch_update_binned(P, B, xyz + 3 * off, m, s->sm_count, s->stream);
+                cudaError_t e = launch_update_binned(P, B, xyz + 3 * off, m, s->sm_count, s->stream, &s->tm);
+                s->tm.stop(s->stream);
                 if (e != cudaSuccess) return fail(CS_ERR_CUDA, "binned update kernels: %s", cudaGetErrorString(e));
                 s->launches += B.nb ? 2 : 1;
             }
@@ -402,7 +412,9 @@ int update_passes_raw(cs_sketch* s, const float* xyz, uint64_t n, uint64_t index
     const uint64_t row_bytes = s->w * sizeof(int32_t);
     const uint64_t all_bytes = row_bytes * s->d * s->n_scales;
     if (all_bytes <= s->table_budget) {
+        s->tm.mark(PH_SCATTER, s->stream);
         cudaError_t e = launch_update(full, xyz, n, s->sm_count, s->stream);
+        s->tm.stop(s->stream);
         if (e != cudaSuccess) return fail(CS_ERR_CUDA, "update kernel: %s", cudaGetErrorString(e));
         s->launches += 1;
         return CS_OK;
@@ -421,7 +433,9 @@ int update_passes_raw(cs_sketch* s, const float* xyz, uint64_t n, uint64_t index
                 P.sc[i] = full.sc[s0 + i];
                 for (int j = 0; j < s->d; ++j) P.rows[i * s->d + j] = full.rows[(s0 + i) * s->d + j];
             }
+            s->tm.mark(PH_SCATTER, s->stream);
             cudaError_t e = launch_update(P, xyz, n, s->sm_count, s->stream);
+            s->tm.stop(s->stream);
             if (e != cudaSuccess) return fail(CS_ERR_CUDA, "update kernel: %s", cudaGetErrorString(e));
             s->launches += 1;
         }
@@ -438,7 +452,9 @@ int update_passes_raw(cs_sketch* s, const float* xyz, uint64_t n, uint64_t index
             P.sc[0] = full.sc[i];
             P.sc[0].T = full.sc[i].T + (uint64_t)j0 * s->w;
             for (int j = 0; j < nr; ++j) P.rows[j] = full.rows[i * s->d + j0 + j];
+            s->tm.mark(PH_SCATTER, s->stream);
             cudaError_t e = launch_update(P, xyz, n, s->sm_count, s->stream);
+            s->tm.stop(s->stream);
             if (e != cudaSuccess) return fail(CS_ERR_CUDA, "update kernel: %s", cudaGetErrorString(e));
             s->launches += 1;
         }
@@ -492,7 +508,9 @@ int launch_scan_chunk(cs_sketch* s, const float* xyz, uint64_t n, uint64_t index
         for (int i = 0; i < s->n_scales; ++i) {
             if (!s->bm[i]) CS_CUDA(cudaMalloc(&s->bm[i], ((counters + 31) / 32) * sizeof(uint32_t)));
             if (!s->bm_valid[i] || s->tau_bm[i] != s->st_host[i].tau) {
+                s->tm.mark(PH_BITMAP, s->stream);
                 cudaError_t eb = launch_build_bitmap(s->T[i], counters, s->st_host[i].tau, s->bm[i], s->stream);
+                s->tm.stop(s->stream);
                 if (eb != cudaSuccess) return fail(CS_ERR_CUDA, "bitmap kernel: %s", cudaGetErrorString(eb));
                 s->launches += 1;
                 s->tau_bm[i] = s->st_host[i].tau;
@@ -510,12 +528,15 @@ int launch_scan_chunk(cs_sketch* s, const float* xyz, uint64_t n, uint64_t index
                 rebuilt = true;
             }
             cudaError_t ec = launch_scan_staged_cb(full, S.tg[0], s->stb, s->bm[0], s->coarse, cg, crw, rebuilt, xyz, n,
-                                                   s->sm_count, s->stream, &s->launches);
+                                                   s->sm_count, s->stream, &s->launches, &s->tm);
+            s->tm.stop(s->stream);
             if (ec != cudaSuccess) return fail(CS_ERR_CUDA, "bitmap stage kernels: %s", cudaGetErrorString(ec));
             s->n_scan_launches += 1;
             return CS_OK;
         }
+        s->tm.mark(PH_SCAN_FIRST, s->stream);
         cudaError_t eb = launch_scan_bitmap(full, S, s->bm, xyz, n, s->sm_count, s->stream);
+        s->tm.stop(s->stream);
         if (eb != cudaSuccess) return fail(CS_ERR_CUDA, "bitmap scan kernel: %s", cudaGetErrorString(eb));
         s->launches += 1;
         s->n_scan_launches += 1;
@@ -525,7 +546,9 @@ int launch_scan_chunk(cs_sketch* s, const float* xyz, uint64_t n, uint64_t index
     const uint64_t scale_bytes = row_bytes * s->d;
     cudaError_t e = cudaSuccess;
     if (scale_bytes * s->n_scales <= s->table_budget) {
+        s->tm.mark(PH_SCAN_FIRST, s->stream);
         e = launch_scan(full, S, xyz, n, s->sm_count, s->stream);
+        s->tm.stop(s->stream);
         s->launches += 1;
     } else {
         for (int i = 0; i < s->n_scales && e == cudaSuccess; ++i) {
@@ -536,14 +559,17 @@ int launch_scan_chunk(cs_sketch* s, const float* xyz, uint64_t n, uint64_t index
             if (scale_bytes <= s->table_budget) {
                 ScanParams S1 = {};
                 S1.tg[0] = S.tg[i];
+                s->tm.mark(PH_SCAN_FIRST, s->stream);
                 e = launch_scan(P, S1, xyz, n, s->sm_count, s->stream);
+                s->tm.stop(s->stream);
                 s->launches += 1;
             } else {
                 int rc = ensure_stage_lists(s, n);
                 if (rc) return rc;
                 uint64_t fit = s->table_budget / row_bytes;
                 if (fit < 1) fit = 1;
-                e = launch_scan_staged(P, S.tg[i], s->stb, (int)(fit > 8 ? 8 : fit), xyz, n, s->stream, &s->launches);
+                e = launch_scan_staged(P, S.tg[i], s->stb, (int)(fit > 8 ? 8 : fit), xyz, n, s->stream, &s->launches, &s->tm);
+                s->tm.stop(s->stream);
             }
         }
     }
@@ -678,8 +704,10 @@ constexpr uint64_t COMPACT_MIN_N = 1ull << 20;
 int compact_chunk(cs_sketch* s, const float* xyz, uint64_t m, uint64_t index0, double sample_p, float* dst, uint64_t cap,
                   uint64_t* cnt) {
     CS_CUDA(cudaMemsetAsync(s->word_dev, 0, 4, s->stream));
+    s->tm.mark(PH_COMPACT, s->stream);
     cudaError_t e = launch_compact_kept(xyz, m, index0, s->K, sample_threshold(sample_p), dst, s->word_dev,
                                         (uint32_t)(cap < 0xFFFFFFFFull ? cap : 0xFFFFFFFFull), s->sm_count, s->stream);
+    s->tm.stop(s->stream);
     if (e != cudaSuccess) return fail(CS_ERR_CUDA, "compaction kernel: %s", cudaGetErrorString(e));
     s->launches += 1;
     CS_CUDA(cudaMemcpyAsync(s->word_host, s->word_dev, 4, cudaMemcpyDeviceToHost, s->stream));
@@ -1122,6 +1150,8 @@ int cs_destroy(cs_sketch* s) {
     free_stage_lists(s);
     if (s->bins) cudaFree(s->bins);
     if (s->cursor) cudaFree(s->cursor);
+    if (s->bin_stats) cudaFree(s->bin_stats);
+    s->tm.destroy();
     if (s->kept) cudaFree(s->kept);
     if (s->unpacked) cudaFree(s->unpacked);
     for (int i = 0; i < CS_MAX_SCALES; ++i) if (s->bm[i]) cudaFree(s->bm[i]);
@@ -1646,11 +1676,54 @@ int cs_sketch_add(cs_sketch* s, int scale, const int32_t* in_d_by_w) {
     return CS_OK;
 }
 
+int cs_table_ptr(cs_sketch* s, int scale, int32_t** table_dev_out) {
+    if (!s || !table_dev_out) return fail(CS_ERR_ARG, "null argument");
+    if (scale < 0 || scale >= s->n_scales) return fail(CS_ERR_ARG, "scale out of range");
+    *table_dev_out = s->T[scale];
+    return CS_OK;
+}
+
 int cs_coeffs(cs_sketch* s, int scale, uint64_t* out_4d_host, uint64_t* K_out_host) {
     if (!s || !out_4d_host) return fail(CS_ERR_ARG, "null argument");
     if (scale < 0 || scale >= s->n_scales) return fail(CS_ERR_ARG, "scale out of range");
     memcpy(out_4d_host, s->coef[scale], sizeof(uint64_t) * 4 * s->d);
     if (K_out_host) *K_out_host = s->K;
+    return CS_OK;
+}
+
+int cs_set_timing(cs_sketch* s, int on) {
+    CS_ENTER(s);
+    CS_CUDA(cudaStreamSynchronize(s->stream));
+    s->tm.clear();
+    s->tm.on = on != 0;
+    return CS_OK;
+}
+
+int cs_get_timing(cs_sketch* s, double* ms_out, uint64_t* spans_out) {
+    CS_ENTER(s);
+    if (!ms_out) return fail(CS_ERR_ARG, "null output");
+    CS_CUDA(cudaStreamSynchronize(s->stream));
+    for (int p = 0; p < CS_N_PHASES; ++p) { ms_out[p] = 0.0; if (spans_out) spans_out[p] = 0; }
+    for (const PhaseTimer::Span& sp : s->tm.spans) {
+        float ms = 0.f;
+        CS_CUDA(cudaEventElapsedTime(&ms, s->tm.pool[sp.a], s->tm.pool[sp.b]));
+        ms_out[sp.phase] += ms;
+        if (spans_out) spans_out[sp.phase] += 1;
+    }
+    s->tm.clear();
+    return CS_OK;
+}
+
+int cs_update_stats(cs_sketch* s, uint64_t* out4_host) {
+    CS_ENTER(s);
+    if (!out4_host) return fail(CS_ERR_ARG, "null output");
+    for (int i = 0; i < 4; ++i) out4_host[i] = 0;
+    if (!s->bin_stats) return CS_OK;
+    unsigned long long v[4];
+    CS_CUDA(cudaMemcpyAsync(v, s->bin_stats, sizeof(v), cudaMemcpyDeviceToHost, s->stream));
+    CS_CUDA(cudaStreamSynchronize(s->stream));
+    CS_CUDA(cudaMemsetAsync(s->bin_stats, 0, sizeof(v), s->stream));
+    for (int i = 0; i < 4; ++i) out4_host[i] = v[i];
     return CS_OK;
 }
 

@@ -8,10 +8,49 @@
 #include <cuda_runtime.h>
 #include <stdint.h>
 
+#include <vector>
+
 #include "../../include/cs.h"
 #include "cs_hash.h"
 
 namespace cs {
+
+/* Phase timing (cs_set_timing / cs_get_timing): CUDA events recorded on the handle's stream between the launches of
+ * the kernel classes below; mark(p) closes the running span and opens one of phase p, stop() closes it.  Off: no-ops. */
+enum Phase { PH_SCATTER = 0, PH_APPLY, PH_COMPACT, PH_SCAN_FIRST, PH_SCAN_NEXT, PH_BITMAP, PH_SELECT, PH_OTHER, PH_COUNT };
+struct PhaseTimer {
+    bool on = false;
+    std::vector<cudaEvent_t> pool;
+    size_t used = 0;
+    struct Span { int phase; size_t a, b; };
+    std::vector<Span> spans;
+    int open_phase = -1;
+    size_t open_ev = 0;
+    size_t record(cudaStream_t st) {
+        if (used == pool.size()) {
+            cudaEvent_t e;
+            cudaEventCreate(&e);
+            pool.push_back(e);
+        }
+        cudaEventRecord(pool[used], st);
+        return used++;
+    }
+    void mark(int phase, cudaStream_t st) {
+        if (!on) return;
+        const size_t e = record(st);
+        if (open_phase >= 0) spans.push_back({open_phase, open_ev, e});
+        open_phase = phase;
+        open_ev = e;
+    }
+    void stop(cudaStream_t st) {
+        if (!on || open_phase < 0) return;
+        const size_t e = record(st);
+        spans.push_back({open_phase, open_ev, e});
+        open_phase = -1;
+    }
+    void clear() { spans.clear(); used = 0; open_phase = -1; }
+    void destroy() { for (cudaEvent_t e : pool) cudaEventDestroy(e); pool.clear(); clear(); }
+};
 
 constexpr uint64_t GAMMA = 0x9E3779B97F4A7C15ULL;     // splitmix64 increment
 
@@ -78,11 +117,13 @@ struct BinParams {
     uint32_t log2S;       // <= 15
     uint32_t log2w;
     int32_t rows_direct;  // the first rows_direct rows of the pass use red.global instead of the bins
+    unsigned long long* stats;  // 4 counters (may be NULL): records that left the binned route -- [0] staging buffer full,
+                                // [1] bin region full, [2] leftovers of partial buffers at kernel end; [3] records binned
 };
 constexpr int SCATTER_PAIRS_PER_ROUND = 5;      // pairs of particles per thread between two flush phases of k_bin_scatter
 size_t scatter_smem_bytes(uint32_t nb, uint32_t C);
 cudaError_t launch_update_binned(const PassParams& P, const BinParams& B, const float* xyz, uint64_t n, int sm_count,
-                                 cudaStream_t st);
+                                 cudaStream_t st, PhaseTimer* tm);
 
 /* kernel launchers (cs_kernels.cu) */
 cudaError_t launch_pack_records(const float* xyz, uint64_t n, float qscale21, uint64_t* recs, cudaStream_t st);
@@ -105,11 +146,11 @@ struct StageBuffers {
 };
 uint64_t staged_list_entries(uint64_t n, uint32_t blocks);
 cudaError_t launch_scan_staged(const PassParams& P, const ScanTarget& tg, const StageBuffers& B, int rows_per_stage,
-                               const float* xyz, uint64_t n, cudaStream_t st, uint64_t* launches);
+                               const float* xyz, uint64_t n, cudaStream_t st, uint64_t* launches, PhaseTimer* tm);
 bool coarse_shape(int d, int rank, uint64_t w, uint32_t* g_out, uint32_t* row_words_out);
 cudaError_t launch_scan_staged_cb(const PassParams& P, const ScanTarget& tg, const StageBuffers& B, const uint32_t* fine,
                                   uint32_t* coarse, uint32_t g, uint32_t row_words, bool rebuild_coarse, const float* xyz,
-                                  uint64_t n, int sm_count, cudaStream_t st, uint64_t* launches);
+                                  uint64_t n, int sm_count, cudaStream_t st, uint64_t* launches, PhaseTimer* tm);
 cudaError_t launch_scan_cells(const PassParams& P, const ScanParams& S, int scale, const uint64_t* cells,
                               uint64_t m, cudaStream_t st);
 cudaError_t launch_scan_range(const PassParams& P, const ScanParams& S, int scale, uint64_t first, uint64_t m,

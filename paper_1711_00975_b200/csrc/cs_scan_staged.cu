@@ -357,7 +357,7 @@ uint64_t staged_list_entries(uint64_t n, uint32_t blocks) {
 
 /* P: PassParams of ONE scale (n_scales = 1, rows[0..d), d = all its rows).  rows_per_stage in [1, 8]. */
 cudaError_t launch_scan_staged(const PassParams& P, const ScanTarget& tg, const StageBuffers& B, int rows_per_stage,
-                               const float* xyz, uint64_t n, cudaStream_t st, uint64_t* launches) {
+                               const float* xyz, uint64_t n, cudaStream_t st, uint64_t* launches, PhaseTimer* tm) {
     uint32_t head;
     uint64_t groups;
     split_aligned(xyz, n, &head, &groups);
@@ -383,6 +383,7 @@ cudaError_t launch_scan_staged(const PassParams& P, const ScanTarget& tg, const 
         Q.row0 = row0;
         Q.d_all = P.d;
         Q.pad = 0;
+        if (tm) tm->mark(i == 0 ? PH_SCAN_FIRST : PH_SCAN_NEXT, st);
         if (pow2) {
             if (last) launch_stage_r<true, true>(R, i == 0, blocks, P, Q, tg, xyz, n, head, groups, gpb, st);
             else      launch_stage_r<true, false>(R, i == 0, blocks, P, Q, tg, xyz, n, head, groups, gpb, st);
@@ -435,9 +436,10 @@ bool coarse_shape(int d, int rank, uint64_t w, uint32_t* g_out, uint32_t* row_wo
 /* fine: bitmap of the scale (bit j*w + b), already built for the current tau; coarse: scratch of FIRST*row_words words */
 cudaError_t launch_scan_staged_cb(const PassParams& P, const ScanTarget& tg, const StageBuffers& B, const uint32_t* fine,
                                   uint32_t* coarse, uint32_t g, uint32_t row_words, bool rebuild_coarse, const float* xyz,
-                                  uint64_t n, int sm_count, cudaStream_t st, uint64_t* launches) {
+                                  uint64_t n, int sm_count, cudaStream_t st, uint64_t* launches, PhaseTimer* tm) {
     const int first = P.rank + 1, rest = P.d - first;
     if (rebuild_coarse) {
+        if (tm) tm->mark(PH_BITMAP, st);
         const uint64_t words = (uint64_t)first * row_words;
         uint64_t blocks = (words + 255) / 256;
         if (blocks > 148 * 8) blocks = 148 * 8;
@@ -460,6 +462,7 @@ cudaError_t launch_scan_staged_cb(const PassParams& P, const ScanTarget& tg, con
     C.big = P.sc[0].big;
     const size_t smem = (size_t)first * row_words * 4;
     cudaError_t e = cudaSuccess;
+    if (tm) tm->mark(PH_SCAN_FIRST, st);
 #define CS_CB(F)                                                                                              \
     case F:                                                                                                   \
         e = cudaFuncSetAttribute(k_stage_first_cb<F>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem); \
@@ -474,6 +477,7 @@ cudaError_t launch_scan_staged_cb(const PassParams& P, const ScanTarget& tg, con
     Q2.in = B.list[0]; Q2.cnt_in = B.cnt[0];
     Q2.out = B.list[1]; Q2.cnt_out = B.cnt[1];
     Q2.row0 = first;
+    if (tm) tm->mark(PH_SCAN_NEXT, st);
     launch_stage_r<true, true>(rest, false, blocks, P, Q2, tg, xyz, n, head, groups, gpb, st);
     *launches += 1;
     return cudaGetLastError();

@@ -76,6 +76,7 @@ struct InsertCtx {
     uint32_t log2S, smask; // slice shift, (1 << log2S) - 1
     uint32_t log2w, wmask;
     int32_t rows_direct;
+    uint32_t stat_addr;    // shared address of the CTA's 4 route counters (BinParams::stats)
 };
 
 /* BIG: cell ids of the mesh can exceed 2^31 (two-limb form of cs_hash.h). */
@@ -117,7 +118,10 @@ __device__ __forceinline__ void bin_particle(const PassParams& P, const InsertCt
         if (slot < X.C) sts_u16(X.buf_addr + bin * X.C2 + slot * 2u, ((key & X.smask) << 1) + sb);
         else            ovf |= 1u << j;                                 // staging buffer full
     }
-    if (ovf) apply_rows_direct(P, X.wmask, c0, c1, ovf);
+    if (ovf) {
+        asm volatile("red.shared.add.u32 [%0], %1;" :: "r"(X.stat_addr), "r"((uint32_t)__popc(ovf)) : "memory");
+        apply_rows_direct(P, X.wmask, c0, c1, ovf);
+    }
 }
 
 /* Particles [head, head + 2*pairs) are read as pairs (3 x 8 B per thread, 8-byte aligned); the <= 1 particle
@@ -128,6 +132,8 @@ __global__ void __launch_bounds__(BIN_THREADS, 1)
 k_bin_scatter(const __grid_constant__ PassParams P, const __grid_constant__ BinParams B,
               const float* __restrict__ xyz, uint64_t n, uint32_t head, uint64_t pairs) {
     extern __shared__ __align__(16) unsigned char smem_raw[];
+    __shared__ uint32_t s_stat[4];
+    if (threadIdx.x < 4) s_stat[threadIdx.x] = 0;
     const uint32_t NT = blockDim.x;                                  // 512 or 1024
     uint32_t* cnt = reinterpret_cast<uint32_t*>(smem_raw);
     uint32_t* qlen = cnt + B.nb;
@@ -143,6 +149,7 @@ k_bin_scatter(const __grid_constant__ PassParams P, const __grid_constant__ BinP
     X.log2S = B.log2S; X.smask = (1u << B.log2S) - 1u;
     X.log2w = B.log2w; X.wmask = (uint32_t)(P.w - 1);
     X.rows_direct = B.rows_direct;
+    X.stat_addr = (uint32_t)__cvta_generic_to_shared(s_stat);
 
     const float2* body = reinterpret_cast<const float2*>(xyz + 3 * (uint64_t)head);
     const uint64_t per_sub = (uint64_t)gridDim.x * NT;                 // pairs of one sub-round over the grid
@@ -190,7 +197,10 @@ k_bin_scatter(const __grid_constant__ PassParams P, const __grid_constant__ BinP
                 bin = queue[e];
                 c = min(cnt[bin], B.C);
                 units = c / UNIT;
-                if (l4 == 0) base = atomicAdd(&B.cursor[bin], units * UNIT);
+                if (l4 == 0) {
+                    base = atomicAdd(&B.cursor[bin], units * UNIT);
+                    atomicAdd(&s_stat[3], units * UNIT);
+                }
             }
             base = __shfl_sync(0xFFFFFFFFu, base, grp * 4);
             if (on) {
@@ -201,6 +211,8 @@ k_bin_scatter(const __grid_constant__ PassParams P, const __grid_constant__ BinP
                     if (at + UNIT <= B.cap) {
                         st_stream16u(reinterpret_cast<uint4*>(B.bins + (uint64_t)bin * B.cap + at + l4 * 8), v);
                     } else {                                           // bin region full: apply directly
+                        atomicAdd(&s_stat[1], 8u);
+                        if (l4 == 0) atomicSub(&s_stat[3], UNIT);
                         const uint32_t wds[4] = {v.x, v.y, v.z, v.w};
 #pragma unroll
                         for (int k = 0; k < 4; ++k) {
@@ -223,7 +235,10 @@ k_bin_scatter(const __grid_constant__ PassParams P, const __grid_constant__ BinP
     for (uint32_t bin = threadIdx.x; bin < B.nb; bin += NT) {
         const uint32_t c = min(cnt[bin], B.C);
         for (uint32_t i = 0; i < c; ++i) apply_direct(T, bin, B.log2S, buf[bin * B.C + i]);
+        if (c) atomicAdd(&s_stat[2], c);
     }
+    __syncthreads();
+    if (threadIdx.x < 4 && B.stats && s_stat[threadIdx.x]) atomicAdd(&B.stats[threadIdx.x], (unsigned long long)s_stat[threadIdx.x]);
     if (blockIdx.x == 0 && threadIdx.x < 2) {
         const uint64_t tail0 = (uint64_t)head + 2 * pairs;
         uint64_t i = ~0ull;
@@ -292,8 +307,9 @@ static cudaError_t launch_scatter_r(const PassParams& P, const BinParams& B, con
 /* P: PassParams of ONE scale restricted to the R = P.d rows of this pass (rows[0..R), sc[0].T = first row).
  * The caller has zeroed B.cursor[0..nb) on the stream.  Launches scatter + apply. */
 cudaError_t launch_update_binned(const PassParams& P, const BinParams& B, const float* xyz, uint64_t n, int sm_count,
-                                 cudaStream_t st) {
+                                 cudaStream_t st, PhaseTimer* tm) {
     cudaError_t e;
+    if (tm) tm->mark(PH_SCATTER, st);
     switch (P.d) {
         case 1: e = launch_scatter_r<1>(P, B, xyz, n, sm_count, st); break;
         case 2: e = launch_scatter_r<2>(P, B, xyz, n, sm_count, st); break;
@@ -307,6 +323,7 @@ cudaError_t launch_update_binned(const PassParams& P, const BinParams& B, const 
     }
     if (e != cudaSuccess) return e;
     if (B.nb == 0) return cudaSuccess;                                       // every row of the pass is direct
+    if (tm) tm->mark(PH_APPLY, st);
     const size_t smem = (size_t)4 << B.log2S;
     e = cudaFuncSetAttribute(k_bin_apply, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
     if (e != cudaSuccess) return e;

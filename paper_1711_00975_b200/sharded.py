@@ -29,12 +29,19 @@ def shard_bounds(n_total: int, rank: int, world: int, align: int = 4):
 
 
 def merge_tables(engine, dist) -> None:
-    """T <- sum over ranks of T (one all-reduce per scale), applied as T += (total - own)."""
+    """T <- sum over ranks of T: one all-reduce per scale, IN PLACE on the engine's own table when it exposes it
+    (binding.CountSketch.table_view: no table-sized temporaries); engines without a view (the CPU test adapter) fall
+    back to read + all-reduce + add of the difference."""
     for s in range(engine.n_scales):
+        view = engine.table_view(s) if hasattr(engine, "table_view") else None
+        if view is not None:
+            dist.all_reduce(view, op=dist.ReduceOp.SUM)
+            continue
         own = engine.sketch(s)
         total = own.clone()
         dist.all_reduce(total, op=dist.ReduceOp.SUM)
-        engine.sketch_add((total - own).contiguous(), s)
+        total -= own
+        engine.sketch_add(total, s)
 
 
 def merge_topk(engine, k: int, dist, world: int):
@@ -52,7 +59,7 @@ def merge_topk(engine, k: int, dist, world: int):
 
 
 def sharded_pass(engine, xyz_shard, index0: int, sample_p: float, k: int, thr_min: int, dist=None, world: int = 1,
-                 update=None, scan=None, topk_device=None):
+                 update=None, scan=None, topk_device=None, force_merge: bool = False):
     """reset -> update(shard) -> [all-reduce tables] -> re-scan(shard) -> [merge top-k]; returns per-scale (ids, est).
 
     `update` / `scan` override the engine methods used for the two passes (the host-streamed variants);
@@ -60,12 +67,13 @@ def sharded_pass(engine, xyz_shard, index0: int, sample_p: float, k: int, thr_mi
     engine.reset()
     engine.set_update_index(index0)
     (update or engine.update)(xyz_shard, sample_p)
-    if world > 1:
+    merge = world > 1 or (force_merge and dist is not None)     # force_merge: run the exchange steps on a 1-rank group
+    if merge:
         merge_tables(engine, dist)
     engine.scan_begin(k, thr_min)
     engine.set_scan_index(index0)
     (scan or engine.scan)(xyz_shard, sample_p)
-    if world > 1:
+    if merge:
         return merge_topk(engine, k, dist, world)
     if topk_device is not None:
         return [engine.topk(k, s, device=topk_device) for s in range(engine.n_scales)]
