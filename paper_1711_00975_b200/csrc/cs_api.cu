@@ -98,6 +98,10 @@ struct cs_sketch {
     uint32_t cap = 0;
     uint32_t cap_min = MIN_CAP;        /* cs_set_candidate_capacity */
     SelectBuffers sb[CS_MAX_SCALES] = {};
+    unsigned long long* seen[CS_MAX_SCALES] = {};   /* duplicate filter of the re-scan (cs_scan_common.cuh), per scale */
+    uint64_t seen_slots = 0;
+    bool use_seen[CS_MAX_SCALES] = {};    /* switched on per scale once a compaction finds the list heavily duplicated */
+    uint32_t compact_n[CS_MAX_SCALES] = {};   /* entries the compaction in flight started from (0: none in flight) */
     int cur[CS_MAX_SCALES] = {};
     bool dirty[CS_MAX_SCALES] = {};
     uint32_t last_compact[CS_MAX_SCALES] = {};
@@ -203,7 +207,10 @@ void free_candidates(cs_sketch* s) {
         }
         if (s->sb[i].scratch) cudaFree(s->sb[i].scratch);
         s->sb[i].scratch = nullptr;
+        if (s->seen[i]) cudaFree(s->seen[i]);
+        s->seen[i] = nullptr;
     }
+    s->seen_slots = 0;
     s->cap = 0;
 }
 
@@ -218,7 +225,19 @@ int alloc_candidates(cs_sketch* s, uint32_t cap) {
         CS_CUDA(cudaMemsetAsync(s->sb[i].scratch, 0, (size_t)select_scratch_words(cap) * sizeof(uint32_t), s->stream));
         s->cur[i] = 0;
     }
+    /* duplicate filter of the re-scan: 2 slots per list entry, at most 2^25 slots (256 MiB) per scale */
+    uint64_t slots = 2 * (uint64_t)cap;
+    if (slots > (1ull << 25)) slots = 1ull << 25;
+    for (int i = 0; i < s->n_scales; ++i) CS_CUDA(cudaMalloc(&s->seen[i], slots * sizeof(unsigned long long)));
+    s->seen_slots = slots;
     s->cap = cap;
+    return CS_OK;
+}
+
+/* Empty the duplicate filters (cs_scan_begin; before a chunk whose entries were dropped is re-run). */
+int clear_seen(cs_sketch* s) {
+    for (int i = 0; i < s->n_scales; ++i)
+        if (s->seen[i]) CS_CUDA(cudaMemsetAsync(s->seen[i], 0xFF, s->seen_slots * sizeof(unsigned long long), s->stream));
     return CS_OK;
 }
 
@@ -251,7 +270,16 @@ int grow_candidates(cs_sketch* s) {
 int read_states(cs_sketch* s) {
     CS_CUDA(cudaMemcpyAsync(s->st_host, s->st_dev, sizeof(ScanState) * s->n_scales, cudaMemcpyDeviceToHost, s->stream));
     CS_CUDA(cudaStreamSynchronize(s->stream));
-    for (int i = 0; i < s->n_scales; ++i) s->cur[i] = (int)(s->st_host[i].half & 1u);   /* compactions move the list */
+    for (int i = 0; i < s->n_scales; ++i) {
+        s->cur[i] = (int)(s->st_host[i].half & 1u);          /* compactions move the list */
+        /* The duplicate filter costs one atomicCAS at a random address per cell that passes the last stage: it pays when
+         * cells arrive many times (coarse meshes, concentrated streams: measured 2x fewer launches at cfg 1), not when
+         * almost every cell holds one particle (cfg 5: +2.4 ms).  Decided from what the last compaction found. */
+        if (s->compact_n[i]) {
+            if (s->compact_n[i] >= 4096 && 2 * (uint64_t)s->compact_n[i] >= 3 * (uint64_t)s->st_host[i].uniq) s->use_seen[i] = true;
+            s->compact_n[i] = 0;
+        }
+    }
     return CS_OK;
 }
 
@@ -266,6 +294,7 @@ int compact_scale(cs_sketch* s, int i) {
     if (e != cudaSuccess) return fail(CS_ERR_CUDA, "select_compact: %s", cudaGetErrorString(e));
     s->dirty[i] = false;
     s->n_compactions[i] += 1;
+    s->compact_n[i] = n;
     return CS_OK;
 }
 
@@ -276,6 +305,8 @@ void fill_scan_params(cs_sketch* s, ScanParams* S) {
         S->tg[i].ek = s->sb[i].ek[s->cur[i]];
         S->tg[i].st = s->st_dev + i;
         S->tg[i].cap = s->cap;
+        S->tg[i].seen = s->seen[i];
+        S->tg[i].seen_mask = (s->seen[i] && s->use_seen[i]) ? (uint32_t)(s->seen_slots - 1) : 0u;
     }
 }
 
@@ -498,8 +529,8 @@ int launch_scan_chunk(cs_sketch* s, const float* xyz, uint64_t n, uint64_t index
     fill_scan_params(s, &S);
     /* bitmap prefilter: valid once every scale collects against a tau >= 1 (|T| >= tau is then necessary for a row
      * to pass); rebuilt (d*w/8 bytes, microseconds) whenever a compaction has raised tau */
-    uint32_t cg0 = 0, crw0 = 0;
-    const bool staged_bm = s->n_scales == 1 && coarse_shape(s->d, s->P.rank, s->w, &cg0, &crw0);
+    CoarseShape cshape;
+    const bool staged_bm = s->n_scales == 1 && coarse_shape(s->d, s->P.rank, s->w, &cshape);
     bool use_bm = (s->scan_mode == 2 || s->scan_mode == 3 || (s->scan_mode == 0 && staged_bm)) && (s->w & (s->w - 1)) == 0;
     for (int i = 0; i < s->n_scales && use_bm; ++i) use_bm = s->st_host[i].tau >= 1;
     if (use_bm) {
@@ -518,16 +549,15 @@ int launch_scan_chunk(cs_sketch* s, const float* xyz, uint64_t n, uint64_t index
                 rebuilt = true;
             }
         }
-        uint32_t cg = 0, crw = 0;
-        if (s->scan_mode != 2 && s->n_scales == 1 && coarse_shape(s->d, s->P.rank, s->w, &cg, &crw)) {
+        if (s->scan_mode != 2 && staged_bm) {
             /* bitmap first stage (coarse bitmap in shared memory) + the remaining rows on dense warps */
             int rc = ensure_stage_lists(s, n);
             if (rc) return rc;
             if (!s->coarse) {
-                CS_CUDA(cudaMalloc(&s->coarse, (size_t)((s->d - 1) / 2 + 1) * crw * sizeof(uint32_t)));
+                CS_CUDA(cudaMalloc(&s->coarse, (size_t)cshape.row_off[s->P.rank + 1] * sizeof(uint32_t)));
                 rebuilt = true;
             }
-            cudaError_t ec = launch_scan_staged_cb(full, S.tg[0], s->stb, s->bm[0], s->coarse, cg, crw, rebuilt, xyz, n,
+            cudaError_t ec = launch_scan_staged_cb(full, S.tg[0], s->stb, s->bm[0], s->coarse, cshape, rebuilt, xyz, n,
                                                    s->sm_count, s->stream, &s->launches, &s->tm);
             s->tm.stop(s->stream);
             if (ec != cudaSuccess) return fail(CS_ERR_CUDA, "bitmap stage kernels: %s", cudaGetErrorString(ec));
@@ -584,8 +614,10 @@ bool wants_compaction(const cs_sketch* s, int i) {
     uint64_t base = s->last_compact[i];
     if (base < s->k_max) base = s->k_max;
     if (base < 8192) base = 8192;
-    /* compacting raises tau (the k_max-th estimate seen so far), which sharpens every later chunk's filter */
-    return s->dirty[i] && (c > s->cap / 2 || 2 * (uint64_t)c >= 3 * base);
+    /* compacting raises tau (the k_max-th estimate seen so far), which sharpens every later chunk's filter -- unless tau
+     * already sits at the excursion limit thr_min, above which it never goes: then only buffer pressure counts */
+    const bool tau_capped = s->thr_min != INT32_MAX && s->st_host[i].tau >= s->thr_min;
+    return s->dirty[i] && (c > s->cap / 2 || (!tau_capped && 2 * (uint64_t)c >= 3 * base));
 }
 
 /* Replay n device-resident particles against the tables, collecting candidates.
@@ -649,7 +681,10 @@ int scan_device_raw(cs_sketch* s, const float* xyz, uint64_t n, double sample_p)
             s->rate = r;
             if (!overflow) break;
             /* Entries past the capacity were dropped: dedupe / cut every list, then re-run this chunk with a
-             * size that cannot overflow.  What the failed run appended is valid and is deduplicated later. */
+             * size that cannot overflow.  What the failed run appended is valid and is deduplicated later.  The
+             * duplicate filter knows the dropped cells as seen: it is emptied first. */
+            rc = clear_seen(s);
+            if (rc) return rc;
             for (int i = 0; i < s->n_scales; ++i) {
                 rc = compact_scale(s, i);
                 if (rc) return rc;
@@ -1388,10 +1423,14 @@ int cs_scan_begin(cs_sketch* s, uint64_t k_max, int32_t thr_min) {
         s->st_host[i].uniq = 0;
         s->st_host[i].half = 0;
         s->cur[i] = 0;
+        s->use_seen[i] = false;
+        s->compact_n[i] = 0;
         s->dirty[i] = false; s->last_compact[i] = 0; s->n_compactions[i] = 0;
     }
     CS_CUDA(cudaMemcpyAsync(s->st_dev, s->st_host, sizeof(ScanState) * s->n_scales, cudaMemcpyHostToDevice, s->stream));
     CS_CUDA(cudaStreamSynchronize(s->stream));
+    int rcs = clear_seen(s);
+    if (rcs) return rcs;
     s->scanning = true;
     return CS_OK;
 }

@@ -83,7 +83,9 @@ struct ScanTarget {
     uint32_t* ek;      // candidate keys: 0x7FFFFFFF - est  (ascending key = descending estimate)
     ScanState* st;
     uint32_t cap;
-    uint32_t pad;
+    uint32_t seen_mask;            // slots - 1 of the seen set (0: no set)
+    unsigned long long* seen;      // open-addressing set of the cells that reached the final check of this scan (see
+                                   // seen_first_time, cs_scan_common.cuh); all-ones = empty slot
 };
 
 /* Everything a pass over particles needs, passed by value as a __grid_constant__ kernel parameter
@@ -147,9 +149,15 @@ struct StageBuffers {
 uint64_t staged_list_entries(uint64_t n, uint32_t blocks);
 cudaError_t launch_scan_staged(const PassParams& P, const ScanTarget& tg, const StageBuffers& B, int rows_per_stage,
                                const float* xyz, uint64_t n, cudaStream_t st, uint64_t* launches, PhaseTimer* tm);
-bool coarse_shape(int d, int rank, uint64_t w, uint32_t* g_out, uint32_t* row_words_out);
+/* Coarse bitmap of the first rank+1 rows held in shared memory by the first scan stage: the first n_fine rows at one bit
+ * per 2^(g-1) counters, the others at one bit per 2^g counters (as fine as 224 KB of shared memory allow). */
+struct CoarseShape {
+    uint32_t g, n_fine;
+    uint32_t row_off[6];       // word offset of row j; row_off[first] = total words
+};
+bool coarse_shape(int d, int rank, uint64_t w, CoarseShape* out);
 cudaError_t launch_scan_staged_cb(const PassParams& P, const ScanTarget& tg, const StageBuffers& B, const uint32_t* fine,
-                                  uint32_t* coarse, uint32_t g, uint32_t row_words, bool rebuild_coarse, const float* xyz,
+                                  uint32_t* coarse, const CoarseShape& shape, bool rebuild_coarse, const float* xyz,
                                   uint64_t n, int sm_count, cudaStream_t st, uint64_t* launches, PhaseTimer* tm);
 cudaError_t launch_scan_cells(const PassParams& P, const ScanParams& S, int scale, const uint64_t* cells,
                               uint64_t m, cudaStream_t st);

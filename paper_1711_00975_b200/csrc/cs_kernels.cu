@@ -117,70 +117,82 @@ cudaError_t launch_update(const PassParams& P, const float* xyz, uint64_t n, int
  * the kept particles in the buffer is arbitrary (Add commutes; candidates are a set).
  * ------------------------------------------------------------------------------------------------------ */
 
-/* One block iteration = 1024 particles: the kept ones are counted per warp, the block reserves its output range
- * with ONE global atomic (a per-warp atomic on the single counter serialises at the L2: 8 M same-address atomics
- * per 2^28 particles), and every lane writes its kept particles at its rank. */
+/* One block iteration = 4096 particles (4 groups of 4 per thread): every thread first evaluates its 16 sampling hashes,
+ * the block reserves its output range with ONE global atomic (a reservation per warp or per 1024 particles serialises at
+ * the L2: same-address atomics), then the groups that hold a kept particle are loaded (3 x 16 B) and the kept particles
+ * written at the thread's offset.  The order of the kept particles in the buffer is arbitrary. */
+constexpr int CK_U = 4;
 __global__ void __launch_bounds__(PASS_THREADS)
 k_compact_kept(const float* __restrict__ xyz, uint64_t n, uint32_t head, uint64_t groups, uint64_t index0, uint64_t K,
                uint64_t Tp, float* __restrict__ out, uint32_t* count, uint32_t cap) {
     __shared__ uint32_t s_warp[PASS_THREADS / 32];
     __shared__ uint32_t s_base;
-    const uint64_t stride = (uint64_t)gridDim.x * PASS_THREADS;
+    const uint64_t per_iter = (uint64_t)PASS_THREADS * CK_U;
+    const uint64_t stride = (uint64_t)gridDim.x * per_iter;
     const float4* body = reinterpret_cast<const float4*>(xyz + 3 * (uint64_t)head);
     const uint32_t lane = threadIdx.x & 31u, warp = threadIdx.x >> 5;
-    const uint32_t below = (1u << lane) - 1u;
     /* block-uniform trip count; block 0 runs one extra iteration for the <= 6 edge particles (thread = particle) */
     const uint64_t iters = (groups + stride - 1) / stride;
     for (uint64_t it = 0; it < iters + (blockIdx.x == 0 ? 1 : 0); ++it) {
         const bool edge = it == iters;
-        float px[4] = {0.f, 0.f, 0.f, 0.f}, py[4] = {0.f, 0.f, 0.f, 0.f}, pz[4] = {0.f, 0.f, 0.f, 0.f};
-        bool k[4] = {false, false, false, false};
+        const uint64_t g0 = it * stride + (uint64_t)blockIdx.x * per_iter + threadIdx.x;
+        uint32_t kbits = 0;                                  // bit 4*u + q: particle q of group g0 + u*PASS_THREADS
+        uint64_t edge_i = 0;
         if (!edge) {
-            const uint64_t g = it * stride + (uint64_t)blockIdx.x * PASS_THREADS + threadIdx.x;
-            if (g < groups) {
-                const uint64_t i0 = index0 + head + 4 * g;
 #pragma unroll
-                for (int q = 0; q < 4; ++q) k[q] = keep_particle(K, i0 + q, Tp);
-                if (k[0] || k[1] || k[2] || k[3]) {       // 48 B are only fetched where something is kept
-                    const float4 q0 = ld_stream16(body + 3 * g), q1 = ld_stream16(body + 3 * g + 1),
-                                 q2 = ld_stream16(body + 3 * g + 2);
-                    px[0] = q0.x; py[0] = q0.y; pz[0] = q0.z;
-                    px[1] = q0.w; py[1] = q1.x; pz[1] = q1.y;
-                    px[2] = q1.z; py[2] = q1.w; pz[2] = q2.x;
-                    px[3] = q2.y; py[3] = q2.z; pz[3] = q2.w;
+            for (int u = 0; u < CK_U; ++u) {
+                const uint64_t g = g0 + (uint64_t)u * PASS_THREADS;
+                if (g < groups) {
+                    const uint64_t i0 = index0 + head + 4 * g;
+#pragma unroll
+                    for (int q = 0; q < 4; ++q) kbits |= (uint32_t)keep_particle(K, i0 + q, Tp) << (4 * u + q);
                 }
             }
         } else {
             const uint64_t tail0 = (uint64_t)head + 4 * groups;
             const uint64_t n_edge = (uint64_t)head + (n - tail0);
             if (threadIdx.x < n_edge) {
-                const uint64_t i = threadIdx.x < head ? threadIdx.x : tail0 + (threadIdx.x - head);
-                k[0] = keep_particle(K, index0 + i, Tp);
-                const float* p = xyz + 3 * i;
-                px[0] = ld_stream4(p); py[0] = ld_stream4(p + 1); pz[0] = ld_stream4(p + 2);
+                edge_i = threadIdx.x < head ? threadIdx.x : tail0 + (threadIdx.x - head);
+                kbits = keep_particle(K, index0 + edge_i, Tp) ? 1u : 0u;
             }
         }
-        uint32_t m[4], tot = 0;
+        const uint32_t c = __popc(kbits);
+        uint32_t incl = c;
 #pragma unroll
-        for (int q = 0; q < 4; ++q) { m[q] = __ballot_sync(0xFFFFFFFFu, k[q]); tot += __popc(m[q]); }
-        if (lane == 0) s_warp[warp] = tot;
+        for (int off = 1; off < 32; off <<= 1) {
+            const uint32_t v = __shfl_up_sync(0xFFFFFFFFu, incl, off);
+            if (lane >= off) incl += v;
+        }
+        if (lane == 31) s_warp[warp] = incl;
         __syncthreads();
         if (threadIdx.x == 0) {
             uint32_t sum = 0;
-            for (int w = 0; w < PASS_THREADS / 32; ++w) { const uint32_t c = s_warp[w]; s_warp[w] = sum; sum += c; }
+            for (int w = 0; w < PASS_THREADS / 32; ++w) { const uint32_t x = s_warp[w]; s_warp[w] = sum; sum += x; }
             s_base = sum ? atomicAdd(count, sum) : 0;
         }
         __syncthreads();
-        uint64_t pos = (uint64_t)s_base + s_warp[warp];
+        uint64_t pos = (uint64_t)s_base + s_warp[warp] + incl - c;
+        if (!edge) {
 #pragma unroll
-        for (int q = 0; q < 4; ++q) {
-            if (k[q]) {
-                const uint64_t at = pos + __popc(m[q] & below);
-                if (at < cap) {                           // *count > cap is reported to the host, which then falls back
-                    out[3 * at] = px[q]; out[3 * at + 1] = py[q]; out[3 * at + 2] = pz[q];
+            for (int u = 0; u < CK_U; ++u) {
+                const uint32_t kb = (kbits >> (4 * u)) & 15u;
+                if (kb) {                                    // 48 B are only fetched where something is kept
+                    const uint64_t g = g0 + (uint64_t)u * PASS_THREADS;
+                    const float4 q0 = ld_stream16(body + 3 * g), q1 = ld_stream16(body + 3 * g + 1),
+                                 q2 = ld_stream16(body + 3 * g + 2);
+                    const float px[4] = {q0.x, q0.w, q1.z, q2.y}, py[4] = {q0.y, q1.x, q1.w, q2.z},
+                                pz[4] = {q0.z, q1.y, q2.x, q2.w};
+#pragma unroll
+                    for (int q = 0; q < 4; ++q)
+                        if (kb & (1u << q)) {
+                            if (pos < cap) { out[3 * pos] = px[q]; out[3 * pos + 1] = py[q]; out[3 * pos + 2] = pz[q]; }
+                            ++pos;                           // *count > cap is reported to the host, which then falls back
+                        }
                 }
             }
-            pos += __popc(m[q]);
+        } else if (kbits) {
+            const float* p = xyz + 3 * edge_i;
+            if (pos < cap) { out[3 * pos] = ld_stream4(p); out[3 * pos + 1] = ld_stream4(p + 1); out[3 * pos + 2] = ld_stream4(p + 2); }
         }
         __syncthreads();                                  // s_warp / s_base are rewritten by the next iteration
     }
@@ -192,7 +204,7 @@ cudaError_t launch_compact_kept(const float* xyz, uint64_t n, uint64_t index0, u
     uint32_t head;
     uint64_t groups;
     split_aligned(xyz, n, &head, &groups);
-    int blocks = blocks_for(k_compact_kept, sm_count, groups);
+    int blocks = blocks_for(k_compact_kept, sm_count, (groups + CK_U - 1) / CK_U);
     k_compact_kept<<<blocks, PASS_THREADS, 0, st>>>(xyz, n, head, groups, index0, K, Tp, out, count, cap);
     return cudaGetLastError();
 }

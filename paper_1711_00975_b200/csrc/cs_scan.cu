@@ -27,6 +27,7 @@ __device__ __forceinline__ void scan_particle(const PassParams& P, const ScanPar
             c = cell_of(x, y, z, P.sc[s]);
             emit = P.sc[s].big ? estimate_ge<D, POW2, true>(P, s, c, tau[s], est)
                                : estimate_ge<D, POW2, false>(P, s, c, tau[s], est);
+            if (emit) emit = seen_first_time(S.tg[s], c);
         }
         append_candidate(S.tg[s], emit, c, est);
     }
@@ -107,7 +108,7 @@ k_scan_cells(const __grid_constant__ PassParams P, const __grid_constant__ ScanP
         if (i < m) {
             c = cells[i];
             e = estimate_any<D, POW2>(P, s, c);
-            emit = e >= tau;
+            emit = e >= tau && seen_first_time(S.tg[s], c);
         }
         append_candidate(S.tg[s], emit, c, e);
     }

@@ -102,7 +102,7 @@ __device__ __forceinline__ void scan_particle_bm(const PassParams& P, const Scan
             const uint32_t c0 = cell_c0(c), c1 = cell_c1(c);
             const bool live = P.sc[s].big ? bitmap_survives<D, true>(P, s, Bm.bm[s], c0, c1)
                                           : bitmap_survives<D, false>(P, s, Bm.bm[s], c0, c1);
-            if (live) {                                  // rare: exact estimate from the counters
+            if (live && seen_first_time(S.tg[s], c)) {   // rare: exact estimate from the counters, once per cell
                 emit = P.sc[s].big ? estimate_ge<D, true, true>(P, s, c, tau[s], est)
                                    : estimate_ge<D, true, false>(P, s, c, tau[s], est);
             }

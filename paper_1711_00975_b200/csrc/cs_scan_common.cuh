@@ -57,6 +57,23 @@ __device__ __forceinline__ int32_t estimate_full(const PassParams& P, int s, uin
     return est;
 }
 
+/* Duplicate filter of the re-scan.  The same cell arrives once per particle it holds (tens of times for the heavy cells
+ * of a coarse mesh), always with the same estimate: only its first arrival needs the exact estimate and a list entry.
+ * The set holds every cell that reached this point since cs_scan_begin -- appended or found below tau, which only rises.
+ * Returns true for the first arrival.  A crowded table (more than 32 probes) answers true: a duplicate entry is
+ * harmless, the selector removes it.  The host clears the set before it re-runs a chunk whose entries were dropped. */
+static __device__ __noinline__ bool seen_first_time(const ScanTarget& tg, uint64_t c) {
+    if (tg.seen_mask == 0 || c == ~0ull) return true;
+    uint32_t s = (uint32_t)(mix64(c) >> 24) & tg.seen_mask;
+    for (int probe = 0; probe < 32; ++probe) {
+        const unsigned long long old = atomicCAS(tg.seen + s, ~0ull, (unsigned long long)c);
+        if (old == ~0ull) return true;
+        if (old == c) return false;
+        s = (s + 1) & tg.seen_mask;
+    }
+    return true;
+}
+
 /* Warp-aggregated append of (c, est) to the candidate list of one scale.  Must be reached by all 32 lanes.
  * One global atomic per warp that has something to append; the estimate range of the list (which bounds the radix
  * passes of the selector) is computed when the list is compacted (k_est_range), not here: three atomics per append on

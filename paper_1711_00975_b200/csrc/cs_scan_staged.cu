@@ -56,18 +56,14 @@ __device__ __noinline__ int32_t estimate_all_rows(const PassParams& P, int d, ui
     return select_rt(v, d, P.rank);
 }
 
-/* One cell through one stage.  Must be reached by all 32 lanes (the appends are warp-aggregated). */
-template <int R, bool POW2, bool LAST>
-__device__ __forceinline__ void stage_cell(const PassParams& P, const StageParams& Q, const ScanTarget& tg,
-                                           int32_t tau, int max_fail, bool live, uint64_t c, int fails,
-                                           uint64_t* seg_out, uint32_t* s_cnt) {
-    if (live) {
-        fails = P.sc[0].big ? stage_rows<R, POW2, true>(P, Q.row0, c, tau, fails, max_fail)
-                            : stage_rows<R, POW2, false>(P, Q.row0, c, tau, fails, max_fail);
-        live = fails <= max_fail;
-    }
+/* What follows the rows of a stage for one cell: the exact estimate and the candidate append (last stage) or the entry
+ * in the survivor list.  Must be reached by all 32 lanes (the appends are warp-aggregated). */
+template <bool POW2, bool LAST>
+__device__ __forceinline__ void stage_finish(const PassParams& P, const StageParams& Q, const ScanTarget& tg, int32_t tau,
+                                             bool live, uint64_t c, int fails, uint64_t* seg_out, uint32_t* s_cnt) {
     if (LAST) {
         int32_t est = 0;
+        if (live) live = seen_first_time(tg, c);             // later arrivals of a cell: nothing left to do
         if (live) est = P.sc[0].big ? estimate_all_rows<POW2, true>(P, Q.d_all, c)
                                     : estimate_all_rows<POW2, false>(P, Q.d_all, c);
         /* with exact fail counts live already implies est >= tau; a bitmap first stage counts conservatively */
@@ -83,6 +79,19 @@ __device__ __forceinline__ void stage_cell(const PassParams& P, const StageParam
             if (live) seg_out[base + __popc(mask & ((1u << lane) - 1u))] = c | ((uint64_t)fails << FAIL_SHIFT);
         }
     }
+}
+
+/* One cell through one stage: rows, then stage_finish.  Must be reached by all 32 lanes. */
+template <int R, bool POW2, bool LAST>
+__device__ __forceinline__ void stage_cell(const PassParams& P, const StageParams& Q, const ScanTarget& tg,
+                                           int32_t tau, int max_fail, bool live, uint64_t c, int fails,
+                                           uint64_t* seg_out, uint32_t* s_cnt) {
+    if (live) {
+        fails = P.sc[0].big ? stage_rows<R, POW2, true>(P, Q.row0, c, tau, fails, max_fail)
+                            : stage_rows<R, POW2, false>(P, Q.row0, c, tau, fails, max_fail);
+        live = fails <= max_fail;
+    }
+    stage_finish<POW2, LAST>(P, Q, tg, tau, live, c, fails, seg_out, s_cnt);
 }
 
 /* Stage 0: block b owns position groups [b*gpb, (b+1)*gpb); block 0 also takes the <= 6 edge particles. */
@@ -184,9 +193,9 @@ constexpr int CB_THREADS = 1024;
 
 struct CoarseParams {
     const uint32_t* fine;      // fine bitmap: bit (j*w + b)
-    const uint32_t* coarse;    // rows 0 .. FIRST-1, row_words words each
-    uint32_t g;                // log2 counters per coarse bit
-    uint32_t row_words;        // (w >> g) / 32
+    const uint32_t* coarse;    // rows 0 .. FIRST-1, row j at word offset row_off[j]
+    uint32_t g_row[5];         // log2 counters per coarse bit of row j
+    uint32_t row_off[6];       // row_off[FIRST] = total words (a multiple of 4)
     uint32_t big;              // cell ids of the mesh can exceed 2^31
     uint32_t nseg;             // segments = grid size of the following stages
 };
@@ -208,7 +217,7 @@ k_stage_first_cb(const __grid_constant__ PassParams P, const __grid_constant__ S
                  uint64_t groups, uint64_t gpb) {
     extern __shared__ __align__(16) uint32_t cb_smem[];
     __shared__ uint32_t s_cnt;
-    const uint32_t cwords = (uint32_t)FIRST * C.row_words;                            // a multiple of 4
+    const uint32_t cwords = C.row_off[FIRST];                                         // a multiple of 4
     {
         const uint4* src = reinterpret_cast<const uint4*>(C.coarse);
         uint4* dst = reinterpret_cast<uint4*>(cb_smem);
@@ -227,14 +236,20 @@ k_stage_first_cb(const __grid_constant__ PassParams P, const __grid_constant__ S
         uint64_t* out = Q.out + (uint64_t)seg * Q.seg_cap;
         const uint64_t g_lo = (uint64_t)seg * gpb;
         const uint64_t g_hi = g_lo + gpb < groups ? g_lo + gpb : groups;
+        /* the positions of the next iteration are fetched before this one is hashed (a load issued right before its
+         * first use stalls the warp for the whole trip to HBM) */
+        float4 n0 = make_float4(0.f, 0.f, 0.f, 0.f), n1 = n0, n2 = n0;
+        {
+            const uint64_t gf = g_lo + threadIdx.x;
+            if (gf < g_hi) { n0 = ld_stream16(body + 3 * gf); n1 = ld_stream16(body + 3 * gf + 1); n2 = ld_stream16(body + 3 * gf + 2); }
+        }
         for (uint64_t g0 = g_lo + (threadIdx.x - lane); g0 < g_hi; g0 += CB_THREADS) {
             const uint64_t g = g0 + lane;
             const bool in = g < g_hi;
-            float4 q0 = make_float4(0.f, 0.f, 0.f, 0.f), q1 = q0, q2 = q0;
-            if (in) {
-                q0 = ld_stream16(body + 3 * g);
-                q1 = ld_stream16(body + 3 * g + 1);
-                q2 = ld_stream16(body + 3 * g + 2);
+            const float4 q0 = n0, q1 = n1, q2 = n2;
+            {
+                const uint64_t gn = g + CB_THREADS;
+                if (gn < g_hi) { n0 = ld_stream16(body + 3 * gn); n1 = ld_stream16(body + 3 * gn + 1); n2 = ld_stream16(body + 3 * gn + 2); }
             }
             bool keep[4] = {in, in, in, in};
             if (P.sample && in) {
@@ -260,8 +275,8 @@ k_stage_first_cb(const __grid_constant__ PassParams P, const __grid_constant__ S
                 for (int q = 0; q < 2; ++q)
 #pragma unroll
                     for (int j = 0; j < FIRST; ++j) {
-                        const uint32_t i = h[q][j] >> C.g;
-                        wd[q][j] = (lds_u32s(cs_addr + ((uint32_t)j * C.row_words + (i >> 5)) * 4u) >> (i & 31u)) & 1u;
+                        const uint32_t i = h[q][j] >> C.g_row[j];
+                        wd[q][j] = (lds_u32s(cs_addr + (C.row_off[j] + (i >> 5)) * 4u) >> (i & 31u)) & 1u;
                     }
 #pragma unroll
                 for (int q = 0; q < 2; ++q)
@@ -417,34 +432,52 @@ k_build_coarse(const uint32_t* __restrict__ fine, uint64_t n_coarse_words, int g
     }
 }
 
-/* Group size 2^g of the coarse bitmap: the smallest whose FIRST rows fit the shared-memory budget.
- * false: shape not supported by the bitmap first stage (the caller uses the plain stages). */
-bool coarse_shape(int d, int rank, uint64_t w, uint32_t* g_out, uint32_t* row_words_out) {
+/* Shape of the coarse bitmap: g = the smallest group size 2^g whose FIRST rows fit the shared-memory budget, then as
+ * many leading rows as still fit at 2^(g-1).  false: shape not supported by the bitmap first stage (the caller uses the
+ * plain stages). */
+bool coarse_shape(int d, int rank, uint64_t w, CoarseShape* out) {
     const int first = rank + 1, rest = d - first;
+    const uint64_t budget = 190 * 1024;                                       // all rows at 2^g
+    /* with leading rows at 2^(g-1).  What is left of the 228 KB is the L1 cache of the position loads and of the fine-bitmap
+     * gathers: measured at cfg 3 (g = 4), first stage 13.2 / 12.6 / 12.0 / 17.3 ms with 128 / 160 / 192 / 224 KB of bitmap */
+    const uint64_t budget_fine = 192 * 1024;
     if (first > 5 || rest < 1 || rest > 8 || (w & (w - 1)) || w < 4096) return false;
     for (uint32_t g = 0; g <= 8; ++g) {
         if ((w >> g) < 128) break;
-        if ((uint64_t)first * ((w >> g) / 8) <= 190 * 1024) {
-            *g_out = g;
-            *row_words_out = (uint32_t)((w >> g) / 32);
-            return true;
+        const uint64_t row = (w >> g) / 8;                                    // bytes per row at 2^g
+        if ((uint64_t)first * row > budget) continue;
+        uint32_t nf = 0;
+        if (g >= 1)
+            while (nf < (uint32_t)first && (uint64_t)(nf + 1) * 2 * row + (uint64_t)(first - nf - 1) * row <= budget_fine) ++nf;
+        out->g = g;
+        out->n_fine = nf;
+        uint32_t off = 0;
+        for (int j = 0; j <= first; ++j) {
+            out->row_off[j] = off;
+            off += (uint32_t)(((uint32_t)j < nf ? 2 * row : row) / 4);
         }
+        return true;
     }
     return false;
 }
 
-/* fine: bitmap of the scale (bit j*w + b), already built for the current tau; coarse: scratch of FIRST*row_words words */
+/* fine: bitmap of the scale (bit j*w + b), already built for the current tau; coarse: scratch of shape.row_off[first] words */
 cudaError_t launch_scan_staged_cb(const PassParams& P, const ScanTarget& tg, const StageBuffers& B, const uint32_t* fine,
-                                  uint32_t* coarse, uint32_t g, uint32_t row_words, bool rebuild_coarse, const float* xyz,
+                                  uint32_t* coarse, const CoarseShape& shape, bool rebuild_coarse, const float* xyz,
                                   uint64_t n, int sm_count, cudaStream_t st, uint64_t* launches, PhaseTimer* tm) {
     const int first = P.rank + 1, rest = P.d - first;
     if (rebuild_coarse) {
         if (tm) tm->mark(PH_BITMAP, st);
-        const uint64_t words = (uint64_t)first * row_words;
-        uint64_t blocks = (words + 255) / 256;
-        if (blocks > 148 * 8) blocks = 148 * 8;
-        k_build_coarse<<<(int)blocks, 256, 0, st>>>(fine, words, (int)g, coarse);
-        *launches += 1;
+        for (int part = 0; part < 2; ++part) {              // rows [0, n_fine) at g-1, rows [n_fine, first) at g
+            const uint32_t j0 = part ? shape.n_fine : 0, j1 = part ? (uint32_t)first : shape.n_fine;
+            if (j0 == j1) continue;
+            const uint64_t words = shape.row_off[j1] - shape.row_off[j0];
+            uint64_t blocks = (words + 255) / 256;
+            if (blocks > 148 * 8) blocks = 148 * 8;
+            k_build_coarse<<<(int)blocks, 256, 0, st>>>(fine + (uint64_t)j0 * P.w / 32, words, (int)(part ? shape.g : shape.g - 1),
+                                                        coarse + shape.row_off[j0]);
+            *launches += 1;
+        }
     }
     uint32_t head;
     uint64_t groups;
@@ -458,9 +491,11 @@ cudaError_t launch_scan_staged_cb(const PassParams& P, const ScanTarget& tg, con
     Q.out = B.list[0]; Q.cnt_out = B.cnt[0];
     Q.seg_cap = seg_cap; Q.row0 = 0; Q.d_all = P.d; Q.pad = 0;
     CoarseParams C;
-    C.fine = fine; C.coarse = coarse; C.g = g; C.row_words = row_words; C.nseg = (uint32_t)blocks;
+    C.fine = fine; C.coarse = coarse; C.nseg = (uint32_t)blocks;
+    for (int j = 0; j < 5; ++j) C.g_row[j] = (uint32_t)j < shape.n_fine ? shape.g - 1 : shape.g;
+    for (int j = 0; j < 6; ++j) C.row_off[j] = j <= first ? shape.row_off[j] : 0;
     C.big = P.sc[0].big;
-    const size_t smem = (size_t)first * row_words * 4;
+    const size_t smem = (size_t)shape.row_off[first] * 4;
     cudaError_t e = cudaSuccess;
     if (tm) tm->mark(PH_SCAN_FIRST, st);
 #define CS_CB(F)                                                                                              \
