@@ -656,8 +656,10 @@ int scan_device_raw(cs_sketch* s, const float* xyz, uint64_t n, double sample_p)
         if (s->first_chunk && s->k_max) {                /* a small first chunk fixes a first tau cheaply */
             uint64_t c0 = 8 * s->k_max > (1u << 18) ? 8 * s->k_max : (1u << 18);
             if (chunk > c0) chunk = c0;
-        } else if (s->k_max && chunk > 4 * s->scanned) {  /* tau still rises fast: grow geometrically, not at once */
-            chunk = 4 * s->scanned;
+        } else if (s->k_max && chunk > 4 * s->scanned) {  /* tau still rises fast: grow geometrically, not at once ... */
+            bool capped = s->thr_min != INT32_MAX;           /* ... unless it already sits at the excursion limit everywhere */
+            for (int i = 0; i < s->n_scales && capped; ++i) capped = s->st_host[i].tau >= s->thr_min;
+            if (!capped) chunk = 4 * s->scanned;
         }
         if (chunk > n - done) chunk = n - done;
         if (chunk < n - done) chunk &= ~(uint64_t)3;     /* keep the 16-byte phase of the remaining stream */

@@ -48,42 +48,23 @@ __device__ __forceinline__ int stage_rows(const PassParams& P, int row0, uint64_
     return fails;
 }
 
-template <bool POW2, bool BIG>
-__device__ __noinline__ int32_t estimate_all_rows(const PassParams& P, int d, uint64_t c) {
-    const uint32_t c0 = cell_c0(c), c1 = cell_c1(c);
-    int32_t v[CS_MAX_ROWS];
-    for (int j = 0; j < d; ++j) v[j] = row_value<BIG, POW2>(P, P.sc[0].T, P.rows[j], j, c0, c1);
-    return select_rt(v, d, P.rank);
-}
-
-/* What follows the rows of a stage for one cell: the exact estimate and the candidate append (last stage) or the entry
- * in the survivor list.  Must be reached by all 32 lanes (the appends are warp-aggregated). */
-template <bool POW2, bool LAST>
-__device__ __forceinline__ void stage_finish(const PassParams& P, const StageParams& Q, const ScanTarget& tg, int32_t tau,
-                                             bool live, uint64_t c, int fails, uint64_t* seg_out, uint32_t* s_cnt) {
-    if (LAST) {
-        int32_t est = 0;
-        if (live) live = seen_first_time(tg, c);             // later arrivals of a cell: nothing left to do
-        if (live) est = P.sc[0].big ? estimate_all_rows<POW2, true>(P, Q.d_all, c)
-                                    : estimate_all_rows<POW2, false>(P, Q.d_all, c);
-        /* with exact fail counts live already implies est >= tau; a bitmap first stage counts conservatively */
-        append_candidate(tg, live && est >= tau, c, est);
-    } else {
-        const uint32_t mask = __ballot_sync(0xFFFFFFFFu, live);
-        if (mask) {
-            const uint32_t lane = threadIdx.x & 31u;
-            const int leader = __ffs(mask) - 1;
-            uint32_t base = 0;
-            if ((int)lane == leader) base = atomicAdd(s_cnt, (uint32_t)__popc(mask));
-            base = __shfl_sync(0xFFFFFFFFu, base, leader);
-            if (live) seg_out[base + __popc(mask & ((1u << lane) - 1u))] = c | ((uint64_t)fails << FAIL_SHIFT);
-        }
+/* A cell that is still alive after the rows of a stage goes to the block's segment of the survivor list.  Must be
+ * reached by all 32 lanes (one shared-memory reservation per warp). */
+__device__ __forceinline__ void stage_finish(bool live, uint64_t c, int fails, uint64_t* seg_out, uint32_t* s_cnt) {
+    const uint32_t mask = __ballot_sync(0xFFFFFFFFu, live);
+    if (mask) {
+        const uint32_t lane = threadIdx.x & 31u;
+        const int leader = __ffs(mask) - 1;
+        uint32_t base = 0;
+        if ((int)lane == leader) base = atomicAdd(s_cnt, (uint32_t)__popc(mask));
+        base = __shfl_sync(0xFFFFFFFFu, base, leader);
+        if (live) seg_out[base + __popc(mask & ((1u << lane) - 1u))] = c | ((uint64_t)fails << FAIL_SHIFT);
     }
 }
 
 /* One cell through one stage: rows, then stage_finish.  Must be reached by all 32 lanes. */
-template <int R, bool POW2, bool LAST>
-__device__ __forceinline__ void stage_cell(const PassParams& P, const StageParams& Q, const ScanTarget& tg,
+template <int R, bool POW2>
+__device__ __forceinline__ void stage_cell(const PassParams& P, const StageParams& Q,
                                            int32_t tau, int max_fail, bool live, uint64_t c, int fails,
                                            uint64_t* seg_out, uint32_t* s_cnt) {
     if (live) {
@@ -91,11 +72,11 @@ __device__ __forceinline__ void stage_cell(const PassParams& P, const StageParam
                             : stage_rows<R, POW2, false>(P, Q.row0, c, tau, fails, max_fail);
         live = fails <= max_fail;
     }
-    stage_finish<POW2, LAST>(P, Q, tg, tau, live, c, fails, seg_out, s_cnt);
+    stage_finish(live, c, fails, seg_out, s_cnt);
 }
 
 /* Stage 0: block b owns position groups [b*gpb, (b+1)*gpb); block 0 also takes the <= 6 edge particles. */
-template <int R, bool POW2, bool LAST>
+template <int R, bool POW2>
 __global__ void __launch_bounds__(PASS_THREADS)
 k_stage_first(const __grid_constant__ PassParams P, const __grid_constant__ StageParams Q,
               const __grid_constant__ ScanTarget tg, const float* __restrict__ xyz, uint64_t n, uint32_t head,
@@ -105,7 +86,7 @@ k_stage_first(const __grid_constant__ PassParams P, const __grid_constant__ Stag
     __syncthreads();
     const int32_t tau = tg.st->tau;
     const int max_fail = P.rank;
-    uint64_t* seg = LAST ? nullptr : Q.out + (uint64_t)blockIdx.x * Q.seg_cap;
+    uint64_t* seg = Q.out + (uint64_t)blockIdx.x * Q.seg_cap;
     const float4* body = reinterpret_cast<const float4*>(xyz + 3 * (uint64_t)head);
     const uint64_t g_lo = (uint64_t)blockIdx.x * gpb;
     const uint64_t g_hi = g_lo + gpb < groups ? g_lo + gpb : groups;
@@ -127,10 +108,10 @@ k_stage_first(const __grid_constant__ PassParams P, const __grid_constant__ Stag
             k2 = keep_particle(P.K, i0 + 2, P.Tp);
             k3 = keep_particle(P.K, i0 + 3, P.Tp);
         }
-        stage_cell<R, POW2, LAST>(P, Q, tg, tau, max_fail, k0, cell_of(q0.x, q0.y, q0.z, P.sc[0]), 0, seg, &s_cnt);
-        stage_cell<R, POW2, LAST>(P, Q, tg, tau, max_fail, k1, cell_of(q0.w, q1.x, q1.y, P.sc[0]), 0, seg, &s_cnt);
-        stage_cell<R, POW2, LAST>(P, Q, tg, tau, max_fail, k2, cell_of(q1.z, q1.w, q2.x, P.sc[0]), 0, seg, &s_cnt);
-        stage_cell<R, POW2, LAST>(P, Q, tg, tau, max_fail, k3, cell_of(q2.y, q2.z, q2.w, P.sc[0]), 0, seg, &s_cnt);
+        stage_cell<R, POW2>(P, Q, tau, max_fail, k0, cell_of(q0.x, q0.y, q0.z, P.sc[0]), 0, seg, &s_cnt);
+        stage_cell<R, POW2>(P, Q, tau, max_fail, k1, cell_of(q0.w, q1.x, q1.y, P.sc[0]), 0, seg, &s_cnt);
+        stage_cell<R, POW2>(P, Q, tau, max_fail, k2, cell_of(q1.z, q1.w, q2.x, P.sc[0]), 0, seg, &s_cnt);
+        stage_cell<R, POW2>(P, Q, tau, max_fail, k3, cell_of(q2.y, q2.z, q2.w, P.sc[0]), 0, seg, &s_cnt);
     }
     if (blockIdx.x == 0 && threadIdx.x < 32) {
         const uint64_t tail0 = (uint64_t)head + 4 * groups;
@@ -143,16 +124,14 @@ k_stage_first(const __grid_constant__ PassParams P, const __grid_constant__ Stag
             const float* p = xyz + 3 * i;
             c = cell_of(ld_stream4(p), ld_stream4(p + 1), ld_stream4(p + 2), P.sc[0]);
         }
-        stage_cell<R, POW2, LAST>(P, Q, tg, tau, max_fail, keep, c, 0, seg, &s_cnt);
+        stage_cell<R, POW2>(P, Q, tau, max_fail, keep, c, 0, seg, &s_cnt);
     }
-    if (!LAST) {
-        __syncthreads();
-        if (threadIdx.x == 0) Q.cnt_out[blockIdx.x] = s_cnt;
-    }
+    __syncthreads();
+    if (threadIdx.x == 0) Q.cnt_out[blockIdx.x] = s_cnt;
 }
 
 /* Stage i > 0: block b reads segment b of the previous stage. */
-template <int R, bool POW2, bool LAST>
+template <int R, bool POW2>
 __global__ void __launch_bounds__(PASS_THREADS)
 k_stage_next(const __grid_constant__ PassParams P, const __grid_constant__ StageParams Q,
              const __grid_constant__ ScanTarget tg) {
@@ -162,17 +141,43 @@ k_stage_next(const __grid_constant__ PassParams P, const __grid_constant__ Stage
     const int32_t tau = tg.st->tau;
     const int max_fail = P.rank;
     const uint64_t* seg_in = Q.in + (uint64_t)blockIdx.x * Q.seg_cap;
-    uint64_t* seg = LAST ? nullptr : Q.out + (uint64_t)blockIdx.x * Q.seg_cap;
+    uint64_t* seg = Q.out + (uint64_t)blockIdx.x * Q.seg_cap;
     const uint32_t cnt = Q.cnt_in[blockIdx.x];
     for (uint32_t t0 = 0; t0 < cnt; t0 += PASS_THREADS) {
         const uint32_t t = t0 + threadIdx.x;
         const bool live = t < cnt;
         const uint64_t e = live ? seg_in[t] : 0;
-        stage_cell<R, POW2, LAST>(P, Q, tg, tau, max_fail, live, e & CELL_MASK, (int)(e >> FAIL_SHIFT), seg, &s_cnt);
+        stage_cell<R, POW2>(P, Q, tau, max_fail, live, e & CELL_MASK, (int)(e >> FAIL_SHIFT), seg, &s_cnt);
     }
-    if (!LAST) {
-        __syncthreads();
-        if (threadIdx.x == 0) Q.cnt_out[blockIdx.x] = s_cnt;
+    __syncthreads();
+    if (threadIdx.x == 0) Q.cnt_out[blockIdx.x] = s_cnt;
+}
+
+/* After the last stage: the cells still alive (few) get their exact estimate -- all d rows, values in registers, median
+ * network -- and are appended to the candidate list iff Estimate >= tau (a bitmap first stage counts fails
+ * conservatively) and, when the duplicate filter is on, on their first arrival.  A kernel of its own so that this runs on
+ * full warps: inside the last stage one lane in ten took this path and every warp paid for it (cfg 5: 1400 thread
+ * instructions per surviving cell). */
+template <int D, bool POW2>
+__global__ void __launch_bounds__(PASS_THREADS)
+k_stage_final(const __grid_constant__ PassParams P, const __grid_constant__ StageParams Q,
+              const __grid_constant__ ScanTarget tg) {
+    const int32_t tau = tg.st->tau;
+    const uint64_t* seg_in = Q.in + (uint64_t)blockIdx.x * Q.seg_cap;
+    const uint32_t cnt = Q.cnt_in[blockIdx.x];
+    for (uint32_t t0 = 0; t0 < cnt; t0 += PASS_THREADS) {
+        const uint32_t t = t0 + threadIdx.x;
+        bool emit = false;
+        uint64_t c = 0;
+        int32_t est = 0;
+        if (t < cnt) {
+            c = seg_in[t] & CELL_MASK;
+            if (seen_first_time(tg, c)) {
+                est = P.sc[0].big ? estimate_full<D, POW2, true>(P, 0, c) : estimate_full<D, POW2, false>(P, 0, c);
+                emit = est >= tau;
+            }
+        }
+        append_candidate(tg, emit, c, est);
     }
 }
 
@@ -185,7 +190,7 @@ k_stage_next(const __grid_constant__ PassParams P, const __grid_constant__ Stage
  * Only bucket hashes are needed (no sign hashes).  All four particles of a thread are taken through the phases
  * together, so that up to 4*FIRST gathers per thread are in flight.  Fail counts are conservative (a set bit may
  * still fail on the sign or the exact value); survivors go to the per-segment lists in the format of k_stage_first
- * and the remaining rows run in k_stage_next<.., LAST> on dense warps, which re-checks Estimate >= tau exactly.
+ * and the remaining rows run in k_stage_next on dense warps; k_stage_final then checks Estimate >= tau exactly.
  * One CTA of 512 threads per SM walks the segments blockIdx.x, blockIdx.x + gridDim.x, ...
  * ------------------------------------------------------------------------------------------------------------ */
 
@@ -341,26 +346,34 @@ k_stage_first_cb(const __grid_constant__ PassParams P, const __grid_constant__ S
 
 /* ---- host side ------------------------------------------------------------------------------------------ */
 
-template <int R, bool POW2, bool LAST>
+template <int R, bool POW2>
 static void launch_stage(bool first, int blocks, const PassParams& P, const StageParams& Q, const ScanTarget& tg,
                          const float* xyz, uint64_t n, uint32_t head, uint64_t groups, uint64_t gpb, cudaStream_t st) {
-    if (first) k_stage_first<R, POW2, LAST><<<blocks, PASS_THREADS, 0, st>>>(P, Q, tg, xyz, n, head, groups, gpb);
-    else       k_stage_next<R, POW2, LAST><<<blocks, PASS_THREADS, 0, st>>>(P, Q, tg);
+    if (first) k_stage_first<R, POW2><<<blocks, PASS_THREADS, 0, st>>>(P, Q, tg, xyz, n, head, groups, gpb);
+    else       k_stage_next<R, POW2><<<blocks, PASS_THREADS, 0, st>>>(P, Q, tg);
 }
 
-template <bool POW2, bool LAST>
+/* the survivors of the last stage (list Q.in) -> exact estimates -> candidate list */
+template <bool POW2>
+static void launch_final(int blocks, const PassParams& P, const StageParams& Q, const ScanTarget& tg, cudaStream_t st) {
+#define CS_CALL(DD) k_stage_final<DD, POW2><<<blocks, PASS_THREADS, 0, st>>>(P, Q, tg)
+    CS_DISPATCH_D(CS_CALL)
+#undef CS_CALL
+}
+
+template <bool POW2>
 static void launch_stage_r(int R, bool first, int blocks, const PassParams& P, const StageParams& Q,
                            const ScanTarget& tg, const float* xyz, uint64_t n, uint32_t head, uint64_t groups,
                            uint64_t gpb, cudaStream_t st) {
     switch (R) {
-        case 1: launch_stage<1, POW2, LAST>(first, blocks, P, Q, tg, xyz, n, head, groups, gpb, st); break;
-        case 2: launch_stage<2, POW2, LAST>(first, blocks, P, Q, tg, xyz, n, head, groups, gpb, st); break;
-        case 3: launch_stage<3, POW2, LAST>(first, blocks, P, Q, tg, xyz, n, head, groups, gpb, st); break;
-        case 4: launch_stage<4, POW2, LAST>(first, blocks, P, Q, tg, xyz, n, head, groups, gpb, st); break;
-        case 5: launch_stage<5, POW2, LAST>(first, blocks, P, Q, tg, xyz, n, head, groups, gpb, st); break;
-        case 6: launch_stage<6, POW2, LAST>(first, blocks, P, Q, tg, xyz, n, head, groups, gpb, st); break;
-        case 7: launch_stage<7, POW2, LAST>(first, blocks, P, Q, tg, xyz, n, head, groups, gpb, st); break;
-        default: launch_stage<8, POW2, LAST>(first, blocks, P, Q, tg, xyz, n, head, groups, gpb, st); break;
+        case 1: launch_stage<1, POW2>(first, blocks, P, Q, tg, xyz, n, head, groups, gpb, st); break;
+        case 2: launch_stage<2, POW2>(first, blocks, P, Q, tg, xyz, n, head, groups, gpb, st); break;
+        case 3: launch_stage<3, POW2>(first, blocks, P, Q, tg, xyz, n, head, groups, gpb, st); break;
+        case 4: launch_stage<4, POW2>(first, blocks, P, Q, tg, xyz, n, head, groups, gpb, st); break;
+        case 5: launch_stage<5, POW2>(first, blocks, P, Q, tg, xyz, n, head, groups, gpb, st); break;
+        case 6: launch_stage<6, POW2>(first, blocks, P, Q, tg, xyz, n, head, groups, gpb, st); break;
+        case 7: launch_stage<7, POW2>(first, blocks, P, Q, tg, xyz, n, head, groups, gpb, st); break;
+        default: launch_stage<8, POW2>(first, blocks, P, Q, tg, xyz, n, head, groups, gpb, st); break;
     }
 }
 
@@ -399,15 +412,18 @@ cudaError_t launch_scan_staged(const PassParams& P, const ScanTarget& tg, const 
         Q.d_all = P.d;
         Q.pad = 0;
         if (tm) tm->mark(i == 0 ? PH_SCAN_FIRST : PH_SCAN_NEXT, st);
-        if (pow2) {
-            if (last) launch_stage_r<true, true>(R, i == 0, blocks, P, Q, tg, xyz, n, head, groups, gpb, st);
-            else      launch_stage_r<true, false>(R, i == 0, blocks, P, Q, tg, xyz, n, head, groups, gpb, st);
-        } else {
-            if (last) launch_stage_r<false, true>(R, i == 0, blocks, P, Q, tg, xyz, n, head, groups, gpb, st);
-            else      launch_stage_r<false, false>(R, i == 0, blocks, P, Q, tg, xyz, n, head, groups, gpb, st);
-        }
+        if (pow2) launch_stage_r<true>(R, i == 0, blocks, P, Q, tg, xyz, n, head, groups, gpb, st);
+        else      launch_stage_r<false>(R, i == 0, blocks, P, Q, tg, xyz, n, head, groups, gpb, st);
         *launches += 1;
         cur ^= 1;
+        if (last) {
+            StageParams F = Q;
+            F.in = B.list[cur];
+            F.cnt_in = B.cnt[cur];
+            if (pow2) launch_final<true>(blocks, P, F, tg, st);
+            else      launch_final<false>(blocks, P, F, tg, st);
+            *launches += 1;
+        }
     }
     return cudaGetLastError();
 }
@@ -513,8 +529,12 @@ cudaError_t launch_scan_staged_cb(const PassParams& P, const ScanTarget& tg, con
     Q2.out = B.list[1]; Q2.cnt_out = B.cnt[1];
     Q2.row0 = first;
     if (tm) tm->mark(PH_SCAN_NEXT, st);
-    launch_stage_r<true, true>(rest, false, blocks, P, Q2, tg, xyz, n, head, groups, gpb, st);
-    *launches += 1;
+    launch_stage_r<true>(rest, false, blocks, P, Q2, tg, xyz, n, head, groups, gpb, st);
+    StageParams F = Q2;
+    F.in = B.list[1];
+    F.cnt_in = B.cnt[1];
+    launch_final<true>(blocks, P, F, tg, st);
+    *launches += 2;
     return cudaGetLastError();
 }
 

@@ -278,3 +278,43 @@ def test_scan_begin_rejects_oversized_k(cs):
         g.scan_begin((1 << 26) + 1)
     assert e.value.code == cs.CS_ERR_ARG
     g.close()
+
+
+def test_one_crossing_hierarchical_query_cfg4_shape(cs):
+    """bench.py --workload cfg4 --query hierarchical at reduced size: ONE host-streamed update feeds a coarse and the fine
+    mesh (G = 4642 = 11 * 422), the query is positions-free (Alg. 3): full search of the coarse
+    mesh, then the children of its c*k heaviest cells.  Expected values: the oracle's own full search of the coarse mesh and
+    its estimates of exactly those children.  The candidate set differs from the re-scan's on purpose (full dictionary)."""
+    from paper_1711_00975_b200 import synth
+    Gf, r = 4642, 11
+    wl = synth.CONFIGS["cfg4"].scaled(6 * (1 << 16) + 77, w=1 << 16, G=(Gf // r, Gf))
+    xyz = synth.generate(wl, device="cuda")
+    host = _host_copy(xyz, True)
+    k, c = 300, 4
+    o = ora.OracleSketch(wl.d, wl.w, wl.G, wl.L, wl.seed)
+    o.update(host.numpy())
+    g = cs.CountSketch(wl.d, wl.w, list(wl.G), wl.L, wl.seed)
+    g.set_chunk_sizes(1 << 16, 0, 0, 0)
+    g.update_host(host)
+    g.scan_begin(c * k)
+    g.scan_all(0)
+    parents, pest = g.topk(c * k, 0)
+    cells0 = np.arange((Gf // r) ** 3, dtype=np.uint64)
+    e0 = o.estimate(cells0, 0)
+    order = np.lexsort((cells0, -e0.astype(np.int64)))[: c * k]
+    assert np.array_equal(_ids(parents), cells0[order]) and np.array_equal(pest.cpu().numpy(), e0[order])
+    g.scan_children(parents, 0, 1)
+    kids, kest = g.topk(k, 1, device="cpu")
+    p = cells0[order]
+    Gp = np.uint64(Gf // r)
+    px, py, pz = p % Gp, (p // Gp) % Gp, p // (Gp * Gp)
+    t = np.arange(r ** 3, dtype=np.uint64)
+    R, G64 = np.uint64(r), np.uint64(Gf)
+    cx = (px[:, None] * R + t % R).ravel()
+    cy = (py[:, None] * R + (t // R) % R).ravel()
+    cz = (pz[:, None] * R + t // (R * R)).ravel()
+    kid = np.unique(cx + G64 * (cy + G64 * cz))
+    ek = o.estimate(kid, 1)
+    ordk = np.lexsort((kid, -ek.astype(np.int64)))[:k]
+    assert np.array_equal(_ids(kids), kid[ordk]) and np.array_equal(kest.numpy(), ek[ordk])
+    g.close(); o.close()
