@@ -9,8 +9,9 @@
  *                a cell is dropped once fails > (d-1)/2 (its median is then < tau);
  *                survivors are written as (c | fails << 60) to a list
  *   stage i      list -> rows of group i -> list
- *   last stage   survivors have Estimate(c) >= tau: the full median over all d rows is recomputed for them
- *                (they are few) and (c, est) is appended to the candidate list.
+ *   final        (k_stage_final) the survivors of the last stage have Estimate(c) >= tau (or may have, after a bitmap
+ *                first stage): the exact median over all d rows is computed for them on dense warps and (c, est) is
+ *                appended to the candidate list.
  * Lists are segmented per block (block b of every stage owns segment b), so no global atomic is needed for the
  * survivor lists and the result does not depend on scheduling (the candidate list is sorted afterwards).
  */

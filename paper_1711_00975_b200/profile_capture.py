@@ -98,7 +98,7 @@ def main():
                      "alu_pipe_pct": val("sm__pipe_alu_cycles_active.avg.pct_of_peak_sustained_active"),
                      "fma_pipe_pct": val("sm__pipe_fma_cycles_active.avg.pct_of_peak_sustained_active"),
                      "source": path.name}
-            key = re.match(r"k_[a-z_]+", name).group(0)
+            key = re.match(r"k_[a-z_]+", name).group(0).rstrip("_")
             if key == "k_bin_scatter":
                 entry["thread_instructions_per_particle"] = 32.0 * entry["warp_instructions_per_launch"] / a.particles_per_launch
                 entry["passes_per_particle"] = a.passes_per_particle
