@@ -243,7 +243,11 @@ def main_arm(args, wl):
     t_gen = time.perf_counter()
     if strong:      # one stream of wl.N particles cut into contiguous shards (total work fixed)
         lo, hi = sharded.shard_bounds(wl.N, rank, world)
-        xyz = synth.Catalogue(wl, "cuda").positions(lo, hi - lo)
+        cat = synth.Catalogue(wl, "cuda")
+        xyz = torch.empty((hi - lo, 3), dtype=torch.float32, device="cuda")
+        for i0 in range(lo, hi, 1 << 22):                    # chunked: the generator holds ~20 temporaries per particle
+            m = min(1 << 22, hi - i0)
+            cat.positions(i0, m, out=xyz[i0 - lo:i0 - lo + m])
         index0 = lo
     else:           # rank r owns batch r of the stream (same catalogue, per-batch keys): N particles per GPU
         xyz = synth.generate(wl, device="cuda", batch=rank)
