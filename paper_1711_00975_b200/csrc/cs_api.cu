@@ -324,7 +324,7 @@ bool bad_p(double p) { return !(p > 0.0) || p > 1.0; }
 
 constexpr uint32_t BIN_MAX = 4096;                    /* bins per pass (words of `cursor`) */
 constexpr uint64_t BIN_MIN_N = 1ull << 22;            /* auto mode: below this the direct kernel is as fast */
-constexpr size_t BIN_SMEM = 200 * 1024;               /* shared memory of one scatter CTA */
+constexpr size_t BIN_SMEM = 216 * 1024;               /* shared memory of one scatter CTA (6 pairs per round at cfg 3: 209 KB) */
 
 struct BinPlan {
     uint32_t log2w, log2S, SL, C, threads;
