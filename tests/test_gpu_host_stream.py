@@ -318,3 +318,34 @@ def test_one_crossing_hierarchical_query_cfg4_shape(cs):
     ordk = np.lexsort((kid, -ek.astype(np.int64)))[:k]
     assert np.array_equal(_ids(kids), kid[ordk]) and np.array_equal(kest.numpy(), ek[ordk])
     g.close(); o.close()
+
+
+def test_phase_timing_and_route_counters(cs):
+    """cs_set_timing / cs_get_timing / cs_update_stats: the counters of the binned route account for every record
+    (particles x binned rows), a single-cell stream pushes almost all of them through the overflow routes, and the phase
+    timer reports the kernel classes that ran."""
+    from paper_1711_00975_b200 import synth
+    wl, xyz = _gen("cfg3", (1 << 22) + 2)
+    g = cs.CountSketch(wl.d, wl.w, list(wl.G), wl.L, wl.seed)
+    g.set_update_mode(2, 3)                                   # binned, 3 of 7 rows direct -> 4 binned rows
+    g.set_timing(True)
+    g.update(xyz)
+    st = g.update_stats()
+    # torch allocations are 256-byte aligned and n is even: no head / tail particle outside the pairs
+    assert st["staging_overflow"] + st["region_overflow"] + st["leftover"] + st["binned"] == 4 * ((1 << 22) + 2), st
+    assert st["staging_overflow"] == 0 and st["region_overflow"] == 0          # clustered but spread stream: nothing overflows
+    g.scan_begin(1000)
+    g.scan(xyz)
+    g.topk(1000)
+    tm = g.get_timing()
+    assert tm["update_scatter"][0] > 0 and tm["update_apply"][0] > 0 and tm["scan_first"][0] > 0 and tm["select"][0] > 0
+    assert tm["update_scatter"][1] == 1 and tm["compact_kept"] == (0.0, 0)
+    assert g.get_timing()["update_scatter"] == (0.0, 0)       # read and forgotten
+    g.set_timing(False)
+    g.reset()
+    one = torch.full((1 << 21, 3), 3.3, dtype=torch.float32, device="cuda")
+    g.update(one)
+    st = g.update_stats()
+    assert st["staging_overflow"] + st["region_overflow"] > 0.9 * 4 * (1 << 21), st
+    assert st["staging_overflow"] + st["region_overflow"] + st["leftover"] + st["binned"] == 4 * (1 << 21)
+    g.close()
