@@ -8,7 +8,8 @@ Compared elementwise: the whole int32 table of every scale, 10^5 estimates (occu
 and values, and (cfg 5) the excursion sets at every threshold.
 
 Opt-in: minutes of host time and ~40 GB of host memory.  CS_FULL_PARITY=1 python -m pytest tests/test_full_size_parity.py -m gpu
-(CS_FULL_PARITY_THREADS overrides the number of oracle threads, default = all cores).  Each test appends a line to
+(CS_FULL_PARITY_THREADS overrides the number of oracle threads, default = all cores; CS_FULL_PARITY_CFG4_BATCHES=38 runs
+the cfg 4 test over the whole 10^10-particle stream: 120 GB pinned, 12 minutes).  Each test appends a line to
 gpurun_out/full_parity.log when it passes.
 """
 import os
@@ -127,34 +128,37 @@ def test_cfg4_three_batches_host_streamed_against_the_oracle(cs):
     through cs_update_host / cs_scan_host: 48 staging batches of 2^24 particles, three host calls."""
     from paper_1711_00975_b200 import synth
     wl = synth.CONFIGS["cfg4"]
-    B, nb = wl.batch, 3
+    B = wl.batch
+    nb = int(os.environ.get("CS_FULL_PARITY_CFG4_BATCHES", "3"))     # 38 = the whole 10^10-particle stream (120 GB pinned)
+    N = min(nb * B, wl.N)
     cat = synth.Catalogue(wl, "cuda")
-    host = torch.empty((nb * B, 3), dtype=torch.float32, pin_memory=True)
-    for b in range(nb):
-        host[b * B:(b + 1) * B].copy_(synth.generate(wl, device="cuda", batch=b, n=B, catalogue=cat))
+    host = torch.empty((N, 3), dtype=torch.float32, pin_memory=True)
+    cuts = [(b * B, min((b + 1) * B, N)) for b in range(nb) if b * B < N]
+    for b, (lo, hi) in enumerate(cuts):
+        host[lo:hi].copy_(synth.generate(wl, device="cuda", batch=b, n=hi - lo, catalogue=cat))
     torch.cuda.synchronize()
     host_np = host.numpy()
     k = wl.k
     g = cs.CountSketch(wl.d, wl.w, list(wl.G), wl.L, wl.seed)
-    for b in range(nb):
-        g.update_host(host[b * B:(b + 1) * B])
+    for lo, hi in cuts:
+        g.update_host(host[lo:hi])
     g.scan_begin(k)
-    for b in range(nb):
-        g.scan_host(host[b * B:(b + 1) * B])
+    for lo, hi in cuts:
+        g.scan_host(host[lo:hi])
     stats = g.scan_stats(0)
     t0 = time.perf_counter()
     so = ShardedOracle(wl.d, wl.w, wl.G, wl.L, wl.seed, THREADS)
-    for b in range(nb):
-        so.update(host_np[b * B:(b + 1) * B], 1.0, b * B)
+    for lo, hi in cuts:
+        so.update(host_np[lo:hi], 1.0, lo)
     gt = g.sketch(0).cpu().numpy()
     assert np.array_equal(gt, so.sketch(0)), f"table differs: {_first_diff(gt, so.sketch(0))}"
     _estimates_agree(g, so, wl, host_np, np.random.default_rng(12))
-    tops = [so.select(host_np[b * B:(b + 1) * B], k, ora.INT32_MAX, 1.0, b * B)[0][0] for b in range(nb)]
+    tops = [so.select(host_np[lo:hi], k, ora.INT32_MAX, 1.0, lo)[0][0] for lo, hi in cuts]
     ti, te = _merge(tops, k)
     gi, gv = g.topk(k, 0, device="cpu")
     assert np.array_equal(_ids(gi), ti), f"top-k ids differ: {_first_diff(_ids(gi), ti)}"
     assert np.array_equal(gv.numpy(), te), f"top-k values differ: {_first_diff(gv.numpy(), te)}"
-    _log(f"PASS cfg4 x {nb} batches: N={nb * B} host-streamed (48 staging batches) d={wl.d} w={wl.w} G={list(wl.G)} k={k}: "
+    _log(f"PASS cfg4 x {len(cuts)} batches: N={N} host-streamed ({-(-N // (1 << 24))} staging batches) d={wl.d} w={wl.w} G={list(wl.G)} k={k}: "
          f"int32 table, 1e5 estimates, top-{k} ids+values bit-exact to the oracle over {THREADS} index ranges; scan: {stats}; "
          f"oracle {time.perf_counter() - t0:.0f} s")
     g.close(); so.close()
