@@ -1261,6 +1261,7 @@ int cs_set_chunk_sizes(cs_sketch* s, uint64_t stage_particles, uint64_t update_c
         CS_CUDA(cudaStreamSynchronize(s->stream));
         if (s->copy_stream) CS_CUDA(cudaStreamSynchronize(s->copy_stream));
         free_stage_slots(s);
+        kept_cache_clear(s);                               /* segments keyed by addresses inside the old ring */
         s->stage_particles = stage_particles;
     }
     if (update_chunk) s->bin_chunk = update_chunk;
