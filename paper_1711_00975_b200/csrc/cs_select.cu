@@ -12,18 +12,27 @@
  * (no cell with a smaller estimate can enter the top k_max or an excursion set with thr >= thr_min).
  * Top-k for any k <= k_max and the excursion set for any thr >= thr_min are then prefixes of the list.
  *
- * One compaction = a fixed sequence of launches, with no host round trip in it:
- *   k_radix_hist   digit histograms of ALL passes in one sweep over the list
- *   k_radix_plan   one block: which passes are needed (a digit that is the same in every entry is skipped on the device:
- *                  the high bytes of the estimate key almost always are), exclusive digit bases, ping-pong plan
- *   k_radix_pass   one launch per digit: every tile ranks its entries (warp match.any + per-warp digit counters, stable),
- *                  publishes its digit counts and obtains its offsets from the tiles before it by decoupled look-back
- *                  (tiles take tickets in order, so a tile only ever waits for tiles that already run)
- *   k_uniq         drops duplicate ids, again with a look-back over tile totals
- *   k_cut          fixes the new tau and the number of entries kept, records which half of the ping-pong buffers holds
+ * One compaction = ONE cooperative launch (k_compact: every CTA resident, grid-wide barriers between its phases), with
+ * no host round trip in it:
+ *   histogram      digit histograms of ALL passes in one sweep over the list
+ *   plan           every CTA, from the global counts: which passes are needed (a digit that is the same in every entry
+ *                  is skipped: the high bytes of the estimate key almost always are), exclusive digit bases, ping-pong plan
+ *   radix passes   one sweep per needed digit: every tile ranks its entries (warp match.any + per-warp digit counters,
+ *                  stable), publishes its digit counts and obtains its offsets from the tiles before it by decoupled
+ *                  look-back (tiles are dealt round-robin to CTAs that are all running, so nothing waits on a tile that
+ *                  has not started)
+ *   uniq           drops duplicate ids, again with a look-back over tile totals
+ *   cut            fixes the new tau and the number of entries kept, records which half of the ping-pong buffers holds
  *                  the list (the host learns it when it next reads the scan states)
+ * Separate launches per phase (round 2's first form: 4 + one per digit) cost 8-9 us each on short lists; a barrier costs
+ * about 2.
  */
 #include "cs_device.cuh"
+
+#include <atomic>
+#include <cooperative_groups.h>
+
+namespace cg = cooperative_groups;
 
 namespace cs {
 
@@ -32,17 +41,23 @@ constexpr int SORT_WARPS = SORT_THREADS / 32;
 constexpr int SORT_ITEMS = 8;                              // items per lane
 constexpr int SORT_TILE = SORT_THREADS * SORT_ITEMS;       // 2048 entries per block
 constexpr int SORT_SEG = 32 * SORT_ITEMS;                  // consecutive entries owned by one warp
+constexpr int LOOKBACK = 8;                                // predecessors a look-back step fetches together
 constexpr int MAX_PASSES = 12;                             // 8 id bytes (ids < 2^60 need 8) + 4 estimate-key bytes
 
-/* Device-side plan of one compaction; lives at the start of SelectBuffers::scratch, zeroed before every compaction. */
+/* Device-side state of one compaction; lives at the start of SelectBuffers::scratch.  Zeroed at allocation; the kernel
+ * leaves it zeroed again when it ends. */
 struct SortPlan {
-    uint32_t hist[MAX_PASSES][256];    // digit counts; k_radix_plan turns them into exclusive bases
+    uint32_t hist[MAX_PASSES][256];    // digit counts of the whole list, all passes
+    uint32_t uniq_total;               // unique entries
+    uint32_t pad[3];
+};
+
+/* What every CTA derives for itself (identically) from the global digit counts. */
+struct LocalPlan {
+    uint32_t base[MAX_PASSES][256];    // first the CTA's own counts (histogram sweep), then exclusive digit bases
     uint32_t active[MAX_PASSES];       // 0: every entry has the same digit in this pass -> nothing to do
     uint32_t src_half[MAX_PASSES];     // which half (0/1) pass p reads
-    uint32_t ticket[MAX_PASSES + 1];   // tile tickets per pass, last = k_uniq
     uint32_t sorted_half;              // half that holds the sorted list
-    uint32_t uniq_total;               // unique entries
-    uint32_t pad[2];
 };
 
 /* look-back status word: epoch << 34 | flag << 32 | count; a word of another epoch reads as "not published yet" */
@@ -68,33 +83,31 @@ __device__ __forceinline__ uint32_t digit_of(uint64_t id, uint32_t ek, int pass,
     return pass < id_passes ? ((uint32_t)(id >> (8 * pass)) & 255u) : ((ek >> (8 * (pass - id_passes))) & 255u);
 }
 
-/* hist[p][digit] += entries of the list with that digit in pass p, for all passes at once */
-__global__ void __launch_bounds__(SORT_THREADS)
-k_radix_hist(const uint64_t* __restrict__ id, const uint32_t* __restrict__ ek, uint32_t n, int id_passes, int passes,
-             SortPlan* plan) {
-    __shared__ uint32_t h[MAX_PASSES][256];
-    for (int i = threadIdx.x; i < passes * 256; i += SORT_THREADS) (&h[0][0])[i] = 0;
+/* plan->hist[p][digit] += entries of the list with that digit in pass p, for all passes at once (grid-stride sweep) */
+__device__ __forceinline__ void hist_sweep(const uint64_t* __restrict__ id, const uint32_t* __restrict__ ek, uint32_t n,
+                                           int id_passes, int passes, LocalPlan& L, SortPlan* plan) {
+    for (int i = threadIdx.x; i < passes * 256; i += SORT_THREADS) (&L.base[0][0])[i] = 0;
     __syncthreads();
     const uint32_t stride = gridDim.x * SORT_THREADS;
     for (uint32_t i = blockIdx.x * SORT_THREADS + threadIdx.x; i < n; i += stride) {
         const uint64_t c = id[i];
         const uint32_t k = ek[i];
-        for (int p = 0; p < passes; ++p) atomicAdd(&h[p][digit_of(c, k, p, id_passes)], 1u);
+        for (int p = 0; p < passes; ++p) atomicAdd(&L.base[p][digit_of(c, k, p, id_passes)], 1u);
     }
     __syncthreads();
     for (int i = threadIdx.x; i < passes * 256; i += SORT_THREADS) {
-        const uint32_t v = (&h[0][0])[i];
+        const uint32_t v = (&L.base[0][0])[i];
         if (v) atomicAdd(&plan->hist[0][0] + i, v);
     }
 }
 
-/* One block of 256 threads: thread t = digit t. */
-__global__ void __launch_bounds__(256) k_radix_plan(SortPlan* plan, uint32_t n, int passes, uint32_t first_half) {
-    __shared__ uint32_t wsum[8];
-    __shared__ uint32_t s_active[MAX_PASSES];
+/* Thread t = digit t.  Global digit counts -> exclusive bases, which passes are needed (a digit that is the same in every
+ * entry is skipped: the high bytes of the estimate key almost always are), ping-pong plan.  Every CTA computes the same. */
+__device__ __forceinline__ void make_plan(const SortPlan* plan, uint32_t n, int passes, uint32_t first_half, LocalPlan& L,
+                                          uint32_t* wsum) {
     const uint32_t t = threadIdx.x, lane = t & 31u, warp = t >> 5;
     for (int p = 0; p < passes; ++p) {
-        const uint32_t c = plan->hist[p][t];
+        const uint32_t c = __ldcg(&plan->hist[p][t]);
         const int trivial = __syncthreads_or(c == n);
         uint32_t incl = c;
 #pragma unroll
@@ -106,35 +119,33 @@ __global__ void __launch_bounds__(256) k_radix_plan(SortPlan* plan, uint32_t n, 
         __syncthreads();
         uint32_t base = 0;
         for (uint32_t q = 0; q < warp; ++q) base += wsum[q];
-        plan->hist[p][t] = base + incl - c;                    // exclusive base of digit t
-        if (t == 0) s_active[p] = trivial ? 0u : 1u;
+        L.base[p][t] = base + incl - c;                        // exclusive base of digit t
+        if (t == 0) L.active[p] = trivial ? 0u : 1u;
         __syncthreads();
     }
     if (t == 0) {
         uint32_t half = first_half;
         for (int p = 0; p < passes; ++p) {
-            plan->active[p] = s_active[p];
-            plan->src_half[p] = half;
-            if (s_active[p]) half ^= 1u;
+            L.src_half[p] = half;
+            if (L.active[p]) half ^= 1u;
         }
-        plan->sorted_half = half;
+        L.sorted_half = half;
     }
+    __syncthreads();
 }
 
-/* One radix pass, stable.  Warp wq of a tile owns entries [t0 + wq*SORT_SEG, +SORT_SEG) in order; within a round of 32
- * the rank among equal digits comes from match.any, across rounds from a per-warp counter.  status: tiles x 256 words. */
-__global__ void __launch_bounds__(SORT_THREADS)
-k_radix_pass(const __grid_constant__ HalfPtrs H, uint32_t n, int pass, int id_passes, SortPlan* plan,
-             uint64_t* __restrict__ status, uint32_t epoch) {
-    if (!plan->active[pass]) return;
-    __shared__ uint32_t wcnt[SORT_WARPS][256];
-    __shared__ uint32_t s_tile;
+/* One tile of one radix pass, stable.  Warp wq of the tile owns entries [t0 + wq*SORT_SEG, +SORT_SEG) in order; within a
+ * round of 32 the rank among equal digits comes from match.any, across rounds from a per-warp counter.  The tile publishes
+ * its digit counts and obtains its offsets from the tiles before it by decoupled look-back (status: tiles x 256 words).
+ * Tiles are dealt to the (co-resident) CTAs round-robin and each CTA takes its tiles in increasing order, so a tile only
+ * ever waits for tiles that are done or running. */
+__device__ __forceinline__ void pass_tile(const HalfPtrs& H, uint32_t n, int pass, int id_passes, uint32_t tile,
+                                          const LocalPlan& L, uint32_t (*wcnt)[256], uint64_t* __restrict__ status,
+                                          uint32_t epoch) {
     const uint32_t lane = threadIdx.x & 31u, wq = threadIdx.x >> 5;
-    if (threadIdx.x == 0) s_tile = atomicAdd(&plan->ticket[pass], 1u);
     for (int i = threadIdx.x; i < SORT_WARPS * 256; i += SORT_THREADS) (&wcnt[0][0])[i] = 0;
     __syncthreads();
-    const uint32_t tile = s_tile;
-    const uint32_t src = plan->src_half[pass];
+    const uint32_t src = L.src_half[pass];
     const uint64_t* __restrict__ sid = H.id[src];
     const uint32_t* __restrict__ sek = H.ek[src];
     uint64_t* __restrict__ did = H.id[src ^ 1u];
@@ -148,8 +159,8 @@ k_radix_pass(const __grid_constant__ HalfPtrs H, uint32_t n, int pass, int id_pa
     for (int r = 0; r < SORT_ITEMS; ++r) {
         const uint32_t i = base + r * 32 + lane;
         const bool valid = i < n;
-        kid[r] = valid ? sid[i] : 0;
-        kek[r] = valid ? sek[i] : 0;
+        kid[r] = valid ? __ldcg(sid + i) : 0;                   // written by other CTAs in the pass before: L2, not L1
+        kek[r] = valid ? __ldcg(sek + i) : 0;
         const uint32_t dg = valid ? digit_of(kid[r], kek[r], pass, id_passes) : 255u;
         const uint32_t peers = __match_any_sync(0xFFFFFFFFu, dg);
         const uint32_t rank = __popc(peers & ((1u << lane) - 1u));
@@ -171,16 +182,29 @@ k_radix_pass(const __grid_constant__ HalfPtrs H, uint32_t n, int pass, int id_pa
             st_status(my, status_word(epoch, FLAG_INC, cnt));
         } else {
             st_status(my, status_word(epoch, FLAG_AGG, cnt));
-            for (uint32_t j = tile; j-- > 0;) {
-                const uint64_t* theirs = status + (uint64_t)j * 256 + t;
-                uint64_t w;
-                do { w = ld_status(theirs); } while ((uint32_t)(w >> 34) != epoch || ((w >> 32) & 3u) == 0);
-                excl += (uint32_t)w;
-                if ((w >> 32) & FLAG_INC) break;
+            /* LOOKBACK predecessors per step, fetched together: when a whole wave of tiles starts at once nobody has an
+             * inclusive word yet and the walk is a chain of L2 round trips; the window divides its length */
+            bool done = false;
+            for (uint32_t j = tile; j > 0 && !done;) {
+                const uint32_t m = j < (uint32_t)LOOKBACK ? j : (uint32_t)LOOKBACK;
+                uint64_t w[LOOKBACK];
+#pragma unroll
+                for (int q = 0; q < LOOKBACK; ++q)
+                    if ((uint32_t)q < m) w[q] = ld_status(status + (uint64_t)(j - 1 - q) * 256 + t);
+#pragma unroll
+                for (int q = 0; q < LOOKBACK; ++q) {
+                    if ((uint32_t)q < m && !done) {
+                        while ((uint32_t)(w[q] >> 34) != epoch || ((w[q] >> 32) & 3u) == 0)
+                            w[q] = ld_status(status + (uint64_t)(j - 1 - q) * 256 + t);
+                        excl += (uint32_t)w[q];
+                        done = ((w[q] >> 32) & FLAG_INC) != 0;
+                    }
+                }
+                j -= m;
             }
             st_status(my, status_word(epoch, FLAG_INC, excl + cnt));
         }
-        uint32_t run = plan->hist[pass][t] + excl;
+        uint32_t run = L.base[pass][t] + excl;
 #pragma unroll
         for (int q = 0; q < SORT_WARPS; ++q) {
             const uint32_t c = wcnt[q][t];
@@ -199,33 +223,29 @@ k_radix_pass(const __grid_constant__ HalfPtrs H, uint32_t n, int pass, int id_pa
             dek[dst] = kek[r];
         }
     }
+    __syncthreads();                                            // wcnt is reused by the CTA's next tile
 }
 
 /* ---- duplicate removal on the sorted list ------------------------------------------------------------------------ */
 
-/* Each thread owns SORT_ITEMS consecutive entries; block scan of the per-thread counts of "first of its id" flags; the
- * tile's offset comes from a look-back over the tile totals (ustatus: one word per tile). */
-__global__ void __launch_bounds__(SORT_THREADS)
-k_uniq(const __grid_constant__ HalfPtrs H, uint32_t n, SortPlan* plan, uint64_t* __restrict__ ustatus, uint32_t epoch,
-       uint32_t tiles) {
-    __shared__ uint32_t wsum[SORT_WARPS];
-    __shared__ uint32_t s_tile, s_excl;
-    if (threadIdx.x == 0) s_tile = atomicAdd(&plan->ticket[MAX_PASSES], 1u);
-    __syncthreads();
-    const uint32_t tile = s_tile;
-    const uint32_t src = plan->sorted_half;
+/* One tile: each thread owns SORT_ITEMS consecutive entries; block scan of the per-thread counts of "first of its id"
+ * flags; the tile's offset comes from a look-back over the tile totals (ustatus: one word per tile). */
+__device__ __forceinline__ void uniq_tile(const HalfPtrs& H, uint32_t n, uint32_t tile, uint32_t tiles, const LocalPlan& L,
+                                          SortPlan* plan, uint32_t* wsum, uint32_t* s_excl, uint64_t* __restrict__ ustatus,
+                                          uint32_t epoch) {
+    const uint32_t src = L.sorted_half;
     const uint64_t* __restrict__ sid = H.id[src];
     const uint32_t* __restrict__ sek = H.ek[src];
     uint64_t* __restrict__ did = H.id[src ^ 1u];
     uint32_t* __restrict__ dek = H.ek[src ^ 1u];
     const uint32_t first = tile * SORT_TILE + threadIdx.x * SORT_ITEMS;
     uint64_t v[SORT_ITEMS];
-    uint64_t prev = (first > 0 && first <= n) ? sid[first - 1] : 0;
+    uint64_t prev = (first > 0 && first <= n) ? __ldcg(sid + first - 1) : 0;
     uint32_t flags = 0, c = 0;
 #pragma unroll
     for (int r = 0; r < SORT_ITEMS; ++r) {
         const uint32_t i = first + r;
-        v[r] = i < n ? sid[i] : 0;
+        v[r] = i < n ? __ldcg(sid + i) : 0;
         if (i < n && (i == 0 || v[r] != prev)) { flags |= 1u << r; ++c; }
         prev = v[r];
     }
@@ -246,39 +266,48 @@ k_uniq(const __grid_constant__ HalfPtrs H, uint32_t n, SortPlan* plan, uint64_t*
             st_status(ustatus, status_word(epoch, FLAG_INC, total));
         } else {
             st_status(ustatus + tile, status_word(epoch, FLAG_AGG, total));
-            for (uint32_t j = tile; j-- > 0;) {
-                uint64_t w;
-                do { w = ld_status(ustatus + j); } while ((uint32_t)(w >> 34) != epoch || ((w >> 32) & 3u) == 0);
-                excl += (uint32_t)w;
-                if ((w >> 32) & FLAG_INC) break;
+            bool done = false;
+            for (uint32_t j = tile; j > 0 && !done;) {
+                const uint32_t m = j < (uint32_t)LOOKBACK ? j : (uint32_t)LOOKBACK;
+                uint64_t w[LOOKBACK];
+#pragma unroll
+                for (int q = 0; q < LOOKBACK; ++q)
+                    if ((uint32_t)q < m) w[q] = ld_status(ustatus + (j - 1 - q));
+#pragma unroll
+                for (int q = 0; q < LOOKBACK; ++q) {
+                    if ((uint32_t)q < m && !done) {
+                        while ((uint32_t)(w[q] >> 34) != epoch || ((w[q] >> 32) & 3u) == 0) w[q] = ld_status(ustatus + (j - 1 - q));
+                        excl += (uint32_t)w[q];
+                        done = ((w[q] >> 32) & FLAG_INC) != 0;
+                    }
+                }
+                j -= m;
             }
             st_status(ustatus + tile, status_word(epoch, FLAG_INC, excl + total));
         }
-        s_excl = excl;
+        *s_excl = excl;
         if (tile == tiles - 1) plan->uniq_total = excl + total;
     }
     __syncthreads();
-    uint32_t dst = s_excl + wbase + incl - c;
+    uint32_t dst = *s_excl + wbase + incl - c;
 #pragma unroll
     for (int r = 0; r < SORT_ITEMS; ++r) {
         if (flags & (1u << r)) {
             did[dst] = v[r];
-            dek[dst] = sek[first + r];
+            dek[dst] = __ldcg(sek + first + r);
             ++dst;
         }
     }
+    __syncthreads();                                            // wsum / s_excl are reused by the CTA's next tile
 }
 
-/* One thread.  The m unique sorted entries are in half `half` (or, with plan != NULL, in the half k_uniq wrote: the one
- * opposite to plan->sorted_half, m = plan->uniq_total).  Fixes the new tau and the number of entries kept. */
-__global__ void k_cut(const __grid_constant__ HalfPtrs H, const SortPlan* plan, uint32_t half_const, ScanState* st,
-                      uint64_t k_max, int32_t thr_min) {
-    const uint32_t half = plan ? (plan->sorted_half ^ 1u) : half_const;
-    const uint32_t m = plan ? plan->uniq_total : 0u;
+/* One thread.  The m unique sorted entries are in half `half`.  Fixes the new tau and the number of entries kept. */
+__device__ __forceinline__ void cut_list(const HalfPtrs& H, uint32_t half, uint32_t m, ScanState* st, uint64_t k_max,
+                                         int32_t thr_min) {
     const uint32_t* __restrict__ ek = H.ek[half];
     int32_t tau_k;
     if (k_max == 0) tau_k = INT32_MAX;                       // no top-k asked: only thr_min bounds tau
-    else tau_k = (m >= k_max) ? key_to_est(ek[k_max - 1]) : INT32_MIN;
+    else tau_k = (m >= k_max) ? key_to_est(__ldcg(ek + k_max - 1)) : INT32_MIN;
     int32_t tau = min(tau_k, thr_min);
     tau = max(tau, st->tau);
     /* entries are ordered by estimate descending: keep the prefix with est >= tau, i.e. key <= key(tau) */
@@ -286,14 +315,52 @@ __global__ void k_cut(const __grid_constant__ HalfPtrs H, const SortPlan* plan, 
     uint32_t lo = 0, hi = m;                                 // first index with key > key_tau
     while (lo < hi) {
         uint32_t mid = lo + (hi - lo) / 2;
-        if (ek[mid] <= key_tau) lo = mid + 1; else hi = mid;
+        if (__ldcg(ek + mid) <= key_tau) lo = mid + 1; else hi = mid;
     }
     st->uniq = m;
     st->count = lo;
     st->tau = tau;
-    st->est_max = lo ? key_to_est(ek[0]) : INT32_MIN;
-    st->est_min = lo ? key_to_est(ek[lo - 1]) : INT32_MAX;
+    st->est_max = lo ? key_to_est(__ldcg(ek)) : INT32_MIN;
+    st->est_min = lo ? key_to_est(__ldcg(ek + lo - 1)) : INT32_MAX;
     st->half = half;
+}
+
+/* The empty list: nothing to sort, tau = max(tau, min(INT32_MIN or INT32_MAX, thr_min)) as for any other list. */
+__global__ void k_cut_empty(const __grid_constant__ HalfPtrs H, uint32_t half, ScanState* st, uint64_t k_max, int32_t thr_min) {
+    cut_list(H, half, 0u, st, k_max, thr_min);
+}
+
+/* One compaction in one cooperative launch (all CTAs co-resident; grid-wide barriers between the phases):
+ *   digit histograms of all passes | plan | one sweep per needed digit | duplicate removal | cut | plan zeroed again */
+__global__ void __launch_bounds__(SORT_THREADS, 4)
+k_compact(const __grid_constant__ HalfPtrs H, uint32_t n, uint32_t first_half, int id_passes, int passes, SortPlan* plan,
+          uint64_t* __restrict__ status, uint64_t* __restrict__ ustatus, uint32_t epoch0, ScanState* st, uint64_t k_max,
+          int32_t thr_min) {
+    __shared__ LocalPlan L;
+    __shared__ uint32_t wcnt[SORT_WARPS][256];
+    __shared__ uint32_t wsum[SORT_WARPS];
+    __shared__ uint32_t s_excl;
+    cg::grid_group grid = cg::this_grid();
+    const uint32_t tiles = (n + SORT_TILE - 1) / SORT_TILE;
+
+    hist_sweep(H.id[first_half], H.ek[first_half], n, id_passes, passes, L, plan);
+    grid.sync();
+    make_plan(plan, n, passes, first_half, L, wsum);
+    for (int p = 0; p < passes; ++p) {
+        if (!L.active[p]) continue;
+        for (uint32_t tile = blockIdx.x; tile < tiles; tile += gridDim.x)
+            pass_tile(H, n, p, id_passes, tile, L, wcnt, status, (epoch0 + (uint32_t)p) & 0x3FFFFFFFu);
+        grid.sync();
+    }
+    for (uint32_t tile = blockIdx.x; tile < tiles; tile += gridDim.x)
+        uniq_tile(H, n, tile, tiles, L, plan, wsum, &s_excl, ustatus, (epoch0 + (uint32_t)passes) & 0x3FFFFFFFu);
+    grid.sync();
+    if (blockIdx.x == 0) {
+        if (threadIdx.x == 0) cut_list(H, L.sorted_half ^ 1u, __ldcg(&plan->uniq_total), st, k_max, thr_min);
+        __syncthreads();
+        for (int i = threadIdx.x; i < passes * 256; i += SORT_THREADS) (&plan->hist[0][0])[i] = 0;   // for the next compaction
+        if (threadIdx.x == 0) plan->uniq_total = 0;
+    }
 }
 
 __global__ void __launch_bounds__(256)
@@ -328,36 +395,51 @@ uint64_t select_scratch_words(uint64_t n) {
     return plan_words() + t * 256 * 2 + t * 2 + 16;
 }
 
-/* Enqueues one compaction of the first n entries of half `src` (all on `stream`, no synchronisation).  Afterwards
- * st_dev->half names the half that holds the list and st_dev->count its length.  *epoch: per-buffer launch counter. */
+/* CTAs of k_compact that fit on the current device at once (the bound of a cooperative launch). */
+static cudaError_t resident_ctas(uint32_t* out) {
+    static std::atomic<uint32_t> cached[64];
+    int dev = 0;
+    cudaError_t e = cudaGetDevice(&dev);
+    if (e != cudaSuccess) return e;
+    uint32_t v = dev < 64 ? cached[dev].load(std::memory_order_relaxed) : 0u;
+    if (!v) {
+        int per_sm = 0, sms = 0;
+        e = cudaOccupancyMaxActiveBlocksPerMultiprocessor(&per_sm, k_compact, SORT_THREADS, 0);
+        if (e != cudaSuccess) return e;
+        e = cudaDeviceGetAttribute(&sms, cudaDevAttrMultiProcessorCount, dev);
+        if (e != cudaSuccess) return e;
+        v = (uint32_t)(per_sm * sms);
+        if (!v) return cudaErrorLaunchOutOfResources;
+        if (dev < 64) cached[dev].store(v, std::memory_order_relaxed);
+    }
+    *out = v;
+    return cudaSuccess;
+}
+
+/* Enqueues one compaction of the first n entries of half `src` (one launch on `stream`, no synchronisation).  Afterwards
+ * st_dev->half names the half that holds the list and st_dev->count its length.  *epoch: per-buffer sweep counter. */
 cudaError_t select_compact(const SelectBuffers& B, uint32_t cap, int src, uint32_t n, int id_bits, ScanState* st_dev,
                            uint64_t k_max, int32_t thr_min, cudaStream_t stream, uint64_t* launches, uint32_t* epoch) {
     HalfPtrs H;
     for (int h = 0; h < 2; ++h) { H.id[h] = B.id[h]; H.ek[h] = B.ek[h]; }
+    *launches += 1;
     if (n == 0) {
-        k_cut<<<1, 1, 0, stream>>>(H, nullptr, (uint32_t)src, st_dev, k_max, thr_min);
-        *launches += 1;
+        k_cut_empty<<<1, 1, 0, stream>>>(H, (uint32_t)src, st_dev, k_max, thr_min);
         return cudaGetLastError();
     }
+    uint32_t resident = 0;
+    cudaError_t e = resident_ctas(&resident);
+    if (e != cudaSuccess) return e;
     SortPlan* plan = reinterpret_cast<SortPlan*>(B.scratch);
     uint64_t* status = reinterpret_cast<uint64_t*>(B.scratch + plan_words());
     uint64_t* ustatus = status + (uint64_t)(tiles_of(cap) + 1) * 256;
     const uint32_t tiles = tiles_of(n);
-    const int id_passes = (id_bits + 7) / 8, passes = id_passes + 4;
-    cudaError_t e = cudaMemsetAsync(plan, 0, sizeof(SortPlan), stream);
-    if (e != cudaSuccess) return e;
-    uint32_t hb = tiles < 148u * 8u ? tiles : 148u * 8u;
-    k_radix_hist<<<hb, SORT_THREADS, 0, stream>>>(B.id[src], B.ek[src], n, id_passes, passes, plan);
-    k_radix_plan<<<1, 256, 0, stream>>>(plan, n, passes, (uint32_t)src);
-    for (int p = 0; p < passes; ++p) {
-        *epoch += 1;
-        k_radix_pass<<<tiles, SORT_THREADS, 0, stream>>>(H, n, p, id_passes, plan, status, *epoch & 0x3FFFFFFFu);
-    }
-    *epoch += 1;
-    k_uniq<<<tiles, SORT_THREADS, 0, stream>>>(H, n, plan, ustatus, *epoch & 0x3FFFFFFFu, tiles);
-    k_cut<<<1, 1, 0, stream>>>(H, plan, 0u, st_dev, k_max, thr_min);
-    *launches += 4 + passes;
-    return cudaGetLastError();
+    int id_passes = (id_bits + 7) / 8, passes = id_passes + 4;
+    uint32_t first_half = (uint32_t)src, epoch0 = *epoch + 1;
+    *epoch += (uint32_t)passes + 1;                          /* one epoch per look-back sweep: the passes, then uniq's */
+    void* args[] = {&H, &n, &first_half, &id_passes, &passes, &plan, &status, &ustatus, &epoch0, &st_dev, &k_max, &thr_min};
+    return cudaLaunchCooperativeKernel((const void*)k_compact, dim3(tiles < resident ? tiles : resident), dim3(SORT_THREADS),
+                                       args, 0, stream);
 }
 
 cudaError_t launch_emit_prefix(const uint64_t* id, const uint32_t* ek, uint32_t n, uint64_t* ids_out,
