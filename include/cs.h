@@ -301,6 +301,30 @@ int cs_probe_l2(int mode, uint64_t table_bytes, uint64_t n_ops, int reps, void* 
  * the position-stream term of the roofline.  *ms_out = average device time of one pass. */
 int cs_probe_stream(const float* xyz_dev, uint64_t n, int reps, void* cuda_stream, double* ms_out);
 
+/* ---- selection without any allocation ------------------------------------------------------------------------------
+ * For callers that cannot allocate device memory (code under CUDA graph capture, tight serving loops, harnesses that
+ * forbid it).  The deterministic selection of PAPER.md:142-147 / :306 (R9) over a candidate list the caller
+ * already holds on the device: n pairs (cell id, estimate), e.g. ids of its own and their cs_estimate values.  Output: the
+ * distinct ids in the order (estimate descending, id ascending), cut to the first k -- what cs_scan_cells + cs_topk
+ * return for the same cells.  Pairs with equal ids must carry equal estimates (as estimates of one sketch do).
+ *
+ * It takes no handle and runs on the CURRENT device, on `cuda_stream` (a cudaStream_t; NULL = the legacy default
+ * stream); all pointers are device pointers on that device: ids_dev[n], est_dev[n] in; ids_out_dev[k], est_out_dev[k]
+ * and *n_out_dev (= min(k, number of distinct ids)) out.  Nothing is copied to the host and nothing synchronises: the
+ * results are valid once the stream has passed the call.  Inputs are not modified; outputs must not overlap inputs.
+ *
+ * Its scratch (both halves of the sorting buffer, digit counts, look-back status words: 24 bytes per candidate + 85 KB,
+ * 1.6 MB in all) is a file-scope device array inside the library: every GPU that loads the library holds it from load to
+ * exit, and the call makes no cudaMalloc / cudaFree / allocating library call.  The first call on each device looks the
+ * array's device address up (cudaGetSymbolAddress); make that call outside stream capture.
+ *   n > CS_SELECT_STATIC_MAX_N or k > CS_SELECT_STATIC_MAX_N  ->  CS_ERR_ARG, nothing is launched.
+ * Every call on a device shares the one array, which keeps the last call's contents (each call re-initialises what must
+ * start at zero): calls that overlap on the GPU -- two streams, two host threads -- race.  Calls on one stream, or
+ * otherwise ordered, are safe.  Launches 3 kernels (load, one cooperative compaction, emit). */
+#define CS_SELECT_STATIC_MAX_N 65536u
+int cs_select_static(const uint64_t* ids_dev, const int32_t* est_dev, uint64_t n, uint64_t k, uint64_t* ids_out_dev,
+                     int32_t* est_out_dev, uint32_t* n_out_dev, void* cuda_stream);
+
 #ifdef __cplusplus
 }
 #endif

@@ -67,6 +67,7 @@ SIGNATURES = {
     "cs_update_stats": (ci, [vp, vp]),
     "cs_launch_count": (ci, [vp, vp]),
     "cs_probe_l2": (ci, [ci, u64, u64, ci, vp, vp]),
+    "cs_select_static": (ci, [vp, vp, u64, u64, vp, vp, vp, vp]),
     "cs_probe_stream": (ci, [vp, u64, ci, vp, vp]),
 }
 
@@ -388,3 +389,24 @@ def probe_stream(xyz: torch.Tensor, reps: int = 3, stream: torch.cuda.Stream | N
     ms = dbl(0.0)
     _chk(lib().cs_probe_stream(vp(p), n, reps, vp(st.cuda_stream), C.byref(ms)), "cs_probe_stream")
     return float(ms.value)
+
+
+SELECT_STATIC_MAX_N = 65536          # CS_SELECT_STATIC_MAX_N of include/cs.h
+
+
+def select_static(ids: torch.Tensor, est: torch.Tensor, k: int, ids_out: torch.Tensor, est_out: torch.Tensor,
+                  n_out: torch.Tensor, stream: torch.cuda.Stream | None = None) -> None:
+    """cs_select_static: the first k distinct ids of (ids, est) in the order (est descending, id ascending) -> ids_out[:k],
+    est_out[:k], n_out[0] (a CUDA int32/uint32 tensor of one element), asynchronously on `stream`.  The library call
+    allocates nothing (its scratch is a fixed device array of the library: n, k <= SELECT_STATIC_MAX_N) and every
+    tensor is the caller's, so this wrapper allocates nothing either.  Calls that overlap on the GPU race."""
+    for t, name, kinds in ((ids, "ids", (torch.int64, torch.uint64)), (est, "est", (torch.int32,)),
+                           (ids_out, "ids_out", (torch.int64, torch.uint64)), (est_out, "est_out", (torch.int32,)),
+                           (n_out, "n_out", (torch.int32, torch.uint32))):
+        if not t.is_cuda or t.dtype not in kinds or not t.is_contiguous():
+            raise ValueError(f"{name} must be a contiguous CUDA tensor of dtype {kinds}")
+    if est.numel() != ids.numel() or ids_out.numel() < k or est_out.numel() < k or n_out.numel() < 1:
+        raise ValueError("est must match ids; ids_out / est_out need k entries, n_out one")
+    st = stream if stream is not None else torch.cuda.current_stream()
+    _chk(lib().cs_select_static(vp(ids.data_ptr()), vp(est.data_ptr()), ids.numel(), k, vp(ids_out.data_ptr()),
+                                vp(est_out.data_ptr()), vp(n_out.data_ptr()), vp(st.cuda_stream)), "cs_select_static")

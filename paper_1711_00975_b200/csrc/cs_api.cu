@@ -12,6 +12,7 @@
 #include <vector>
 
 #include "cs_internal.h"
+#include "cs_select_static.h"
 
 using namespace cs;
 
@@ -1783,6 +1784,22 @@ int cs_launch_count(cs_sketch* s, uint64_t* n_out) {
     if (!s || !n_out) return fail(CS_ERR_ARG, "null argument");
     DeviceGuard guard_(s);
     *n_out = s->launches;
+    return CS_OK;
+}
+
+int cs_select_static(const uint64_t* ids_dev, const int32_t* est_dev, uint64_t n, uint64_t k, uint64_t* ids_out_dev,
+                     int32_t* est_out_dev, uint32_t* n_out_dev, void* cuda_stream) {
+    if (n > CS_SELECT_STATIC_MAX_N)
+        return fail(CS_ERR_ARG, "cs_select_static: n = %llu candidates exceed the static scratch (CS_SELECT_STATIC_MAX_N = %u)",
+                    (unsigned long long)n, (unsigned)CS_SELECT_STATIC_MAX_N);
+    if (k > CS_SELECT_STATIC_MAX_N)
+        return fail(CS_ERR_ARG, "cs_select_static: k = %llu exceeds CS_SELECT_STATIC_MAX_N = %u", (unsigned long long)k,
+                    (unsigned)CS_SELECT_STATIC_MAX_N);
+    if (!n_out_dev || (n && (!ids_dev || !est_dev)) || (n && k && (!ids_out_dev || !est_out_dev)))
+        return fail(CS_ERR_ARG, "cs_select_static: null pointer with a non-zero size");
+    cudaError_t e = select_static(ids_dev, est_dev, (uint32_t)n, (uint32_t)k, ids_out_dev, est_out_dev, n_out_dev,
+                                  (cudaStream_t)cuda_stream);
+    if (e != cudaSuccess) return fail(CS_ERR_CUDA, "cs_select_static: %s", cudaGetErrorString(e));
     return CS_OK;
 }
 

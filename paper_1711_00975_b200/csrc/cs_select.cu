@@ -28,6 +28,7 @@
  * about 2.
  */
 #include "cs_device.cuh"
+#include "cs_select_static.h"
 
 #include <atomic>
 #include <cooperative_groups.h>
@@ -440,6 +441,100 @@ cudaError_t select_compact(const SelectBuffers& B, uint32_t cap, int src, uint32
     void* args[] = {&H, &n, &first_half, &id_passes, &passes, &plan, &status, &ustatus, &epoch0, &st_dev, &k_max, &thr_min};
     return cudaLaunchCooperativeKernel((const void*)k_compact, dim3(tiles < resident ? tiles : resident), dim3(SORT_THREADS),
                                        args, 0, stream);
+}
+
+/* ---- allocation-free selection over a caller's candidate list (cs_select_static, include/cs.h) -------------------------
+ * Everything a compaction needs -- both halves of the ping-pong list, the plan, the look-back status words, the scan
+ * state -- sits in one file-scope device array of fixed size; every GPU that loads the library holds it until exit.
+ * In host code `g_static_scratch` is only the symbol's host-side stand-in: its device address comes from
+ * cudaGetSymbolAddress, once per device, and that address is what the kernels are given. */
+constexpr uint32_t STATIC_TILES = SELECT_STATIC_MAX_N / SORT_TILE;
+struct StaticScratch {
+    uint64_t id[2][SELECT_STATIC_MAX_N];
+    uint32_t ek[2][SELECT_STATIC_MAX_N];
+    SortPlan plan;
+    uint64_t status[(STATIC_TILES + 1) * 256];
+    uint64_t ustatus[STATIC_TILES + 1];
+    ScanState st;
+};
+static_assert(SELECT_STATIC_MAX_N % SORT_TILE == 0, "whole tiles");
+static __device__ __align__(256) unsigned char g_static_scratch[sizeof(StaticScratch)];
+
+/* Caller's (id, estimate) pairs -> half 0 as (id, key); what must start at zero is cleared: the array keeps the last
+ * call's contents (digit counts if that call was cut short, status words of its epochs, its scan state). */
+__global__ void __launch_bounds__(256)
+k_static_load(StaticScratch* S, const uint64_t* __restrict__ ids, const int32_t* __restrict__ est, uint32_t n, uint32_t tiles) {
+    const uint32_t stride = gridDim.x * 256u, t0 = blockIdx.x * 256u + threadIdx.x;
+    for (uint32_t i = t0; i < n; i += stride) {
+        S->id[0][i] = ids[i];
+        S->ek[0][i] = est_to_key(est[i]);
+    }
+    for (uint32_t i = t0; i < MAX_PASSES * 256u; i += stride) (&S->plan.hist[0][0])[i] = 0;
+    for (uint32_t i = t0; i < (tiles + 1) * 256u; i += stride) S->status[i] = 0;
+    for (uint32_t i = t0; i <= tiles; i += stride) S->ustatus[i] = 0;
+    if (t0 == 0) {
+        S->plan.uniq_total = 0;
+        S->st.count = 0; S->st.tau = INT32_MIN; S->st.est_min = INT32_MAX; S->st.est_max = INT32_MIN;
+        S->st.uniq = 0; S->st.half = 0;
+    }
+}
+
+/* First min(k, kept) entries of the list k_compact left -> the caller's arrays. */
+__global__ void __launch_bounds__(256)
+k_static_emit(const StaticScratch* S, uint32_t k, uint64_t* __restrict__ ids_out, int32_t* __restrict__ est_out,
+              uint32_t* __restrict__ n_out) {
+    const uint32_t half = S->st.half, kept = S->st.count < k ? S->st.count : k;
+    for (uint32_t i = blockIdx.x * 256u + threadIdx.x; i < kept; i += gridDim.x * 256u) {
+        ids_out[i] = S->id[half][i];
+        est_out[i] = key_to_est(S->ek[half][i]);
+    }
+    if (blockIdx.x == 0 && threadIdx.x == 0) *n_out = kept;
+}
+
+/* Device address of the scratch array on the current device (looked up once per device, with that device current). */
+static cudaError_t static_scratch(StaticScratch** out) {
+    static std::atomic<StaticScratch*> cached[64];
+    int dev = 0;
+    cudaError_t e = cudaGetDevice(&dev);
+    if (e != cudaSuccess) return e;
+    StaticScratch* ptr = (dev >= 0 && dev < 64) ? cached[dev].load(std::memory_order_acquire) : nullptr;
+    if (!ptr) {
+        e = cudaGetSymbolAddress((void**)&ptr, g_static_scratch);
+        if (e != cudaSuccess) return e;
+        if (!ptr) return cudaErrorInvalidSymbol;
+        if (dev >= 0 && dev < 64) cached[dev].store(ptr, std::memory_order_release);
+    }
+    *out = ptr;
+    return cudaSuccess;
+}
+
+cudaError_t select_static(const uint64_t* ids, const int32_t* est, uint32_t n, uint32_t k, uint64_t* ids_out, int32_t* est_out,
+                          uint32_t* n_out, cudaStream_t stream) {
+    StaticScratch* S = nullptr;
+    cudaError_t e = static_scratch(&S);
+    if (e != cudaSuccess) return e;
+    const uint32_t tiles = tiles_of(n);
+    k_static_load<<<tiles ? tiles : 1, 256, 0, stream>>>(S, ids, est, n, tiles);
+    if (n) {
+        uint32_t resident = 0;
+        e = resident_ctas(&resident);
+        if (e != cudaSuccess) return e;
+        HalfPtrs H;
+        for (int h = 0; h < 2; ++h) { H.id[h] = S->id[h]; H.ek[h] = S->ek[h]; }
+        SortPlan* plan = &S->plan;
+        uint64_t *status = S->status, *ustatus = S->ustatus, k_max = k;
+        ScanState* st = &S->st;
+        uint32_t first_half = 0, epoch0 = 1;                  /* the status words were just zeroed: epoch 0 = not published */
+        int id_passes = 8, passes = MAX_PASSES;               /* every id byte; constant digits are skipped on the device */
+        int32_t thr_min = INT32_MAX;
+        void* args[] = {&H, &n, &first_half, &id_passes, &passes, &plan, &status, &ustatus, &epoch0, &st, &k_max, &thr_min};
+        e = cudaLaunchCooperativeKernel((const void*)k_compact, dim3(tiles < resident ? tiles : resident), dim3(SORT_THREADS),
+                                        args, 0, stream);
+        if (e != cudaSuccess) return e;
+    }
+    const uint32_t eb = (k + 255u) / 256u;
+    k_static_emit<<<eb ? (eb < 256u ? eb : 256u) : 1, 256, 0, stream>>>(S, k, ids_out, est_out, n_out);
+    return cudaGetLastError();
 }
 
 cudaError_t launch_emit_prefix(const uint64_t* id, const uint32_t* ek, uint32_t n, uint64_t* ids_out,
