@@ -8,6 +8,11 @@ For every kernel launch in the reports it writes profiles/<tag>_ncu_<kernel>.csv
 profiles/<tag>_kernel_metrics.json, which bench.py reads for `roofline.traffic` and the instruction count per particle.
 The json records the hash of the kernel sources it was captured on (bench.kernel_sources_sha); bench.py ignores it
 once those sources change.  Needs `ncu` on PATH (reading a report needs no GPU).  Not imported by the library.
+
+    python -m paper_1711_00975_b200.profile_capture --launch-list gpurun_out/r2_launches_cfg3.csv profiles/r2_launches_cfg3_last_step.csv
+
+turns the launch list of `ncu --metrics gpu__time_duration.sum --csv --log-file <raw> ... bench.py` into the rows of the
+last step and prints the per-kernel summary.
 """
 from __future__ import annotations
 
@@ -48,7 +53,50 @@ def short_name(full: str) -> str:
     return re.sub(r"[^A-Za-z0-9_]+", "_", name).strip("_")
 
 
+UPDATE_KERNELS = ("k_bin_scatter", "k_bin_apply", "k_update", "k_compact_kept")
+
+
+def launch_list(raw_csv: Path, out_csv: Path):
+    """`ncu --metrics gpu__time_duration.sum --csv --log-file raw_csv ... bench.py` -> the launches of the LAST step (a step
+    starts where an update kernel follows a kernel of the scan / select phases), one row per launch, and a per-kernel
+    summary (markdown) on stdout.  The probe kernels bench.py runs for its denominators are left out."""
+    lines = [l for l in raw_csv.read_text().splitlines() if l.startswith('"')]
+    rows = list(csv.DictReader(lines))
+    seq = []
+    for r in rows:
+        if r["Metric Name"] != "gpu__time_duration.sum":
+            continue
+        name = re.sub(r"^void\s+", "", r["Kernel Name"])
+        name = re.sub(r"\(.*$", "", name).replace("cs::", "").replace("(anonymous namespace)::", "")
+        if name.startswith("k_probe"):
+            continue
+        ns = float(r["Metric Value"]) * {"ns": 1.0, "us": 1e3, "ms": 1e6, "s": 1e9}[r["Metric Unit"]]
+        seq.append((name, ns))
+    starts = [i for i, (nm, _) in enumerate(seq)
+              if nm.startswith(UPDATE_KERNELS) and (i == 0 or not seq[i - 1][0].startswith(UPDATE_KERNELS))]
+    last = seq[starts[-1]:] if starts else seq
+    with open(out_csv, "w", newline="") as f:
+        w = csv.writer(f)
+        w.writerow(["launch", "kernel", "gpu__time_duration.sum [ns]"])
+        for i, (nm, ns) in enumerate(last):
+            w.writerow([i, nm, int(round(ns))])
+    agg = {}
+    for nm, ns in last:
+        c, t = agg.get(nm, (0, 0.0))
+        agg[nm] = (c + 1, t + ns)
+    total = sum(t for _, t in agg.values())
+    print(f"steps found: {len(starts)}; last step: {len(last)} launches, {total / 1e6:.3f} ms under ncu\n")
+    print("| Kernel | Launches | Total ms (ncu) | Share |\n|---|---|---|---|")
+    for nm, (c, t) in sorted(agg.items(), key=lambda kv: -kv[1][1]):
+        print(f"| `{nm}` | {c} | {t / 1e6:.3f} | {100 * t / total:.1f} % |")
+    print(f"| sum | {len(last)} | {total / 1e6:.2f} | |")
+    print("wrote", out_csv)
+
+
 def main():
+    if len(sys.argv) > 1 and sys.argv[1] == "--launch-list":
+        launch_list(Path(sys.argv[2]), Path(sys.argv[3]))
+        return
     ap = argparse.ArgumentParser()
     ap.add_argument("reports", nargs="+")
     ap.add_argument("--tag", default="r2")
