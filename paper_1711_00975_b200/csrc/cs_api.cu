@@ -1142,6 +1142,10 @@ int cs_create_multi(cs_sketch** out, int n_scales, int d, uint64_t w, const uint
     cs_sketch* s = new (std::nothrow) cs_sketch();
     if (!s) return fail(CS_ERR_NOMEM, "host allocation failed");
     s->d = d; s->n_scales = n_scales; s->w = w; s->L = L; s->seed = seed; s->device = dev;
+    /* the selector's 30-bit look-back epochs start three compactions short of where they are rewound (cs_select.cu), so
+     * that every handle that lives that long takes the rewind once, early: a path that otherwise runs after ~10^8
+     * compactions would never be exercised */
+    for (int i = 0; i < n_scales; ++i) s->epoch[i] = 0x3FFFFFFFu - 64u;
     int sm = 0;
     if (cudaDeviceGetAttribute(&sm, cudaDevAttrMultiProcessorCount, dev) == cudaSuccess && sm > 0) s->sm_count = sm;
 

@@ -417,6 +417,17 @@ static cudaError_t resident_ctas(uint32_t* out) {
     return cudaSuccess;
 }
 
+/* k_compact works with any grid that is resident at once (tiles are dealt round-robin).  Where fewer CTAs fit than the
+ * occupancy calculation says (a context restricted to part of the SMs), the launch is refused: halve and retry. */
+static cudaError_t launch_cooperative(uint32_t grid, void** args, cudaStream_t stream) {
+    for (;;) {
+        cudaError_t e = cudaLaunchCooperativeKernel((const void*)k_compact, dim3(grid), dim3(SORT_THREADS), args, 0, stream);
+        if (e != cudaErrorCooperativeLaunchTooLarge || grid == 1) return e;
+        cudaGetLastError();
+        grid /= 2;
+    }
+}
+
 /* Enqueues one compaction of the first n entries of half `src` (one launch on `stream`, no synchronisation).  Afterwards
  * st_dev->half names the half that holds the list and st_dev->count its length.  *epoch: per-buffer sweep counter. */
 cudaError_t select_compact(const SelectBuffers& B, uint32_t cap, int src, uint32_t n, int id_bits, ScanState* st_dev,
@@ -436,11 +447,15 @@ cudaError_t select_compact(const SelectBuffers& B, uint32_t cap, int src, uint32
     uint64_t* ustatus = status + (uint64_t)(tiles_of(cap) + 1) * 256;
     const uint32_t tiles = tiles_of(n);
     int id_passes = (id_bits + 7) / 8, passes = id_passes + 4;
+    if (*epoch >= 0x3FFFFFFFu - 2u * MAX_PASSES) {           /* epochs are 30 bits wide: before they repeat, forget every */
+        e = cudaMemsetAsync(B.scratch, 0, (size_t)select_scratch_words(cap) * sizeof(uint32_t), stream);   /* word written */
+        if (e != cudaSuccess) return e;
+        *epoch = 0;
+    }
     uint32_t first_half = (uint32_t)src, epoch0 = *epoch + 1;
     *epoch += (uint32_t)passes + 1;                          /* one epoch per look-back sweep: the passes, then uniq's */
     void* args[] = {&H, &n, &first_half, &id_passes, &passes, &plan, &status, &ustatus, &epoch0, &st_dev, &k_max, &thr_min};
-    return cudaLaunchCooperativeKernel((const void*)k_compact, dim3(tiles < resident ? tiles : resident), dim3(SORT_THREADS),
-                                       args, 0, stream);
+    return launch_cooperative(tiles < resident ? tiles : resident, args, stream);
 }
 
 /* ---- allocation-free selection over a caller's candidate list (cs_select_static, include/cs.h) -------------------------
@@ -528,8 +543,7 @@ cudaError_t select_static(const uint64_t* ids, const int32_t* est, uint32_t n, u
         int id_passes = 8, passes = MAX_PASSES;               /* every id byte; constant digits are skipped on the device */
         int32_t thr_min = INT32_MAX;
         void* args[] = {&H, &n, &first_half, &id_passes, &passes, &plan, &status, &ustatus, &epoch0, &st, &k_max, &thr_min};
-        e = cudaLaunchCooperativeKernel((const void*)k_compact, dim3(tiles < resident ? tiles : resident), dim3(SORT_THREADS),
-                                        args, 0, stream);
+        e = launch_cooperative(tiles < resident ? tiles : resident, args, stream);
         if (e != cudaSuccess) return e;
     }
     const uint32_t eb = (k + 255u) / 256u;
