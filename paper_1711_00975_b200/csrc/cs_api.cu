@@ -325,7 +325,7 @@ bool bad_p(double p) { return !(p > 0.0) || p > 1.0; }
 
 constexpr uint32_t BIN_MAX = 4096;                    /* bins per pass (words of `cursor`) */
 constexpr uint64_t BIN_MIN_N = 1ull << 22;            /* auto mode: below this the direct kernel is as fast */
-constexpr size_t BIN_SMEM = 216 * 1024;               /* shared memory of one scatter CTA (6 pairs per round at cfg 3: 209 KB) */
+constexpr size_t BIN_SMEM = 216 * 1024;               /* shared memory of one scatter CTA (8 pairs per round at cfg 3: 211 KB) */
 
 struct BinPlan {
     uint32_t log2w, log2S, SL, C, threads;
@@ -336,7 +336,10 @@ int ilog2(uint64_t v) { return bit_length(v) - 1; }
 
 uint32_t staging_capacity(uint32_t threads, uint32_t SL) {
     const double lambda = 2.0 * SCATTER_PAIRS_PER_ROUND * threads / SL;    /* records per bin, round and CTA */
-    uint32_t C = (uint32_t)(32.0 + lambda + 6.0 * std::sqrt(lambda) + 8.0);
+    /* up to 31 records left from the round before + this round's arrivals (Poisson, mean lambda) + 3 sigma: the few
+     * records beyond (measured 3e-8 of all at cfg 3) take the red.global route.  Sized at 6 sigma the same shared memory
+     * holds 6 pairs per round instead of 8, and the flush phases between rounds are what the extra pairs save. */
+    uint32_t C = (uint32_t)(32.0 + lambda + 3.0 * std::sqrt(lambda) + 8.0);
     C = (C + 7u) & ~7u;
     return C > 256 ? 256 : C;                          /* beyond: staging overflows go through red.global */
 }

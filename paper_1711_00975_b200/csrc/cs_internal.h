@@ -122,7 +122,7 @@ struct BinParams {
     unsigned long long* stats;  // 4 counters (may be NULL): records that left the binned route -- [0] staging buffer full,
                                 // [1] bin region full, [2] leftovers of partial buffers at kernel end; [3] records binned
 };
-constexpr int SCATTER_PAIRS_PER_ROUND = 6;      // pairs of particles per thread between two flush phases of k_bin_scatter
+constexpr int SCATTER_PAIRS_PER_ROUND = 8;      // pairs of particles per thread between two flush phases of k_bin_scatter
 size_t scatter_smem_bytes(uint32_t nb, uint32_t C);
 cudaError_t launch_update_binned(const PassParams& P, const BinParams& B, const float* xyz, uint64_t n, int sm_count,
                                  cudaStream_t st, PhaseTimer* tm);
