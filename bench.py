@@ -75,20 +75,29 @@ def load_capture(workload: str):
 
 
 class ClockSampler:
-    """nvidia-smi clocks / throttle reasons sampled DURING the timed region."""
-    Q = ("clocks.sm,clocks.max.sm,power.draw,clocks_event_reasons.hw_slowdown,"
+    """nvidia-smi clocks / throttle reasons sampled DURING the timed region.  power.draw is not queried: with it, about one
+    run in eight of cfg 5 (5 steps of 20 ms) had a step stretched by ~25 ms -- the query holds a driver lock that kernel
+    launches wait for (8 runs without any sampling: 19.6-20.3 ms; 24 runs with this query: 19.6-21.6 ms)."""
+    Q = ("clocks.sm,clocks.max.sm,clocks_event_reasons.hw_slowdown,"
          "clocks_event_reasons.hw_thermal_slowdown,clocks_event_reasons.sw_thermal_slowdown,"
          "clocks_event_reasons.sw_power_cap")
 
-    def __init__(self, index: int):
-        self.index, self.rows, self.proc = index, [], None
+    def __init__(self, index: int, interval_ms: int = 100):
+        self.index, self.rows, self.proc, self.interval_ms = index, [], None, interval_ms
 
     def start(self):
+        if self.interval_ms <= 0:
+            return
         try:
             self.proc = subprocess.Popen(["nvidia-smi", "-i", str(self.index), f"--query-gpu={self.Q}",
-                                          "--format=csv,noheader,nounits", "-lms", "100"],
+                                          "--format=csv,noheader,nounits", "-lms", str(self.interval_ms)],
                                          stdout=subprocess.PIPE, stderr=subprocess.DEVNULL, text=True)
             threading.Thread(target=self._read, daemon=True).start()
+            # nvidia-smi holds driver locks while it starts (about a second): kernel launches issued meanwhile stall, which
+            # showed as an occasional 25 instead of 20 ms per step on cfg 5.  Wait for its first sample before any step.
+            t_end = time.monotonic() + 5.0
+            while not self.rows and time.monotonic() < t_end and self.proc.poll() is None:
+                time.sleep(0.01)
         except Exception:
             self.proc = None
 
@@ -105,7 +114,7 @@ class ClockSampler:
     def stop(self) -> dict:
         if self.proc is None:
             return {"sm_mhz": None, "sm_max_mhz": None, "reasons": ["nvidia-smi unavailable"]}
-        time.sleep(0.15)
+        time.sleep(0.05 + self.interval_ms / 1000.0)
         self.proc.terminate()
         sm, mx, reasons = [], [], set()
         names = ["hw_slowdown", "hw_thermal_slowdown", "sw_thermal_slowdown", "sw_power_cap"]
@@ -116,7 +125,7 @@ class ClockSampler:
                 sm.append(float(r[0])); mx.append(float(r[1]))
             except Exception:
                 continue
-            for nm, v in zip(names, r[3:7]):
+            for nm, v in zip(names, r[2:6]):
                 if v.lower().startswith("active"):
                     reasons.add(nm)
         sm.sort()
@@ -320,7 +329,7 @@ def main_arm(args, wl):
     hbm_peak, hbm_src = _peaks()
     sm_count = torch.cuda.get_device_properties(local).multi_processor_count
 
-    clocks = ClockSampler(local)
+    clocks = ClockSampler(local, args.clock_interval_ms)
     if rank == 0:
         clocks.start()
     for _ in range(args.warmup):
@@ -486,7 +495,7 @@ def streamed_arm(args, wl):
         g.scan_children(parents, 0, 1)
         return [g.topk(k, 1, device="cpu")]
 
-    clocks = ClockSampler(0)
+    clocks = ClockSampler(0, args.clock_interval_ms)
     clocks.start()
     for _ in range(args.warmup):
         step()
@@ -604,6 +613,9 @@ def main():
     ap.add_argument("--scan-mode", type=int, default=0, help="cs_set_scan_mode: 0 auto, 1 plain, 2 bitmap, 3 bitmap stages")
     ap.add_argument("--update-mode", type=int, default=0, help="cs_set_update_mode: 0 auto, 1 direct, 2 binned")
     ap.add_argument("--rows-direct", type=int, default=-1, help="rows of each binned pass that use red.global")
+    ap.add_argument("--clock-interval-ms", type=int, default=100,
+                    help="nvidia-smi sampling period during the timed region (100: the timed region of cfg 5 lasts 100 ms); "
+                         "0 = no sampling (debugging)")
     ap.add_argument("--sweep", action="store_true", help="print the roofline-denominator sweep instead of a bench line")
     args = ap.parse_args()
     if args.sweep:
