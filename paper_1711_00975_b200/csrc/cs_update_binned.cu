@@ -48,10 +48,9 @@ __device__ __forceinline__ void st_stream16u(uint4* p, const uint4& v) {
 }
 
 /* Shared-memory layout of k_bin_scatter (dynamic):
- *   cnt[NB] | qlen | pad | queue[NB] (u16) | buf[NB*C] (u16) | 64 B pad
+ *   cnt[NB] | pad | buf[NB*C] (u16) | 64 B pad
  * All accesses of the hot loop use 32-bit shared-space addresses (no generic-to-shared conversion per access). */
-__host__ __device__ inline size_t smem_off_queue(uint32_t nb) { return (((size_t)nb + 2) * 4 + 15) & ~(size_t)15; }
-__host__ __device__ inline size_t smem_off_buf(uint32_t nb) { return (smem_off_queue(nb) + (size_t)nb * 2 + 15) & ~(size_t)15; }
+__host__ __device__ inline size_t smem_off_buf(uint32_t nb) { return ((size_t)nb * 4 + 15) & ~(size_t)15; }
 size_t scatter_smem_bytes(uint32_t nb, uint32_t C) { return smem_off_buf(nb) + (size_t)nb * C * 2 + 64; }
 
 __device__ __forceinline__ uint32_t atoms_inc(uint32_t addr) {
@@ -126,7 +125,9 @@ __device__ __forceinline__ void bin_particle(const PassParams& P, const InsertCt
 
 /* Particles [head, head + 2*pairs) are read as pairs (3 x 8 B per thread, 8-byte aligned); the <= 1 particle
  * before and the <= 1 after are applied directly by block 0.
- * One round = every thread bins one pair; then the bins holding >= 32 records are queued and flushed. */
+ * One round = every thread bins SCATTER_PAIRS_PER_ROUND pairs; then every bin that holds >= 32 records is flushed.  (A
+ * queue of the bins that are due, built in a phase of its own between two more barriers, cost 0.26 ms of 20.2 at cfg 3:
+ * with ~130 records per bin and round nearly every bin is due.) */
 template <int R, bool BIG>
 __global__ void __launch_bounds__(BIN_THREADS, 1)
 k_bin_scatter(const __grid_constant__ PassParams P, const __grid_constant__ BinParams B,
@@ -136,10 +137,8 @@ k_bin_scatter(const __grid_constant__ PassParams P, const __grid_constant__ BinP
     if (threadIdx.x < 4) s_stat[threadIdx.x] = 0;
     const uint32_t NT = blockDim.x;                                  // 512 or 1024
     uint32_t* cnt = reinterpret_cast<uint32_t*>(smem_raw);
-    uint32_t* qlen = cnt + B.nb;
-    uint16_t* queue = reinterpret_cast<uint16_t*>(smem_raw + smem_off_queue(B.nb));
     uint16_t* buf = reinterpret_cast<uint16_t*>(smem_raw + smem_off_buf(B.nb));
-    for (uint32_t i = threadIdx.x; i < B.nb + 1; i += NT) cnt[i] = 0;          // cnt and qlen
+    for (uint32_t i = threadIdx.x; i < B.nb; i += NT) cnt[i] = 0;
     __syncthreads();
 
     InsertCtx X;
@@ -160,7 +159,6 @@ k_bin_scatter(const __grid_constant__ PassParams P, const __grid_constant__ BinP
     int32_t* T = P.sc[0].T + ((uint64_t)B.rows_direct << B.log2w);      // first binned row: bin << log2S indexes from here
 
     for (uint64_t r = 0; r < rounds; ++r) {
-        if (threadIdx.x == 0) *qlen = 0;                               // last read before the previous barrier
 #pragma unroll 1
         for (int u = 0; u < SCATTER_PAIRS_PER_ROUND; ++u) {
             const uint64_t g = r * per_round + u * per_sub + (uint64_t)blockIdx.x * NT + threadIdx.x;
@@ -174,60 +172,54 @@ k_bin_scatter(const __grid_constant__ PassParams P, const __grid_constant__ BinP
             }
         }
         __syncthreads();
-        /* queue the bins that hold at least one full unit */
-        for (uint32_t b0 = warp * 32; b0 < B.nb; b0 += NT) {
-            const uint32_t bin = b0 + lane;
-            const bool full = bin < B.nb && cnt[bin] >= UNIT;
-            const uint32_t m = __ballot_sync(0xFFFFFFFFu, full);
-            if (m) {
-                uint32_t at = 0;
-                if (lane == 0) at = atomicAdd(qlen, (uint32_t)__popc(m));
-                at = __shfl_sync(0xFFFFFFFFu, at, 0);
-                if (full) queue[at + __popc(m & ((1u << lane) - 1u))] = (uint16_t)bin;
+        /* flush: groups of 4 lanes, one bin each; two bins per group and trip, so that the two reservations (global
+         * atomics that return a value: ~1 us each) are in flight together */
+        const uint32_t nq = B.nb, fstride = (NT / 32) * 8;
+        auto reserve = [&](uint32_t e, uint32_t& c, uint32_t& units, uint32_t& base) -> bool {
+            c = 0; units = 0; base = 0;
+            if (e >= nq) return false;
+            c = min(cnt[e], B.C);
+            units = c / UNIT;
+            if (units == 0) return false;
+            if (l4 == 0) {
+                base = atomicAdd(&B.cursor[e], units * UNIT);
+                atomicAdd(&s_stat[3], units * UNIT);
             }
-        }
-        __syncthreads();
-        /* flush: groups of 4 lanes, one queued bin each */
-        const uint32_t nq = *qlen;
-        for (uint32_t e0 = warp * 8; e0 < nq; e0 += (NT / 32) * 8) {
-            const uint32_t e = e0 + grp;
-            const bool on = e < nq;
-            uint32_t bin = 0, c = 0, units = 0, base = 0;
-            if (on) {
-                bin = queue[e];
-                c = min(cnt[bin], B.C);
-                units = c / UNIT;
-                if (l4 == 0) {
-                    base = atomicAdd(&B.cursor[bin], units * UNIT);
-                    atomicAdd(&s_stat[3], units * UNIT);
-                }
-            }
-            base = __shfl_sync(0xFFFFFFFFu, base, grp * 4);
-            if (on) {
-                uint16_t* src = buf + bin * B.C;
-                for (uint32_t u = 0; u < units; ++u) {
-                    const uint4 v = *reinterpret_cast<const uint4*>(src + u * UNIT + l4 * 8);
-                    const uint32_t at = base + u * UNIT;
-                    if (at + UNIT <= B.cap) {
-                        st_stream16u(reinterpret_cast<uint4*>(B.bins + (uint64_t)bin * B.cap + at + l4 * 8), v);
-                    } else {                                           // bin region full: apply directly
-                        atomicAdd(&s_stat[1], 8u);
-                        if (l4 == 0) atomicSub(&s_stat[3], UNIT);
-                        const uint32_t wds[4] = {v.x, v.y, v.z, v.w};
+            return true;
+        };
+        auto drain = [&](uint32_t bin, uint32_t c, uint32_t units, uint32_t base) {
+            uint16_t* src = buf + bin * B.C;
+            for (uint32_t u = 0; u < units; ++u) {
+                const uint4 v = *reinterpret_cast<const uint4*>(src + u * UNIT + l4 * 8);
+                const uint32_t at = base + u * UNIT;
+                if (at + UNIT <= B.cap) {
+                    st_stream16u(reinterpret_cast<uint4*>(B.bins + (uint64_t)bin * B.cap + at + l4 * 8), v);
+                } else {                                               // bin region full: apply directly
+                    atomicAdd(&s_stat[1], 8u);
+                    if (l4 == 0) atomicSub(&s_stat[3], UNIT);
+                    const uint32_t wds[4] = {v.x, v.y, v.z, v.w};
 #pragma unroll
-                        for (int k = 0; k < 4; ++k) {
-                            apply_direct(T, bin, B.log2S, wds[k] & 0xFFFFu);
-                            apply_direct(T, bin, B.log2S, wds[k] >> 16);
-                        }
+                    for (int k = 0; k < 4; ++k) {
+                        apply_direct(T, bin, B.log2S, wds[k] & 0xFFFFu);
+                        apply_direct(T, bin, B.log2S, wds[k] >> 16);
                     }
                 }
-                /* move the < 32 leftover records to the front, 8 records per lane (source and destination do not
-                 * overlap; what is copied past `left` is never read: the 64 B pad covers the last bin's over-read) */
-                const uint32_t left = c - units * UNIT;
-                if (l4 * 8 < left)
-                    *reinterpret_cast<uint4*>(src + l4 * 8) = *reinterpret_cast<const uint4*>(src + units * UNIT + l4 * 8);
-                if (l4 == 0) cnt[bin] = left;
             }
+            /* move the < 32 leftover records to the front, 8 records per lane (source and destination do not
+             * overlap; what is copied past `left` is never read: the 64 B pad covers the last bin's over-read) */
+            const uint32_t left = c - units * UNIT;
+            if (l4 * 8 < left)
+                *reinterpret_cast<uint4*>(src + l4 * 8) = *reinterpret_cast<const uint4*>(src + units * UNIT + l4 * 8);
+            if (l4 == 0) cnt[bin] = left;
+        };
+        for (uint32_t e0 = warp * 8; e0 < nq; e0 += 2 * fstride) {
+            const uint32_t ea = e0 + grp, eb = ea + fstride;
+            uint32_t ca, ua, ba, cb, ub, bb;
+            const bool ona = reserve(ea, ca, ua, ba), onb = reserve(eb, cb, ub, bb);
+            ba = __shfl_sync(0xFFFFFFFFu, ba, grp * 4);
+            bb = __shfl_sync(0xFFFFFFFFu, bb, grp * 4);
+            if (ona) drain(ea, ca, ua, ba);
+            if (onb) drain(eb, cb, ub, bb);
         }
         __syncthreads();
     }
