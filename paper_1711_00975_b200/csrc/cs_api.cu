@@ -12,6 +12,7 @@
 #include <vector>
 
 #include "cs_internal.h"
+#include "cs_select_batch.h"
 #include "cs_select_static.h"
 
 using namespace cs;
@@ -284,20 +285,29 @@ int read_states(cs_sketch* s) {
     return CS_OK;
 }
 
-/* Sort + dedupe + cut the candidate list of one scale: enqueued only, no synchronisation.  The list may end up in the
- * other half of its ping-pong buffers: the caller reads the states back (read_states) before it uses s->cur again. */
-int compact_scale(cs_sketch* s, int i) {
-    const uint32_t n = s->st_host[i].count < s->cap ? s->st_host[i].count : s->cap;
+/* Sort + dedupe + cut the candidate lists of the scales in `mask`, in one launch: enqueued only, no synchronisation.
+ * A list may end up in the other half of its ping-pong buffers: the caller reads the states back (read_states) before it
+ * uses s->cur again. */
+int compact_scales(cs_sketch* s, uint32_t mask) {
+    CompactRequest req[CS_MAX_SCALES];
+    int count = 0;
+    for (int i = 0; i < s->n_scales; ++i) {
+        if (!(mask >> i & 1u)) continue;
+        const uint32_t n = s->st_host[i].count < s->cap ? s->st_host[i].count : s->cap;
+        req[count++] = CompactRequest{&s->sb[i], s->cur[i], n, s->id_bits[i], s->st_dev + i, &s->epoch[i]};
+        s->dirty[i] = false;
+        s->n_compactions[i] += 1;
+        s->compact_n[i] = n;
+    }
+    if (!count) return CS_OK;
     s->tm.mark(PH_SELECT, s->stream);
-    cudaError_t e = select_compact(s->sb[i], s->cap, s->cur[i], n, s->id_bits[i], s->st_dev + i, s->k_max, s->thr_min, s->stream,
-                                   &s->launches, &s->epoch[i]);
+    cudaError_t e = select_compact_batch(req, count, s->cap, s->k_max, s->thr_min, s->stream, &s->launches);
     s->tm.stop(s->stream);
     if (e != cudaSuccess) return fail(CS_ERR_CUDA, "select_compact: %s", cudaGetErrorString(e));
-    s->dirty[i] = false;
-    s->n_compactions[i] += 1;
-    s->compact_n[i] = n;
     return CS_OK;
 }
+
+int compact_scale(cs_sketch* s, int i) { return compact_scales(s, 1u << i); }
 
 void fill_scan_params(cs_sketch* s, ScanParams* S) {
     memset(S, 0, sizeof(*S));
@@ -637,15 +647,13 @@ int scan_device_raw(cs_sketch* s, const float* xyz, uint64_t n, double sample_p)
             if (fr < free_min) free_min = fr;
         }
         if (free_min < s->cap / 2) {                     /* lists are legitimately large: make room */
-            bool any = false;
+            uint32_t due = 0;
             for (int i = 0; i < s->n_scales; ++i)
-                if (s->dirty[i] && s->st_host[i].count > s->cap / 2) {
-                    int rc = compact_scale(s, i);
-                    if (rc) return rc;
-                    any = true;
-                }
-            if (any) {
-                int rc = read_states(s);
+                if (s->dirty[i] && s->st_host[i].count > s->cap / 2) due |= 1u << i;
+            if (due) {
+                int rc = compact_scales(s, due);
+                if (rc) return rc;
+                rc = read_states(s);
                 if (rc) return rc;
                 for (int i = 0; i < s->n_scales; ++i) s->last_compact[i] = s->st_host[i].count;
                 continue;
@@ -691,10 +699,8 @@ int scan_device_raw(cs_sketch* s, const float* xyz, uint64_t n, double sample_p)
              * duplicate filter knows the dropped cells as seen: it is emptied first. */
             rc = clear_seen(s);
             if (rc) return rc;
-            for (int i = 0; i < s->n_scales; ++i) {
-                rc = compact_scale(s, i);
-                if (rc) return rc;
-            }
+            rc = compact_scales(s, (1u << s->n_scales) - 1u);
+            if (rc) return rc;
             rc = read_states(s);
             if (rc) return rc;
             free_min = s->cap;
@@ -717,15 +723,13 @@ int scan_device_raw(cs_sketch* s, const float* xyz, uint64_t n, double sample_p)
         done += chunk;
         s->scanned += chunk;
         s->first_chunk = false;
-        bool any = false;
+        uint32_t due = 0;
         for (int i = 0; i < s->n_scales; ++i)
-            if (wants_compaction(s, i)) {
-                int rc = compact_scale(s, i);
-                if (rc) return rc;
-                any = true;
-            }
-        if (any) {
-            int rc = read_states(s);
+            if (wants_compaction(s, i)) due |= 1u << i;
+        if (due) {
+            int rc = compact_scales(s, due);
+            if (rc) return rc;
+            rc = read_states(s);
             if (rc) return rc;
             for (int i = 0; i < s->n_scales; ++i)
                 if (!s->dirty[i]) s->last_compact[i] = s->st_host[i].count;
@@ -872,14 +876,20 @@ int scan_device(cs_sketch* s, const float* xyz, uint64_t n, double sample_p) {
     return CS_OK;
 }
 
-/* Bring the list of one scale into its final form (sorted, unique, cut) if anything was appended. */
-int finalize_scale(cs_sketch* s, int i) {
+/* Bring the list of one scale into its final form (sorted, unique, cut) if anything was appended.  others_too (the
+ * result calls cs_topk / cs_excursion): the other scales that wait for the same are compacted in the same launch, and
+ * one read-back (a stream synchronisation) serves them all. */
+int finalize_scale(cs_sketch* s, int i, bool others_too = false) {
     if (!s->dirty[i]) return CS_OK;
-    int rc = compact_scale(s, i);
+    uint32_t due = 0;
+    for (int j = 0; j < s->n_scales; ++j)
+        if (s->dirty[j] && (others_too || j == i)) due |= 1u << j;
+    int rc = compact_scales(s, due);
     if (rc) return rc;
     rc = read_states(s);
     if (rc) return rc;
-    s->last_compact[i] = s->st_host[i].count;
+    for (int j = 0; j < s->n_scales; ++j)
+        if (due >> j & 1u) s->last_compact[j] = s->st_host[j].count;
     return CS_OK;
 }
 
@@ -1602,7 +1612,7 @@ int cs_topk(cs_sketch* s, int scale, uint64_t k, uint64_t* ids_out, int32_t* est
     if (k && (!ids_out || !est_out)) return fail(CS_ERR_ARG, "null output with k > 0");
     if (!s->scanning) return fail(CS_ERR_STATE, "cs_topk before cs_scan_begin");
     if (k > s->k_max) return fail(CS_ERR_ARG, "k exceeds the k_max given to cs_scan_begin");
-    int rc = finalize_scale(s, scale);
+    int rc = finalize_scale(s, scale, true);
     if (rc) return rc;
     const uint32_t held = s->st_host[scale].count;
     const uint32_t n = k < held ? (uint32_t)k : held;
@@ -1620,7 +1630,7 @@ int cs_excursion(cs_sketch* s, int scale, int32_t thr, uint64_t cap, uint64_t* i
     if (cap && (!ids_out || !est_out)) return fail(CS_ERR_ARG, "null output with cap > 0");
     if (!s->scanning) return fail(CS_ERR_STATE, "cs_excursion before cs_scan_begin");
     if (thr < s->thr_min) return fail(CS_ERR_ARG, "thr is below the thr_min given to cs_scan_begin");
-    int rc = finalize_scale(s, scale);
+    int rc = finalize_scale(s, scale, true);
     if (rc) return rc;
     const uint32_t held = s->st_host[scale].count;
     cudaError_t e = launch_count_ge(s->sb[scale].ek[s->cur[scale]], held, thr, s->word_dev, s->stream);

@@ -28,6 +28,7 @@
  * about 2.
  */
 #include "cs_device.cuh"
+#include "cs_select_batch.h"
 #include "cs_select_static.h"
 
 #include <atomic>
@@ -84,13 +85,15 @@ __device__ __forceinline__ uint32_t digit_of(uint64_t id, uint32_t ek, int pass,
     return pass < id_passes ? ((uint32_t)(id >> (8 * pass)) & 255u) : ((ek >> (8 * (pass - id_passes))) & 255u);
 }
 
-/* plan->hist[p][digit] += entries of the list with that digit in pass p, for all passes at once (grid-stride sweep) */
+/* plan->hist[p][digit] += entries of the list with that digit in pass p, for all passes at once (stride = the nct CTAs
+ * that work on this list; bid = this CTA's index among them) */
 __device__ __forceinline__ void hist_sweep(const uint64_t* __restrict__ id, const uint32_t* __restrict__ ek, uint32_t n,
-                                           int id_passes, int passes, LocalPlan& L, SortPlan* plan) {
+                                           int id_passes, int passes, LocalPlan& L, SortPlan* plan, uint32_t bid,
+                                           uint32_t nct) {
     for (int i = threadIdx.x; i < passes * 256; i += SORT_THREADS) (&L.base[0][0])[i] = 0;
     __syncthreads();
-    const uint32_t stride = gridDim.x * SORT_THREADS;
-    for (uint32_t i = blockIdx.x * SORT_THREADS + threadIdx.x; i < n; i += stride) {
+    const uint32_t stride = nct * SORT_THREADS;
+    for (uint32_t i = bid * SORT_THREADS + threadIdx.x; i < n; i += stride) {
         const uint64_t c = id[i];
         const uint32_t k = ek[i];
         for (int p = 0; p < passes; ++p) atomicAdd(&L.base[p][digit_of(c, k, p, id_passes)], 1u);
@@ -331,36 +334,64 @@ __global__ void k_cut_empty(const __grid_constant__ HalfPtrs H, uint32_t half, S
     cut_list(H, half, 0u, st, k_max, thr_min);
 }
 
-/* One compaction in one cooperative launch (all CTAs co-resident; grid-wide barriers between the phases):
- *   digit histograms of all passes | plan | one sweep per needed digit | duplicate removal | cut | plan zeroed again */
+/* One list of a launch of k_compact and the CTAs [cta0, cta0 + ctas) of the grid that work on it. */
+struct CompactList {
+    HalfPtrs H;
+    uint32_t n, first_half;
+    int id_passes, passes;
+    SortPlan* plan;
+    uint64_t* status;
+    uint64_t* ustatus;
+    uint32_t epoch0;
+    ScanState* st;
+    uint32_t cta0, ctas;
+};
+struct CompactBatch {
+    int n_lists, max_passes;
+    uint64_t k_max;
+    int32_t thr_min;
+    CompactList L[CS_MAX_SCALES];
+};
+
+/* The compaction of up to CS_MAX_SCALES lists in one cooperative launch (all CTAs co-resident; grid-wide barriers between
+ * the phases), each list on its own share of the grid:
+ *   digit histograms of all passes | plan | one sweep per needed digit | duplicate removal | cut | plan zeroed again
+ * With one list a pass that no entry needs is skipped with its barrier; with several, every CTA takes the barriers of
+ * max_passes passes (the lists need different ones). */
+template <bool MULTI>
 __global__ void __launch_bounds__(SORT_THREADS, 4)
-k_compact(const __grid_constant__ HalfPtrs H, uint32_t n, uint32_t first_half, int id_passes, int passes, SortPlan* plan,
-          uint64_t* __restrict__ status, uint64_t* __restrict__ ustatus, uint32_t epoch0, ScanState* st, uint64_t k_max,
-          int32_t thr_min) {
+k_compact(const __grid_constant__ CompactBatch B) {
     __shared__ LocalPlan L;
     __shared__ uint32_t wcnt[SORT_WARPS][256];
     __shared__ uint32_t wsum[SORT_WARPS];
     __shared__ uint32_t s_excl;
     cg::grid_group grid = cg::this_grid();
-    const uint32_t tiles = (n + SORT_TILE - 1) / SORT_TILE;
+    int li = 0;
+    if (MULTI)
+        while (li + 1 < B.n_lists && blockIdx.x >= B.L[li].cta0 + B.L[li].ctas) ++li;
+    const CompactList& M = B.L[li];                           // one list: a static index, operands straight from the constant bank
+    const uint32_t bid = blockIdx.x - M.cta0, nct = M.ctas;
+    const uint32_t n = M.n, tiles = (n + SORT_TILE - 1) / SORT_TILE;
 
-    hist_sweep(H.id[first_half], H.ek[first_half], n, id_passes, passes, L, plan);
+    hist_sweep(M.H.id[M.first_half], M.H.ek[M.first_half], n, M.id_passes, M.passes, L, M.plan, bid, nct);
     grid.sync();
-    make_plan(plan, n, passes, first_half, L, wsum);
-    for (int p = 0; p < passes; ++p) {
-        if (!L.active[p]) continue;
-        for (uint32_t tile = blockIdx.x; tile < tiles; tile += gridDim.x)
-            pass_tile(H, n, p, id_passes, tile, L, wcnt, status, (epoch0 + (uint32_t)p) & 0x3FFFFFFFu);
+    make_plan(M.plan, n, M.passes, M.first_half, L, wsum);
+    for (int p = 0; p < B.max_passes; ++p) {
+        const bool mine = p < M.passes && L.active[p];
+        if (!MULTI && !mine) continue;
+        if (mine)
+            for (uint32_t tile = bid; tile < tiles; tile += nct)
+                pass_tile(M.H, n, p, M.id_passes, tile, L, wcnt, M.status, (M.epoch0 + (uint32_t)p) & 0x3FFFFFFFu);
         grid.sync();
     }
-    for (uint32_t tile = blockIdx.x; tile < tiles; tile += gridDim.x)
-        uniq_tile(H, n, tile, tiles, L, plan, wsum, &s_excl, ustatus, (epoch0 + (uint32_t)passes) & 0x3FFFFFFFu);
+    for (uint32_t tile = bid; tile < tiles; tile += nct)
+        uniq_tile(M.H, n, tile, tiles, L, M.plan, wsum, &s_excl, M.ustatus, (M.epoch0 + (uint32_t)M.passes) & 0x3FFFFFFFu);
     grid.sync();
-    if (blockIdx.x == 0) {
-        if (threadIdx.x == 0) cut_list(H, L.sorted_half ^ 1u, __ldcg(&plan->uniq_total), st, k_max, thr_min);
+    if (bid == 0) {
+        if (threadIdx.x == 0) cut_list(M.H, L.sorted_half ^ 1u, __ldcg(&M.plan->uniq_total), M.st, B.k_max, B.thr_min);
         __syncthreads();
-        for (int i = threadIdx.x; i < passes * 256; i += SORT_THREADS) (&plan->hist[0][0])[i] = 0;   // for the next compaction
-        if (threadIdx.x == 0) plan->uniq_total = 0;
+        for (int i = threadIdx.x; i < M.passes * 256; i += SORT_THREADS) (&M.plan->hist[0][0])[i] = 0;   // for the next compaction
+        if (threadIdx.x == 0) M.plan->uniq_total = 0;
     }
 }
 
@@ -405,7 +436,11 @@ static cudaError_t resident_ctas(uint32_t* out) {
     uint32_t v = dev < 64 ? cached[dev].load(std::memory_order_relaxed) : 0u;
     if (!v) {
         int per_sm = 0, sms = 0;
-        e = cudaOccupancyMaxActiveBlocksPerMultiprocessor(&per_sm, k_compact, SORT_THREADS, 0);
+        int per_sm_multi = 0;
+        e = cudaOccupancyMaxActiveBlocksPerMultiprocessor(&per_sm, k_compact<false>, SORT_THREADS, 0);
+        if (e != cudaSuccess) return e;
+        e = cudaOccupancyMaxActiveBlocksPerMultiprocessor(&per_sm_multi, k_compact<true>, SORT_THREADS, 0);
+        if (per_sm_multi < per_sm) per_sm = per_sm_multi;
         if (e != cudaSuccess) return e;
         e = cudaDeviceGetAttribute(&sms, cudaDevAttrMultiProcessorCount, dev);
         if (e != cudaSuccess) return e;
@@ -417,45 +452,82 @@ static cudaError_t resident_ctas(uint32_t* out) {
     return cudaSuccess;
 }
 
-/* k_compact works with any grid that is resident at once (tiles are dealt round-robin).  Where fewer CTAs fit than the
- * occupancy calculation says (a context restricted to part of the SMs), the launch is refused: halve and retry. */
-static cudaError_t launch_cooperative(uint32_t grid, void** args, cudaStream_t stream) {
+/* Shares the grid among the lists of a batch (in proportion to their tiles, at least one CTA each, at most `budget` in
+ * all) and launches k_compact.  k_compact works with any share that is resident at once (tiles are dealt round-robin).
+ * Where fewer CTAs fit than the occupancy calculation says (a context restricted to part of the SMs), the launch is
+ * refused: halve the budget and retry. */
+static cudaError_t launch_batch(CompactBatch& cb, cudaStream_t stream) {
+    uint32_t budget = 0;
+    cudaError_t e = resident_ctas(&budget);
+    if (e != cudaSuccess) return e;
     for (;;) {
-        cudaError_t e = cudaLaunchCooperativeKernel((const void*)k_compact, dim3(grid), dim3(SORT_THREADS), args, 0, stream);
-        if (e != cudaErrorCooperativeLaunchTooLarge || grid == 1) return e;
+        uint64_t total = 0;
+        for (int i = 0; i < cb.n_lists; ++i) total += tiles_of(cb.L[i].n);
+        uint32_t at = 0;
+        for (int i = 0; i < cb.n_lists; ++i) {
+            const uint32_t t = tiles_of(cb.L[i].n);
+            uint32_t c = total <= budget ? t : (uint32_t)((uint64_t)budget * t / total);
+            if (c > t) c = t;
+            if (c < 1) c = 1;
+            cb.L[i].cta0 = at;
+            cb.L[i].ctas = c;
+            at += c;
+        }
+        void* args[] = {&cb};
+        const void* fn = cb.n_lists > 1 ? (const void*)k_compact<true> : (const void*)k_compact<false>;
+        e = cudaLaunchCooperativeKernel(fn, dim3(at), dim3(SORT_THREADS), args, 0, stream);
+        if (e != cudaErrorCooperativeLaunchTooLarge || budget <= (uint32_t)cb.n_lists) return e;
         cudaGetLastError();
-        grid /= 2;
+        budget /= 2;
     }
+}
+
+cudaError_t select_compact_batch(const CompactRequest* req, int count, uint32_t cap, uint64_t k_max, int32_t thr_min,
+                                 cudaStream_t stream, uint64_t* launches) {
+    if (count < 0 || count > CS_MAX_SCALES) return cudaErrorInvalidValue;
+    CompactBatch cb;
+    cb.n_lists = 0; cb.max_passes = 0; cb.k_max = k_max; cb.thr_min = thr_min;
+    for (int r = 0; r < count; ++r) {
+        const CompactRequest& q = req[r];
+        HalfPtrs H;
+        for (int h = 0; h < 2; ++h) { H.id[h] = q.B->id[h]; H.ek[h] = q.B->ek[h]; }
+        if (q.n == 0) {
+            k_cut_empty<<<1, 1, 0, stream>>>(H, (uint32_t)q.src, q.st_dev, k_max, thr_min);
+            *launches += 1;
+            cudaError_t e = cudaGetLastError();
+            if (e != cudaSuccess) return e;
+            continue;
+        }
+        if (*q.epoch >= 0x3FFFFFFFu - 2u * MAX_PASSES) {     /* epochs are 30 bits wide: before they repeat, forget every */
+            cudaError_t e = cudaMemsetAsync(q.B->scratch, 0, (size_t)select_scratch_words(cap) * sizeof(uint32_t), stream);
+            if (e != cudaSuccess) return e;                  /* word written */
+            *q.epoch = 0;
+        }
+        CompactList& M = cb.L[cb.n_lists++];
+        M.H = H;
+        M.n = q.n;
+        M.first_half = (uint32_t)q.src;
+        M.id_passes = (q.id_bits + 7) / 8;
+        M.passes = M.id_passes + 4;
+        M.plan = reinterpret_cast<SortPlan*>(q.B->scratch);
+        M.status = reinterpret_cast<uint64_t*>(q.B->scratch + plan_words());
+        M.ustatus = M.status + (uint64_t)(tiles_of(cap) + 1) * 256;
+        M.epoch0 = *q.epoch + 1;
+        *q.epoch += (uint32_t)M.passes + 1;                  /* one epoch per look-back sweep: the passes, then uniq's */
+        M.st = q.st_dev;
+        if (M.passes > cb.max_passes) cb.max_passes = M.passes;
+    }
+    if (cb.n_lists == 0) return cudaSuccess;
+    *launches += 1;
+    return launch_batch(cb, stream);
 }
 
 /* Enqueues one compaction of the first n entries of half `src` (one launch on `stream`, no synchronisation).  Afterwards
  * st_dev->half names the half that holds the list and st_dev->count its length.  *epoch: per-buffer sweep counter. */
 cudaError_t select_compact(const SelectBuffers& B, uint32_t cap, int src, uint32_t n, int id_bits, ScanState* st_dev,
                            uint64_t k_max, int32_t thr_min, cudaStream_t stream, uint64_t* launches, uint32_t* epoch) {
-    HalfPtrs H;
-    for (int h = 0; h < 2; ++h) { H.id[h] = B.id[h]; H.ek[h] = B.ek[h]; }
-    *launches += 1;
-    if (n == 0) {
-        k_cut_empty<<<1, 1, 0, stream>>>(H, (uint32_t)src, st_dev, k_max, thr_min);
-        return cudaGetLastError();
-    }
-    uint32_t resident = 0;
-    cudaError_t e = resident_ctas(&resident);
-    if (e != cudaSuccess) return e;
-    SortPlan* plan = reinterpret_cast<SortPlan*>(B.scratch);
-    uint64_t* status = reinterpret_cast<uint64_t*>(B.scratch + plan_words());
-    uint64_t* ustatus = status + (uint64_t)(tiles_of(cap) + 1) * 256;
-    const uint32_t tiles = tiles_of(n);
-    int id_passes = (id_bits + 7) / 8, passes = id_passes + 4;
-    if (*epoch >= 0x3FFFFFFFu - 2u * MAX_PASSES) {           /* epochs are 30 bits wide: before they repeat, forget every */
-        e = cudaMemsetAsync(B.scratch, 0, (size_t)select_scratch_words(cap) * sizeof(uint32_t), stream);   /* word written */
-        if (e != cudaSuccess) return e;
-        *epoch = 0;
-    }
-    uint32_t first_half = (uint32_t)src, epoch0 = *epoch + 1;
-    *epoch += (uint32_t)passes + 1;                          /* one epoch per look-back sweep: the passes, then uniq's */
-    void* args[] = {&H, &n, &first_half, &id_passes, &passes, &plan, &status, &ustatus, &epoch0, &st_dev, &k_max, &thr_min};
-    return launch_cooperative(tiles < resident ? tiles : resident, args, stream);
+    const CompactRequest q = {&B, src, n, id_bits, st_dev, epoch};
+    return select_compact_batch(&q, 1, cap, k_max, thr_min, stream, launches);
 }
 
 /* ---- allocation-free selection over a caller's candidate list (cs_select_static, include/cs.h) -------------------------
@@ -531,19 +603,16 @@ cudaError_t select_static(const uint64_t* ids, const int32_t* est, uint32_t n, u
     const uint32_t tiles = tiles_of(n);
     k_static_load<<<tiles ? tiles : 1, 256, 0, stream>>>(S, ids, est, n, tiles);
     if (n) {
-        uint32_t resident = 0;
-        e = resident_ctas(&resident);
-        if (e != cudaSuccess) return e;
-        HalfPtrs H;
-        for (int h = 0; h < 2; ++h) { H.id[h] = S->id[h]; H.ek[h] = S->ek[h]; }
-        SortPlan* plan = &S->plan;
-        uint64_t *status = S->status, *ustatus = S->ustatus, k_max = k;
-        ScanState* st = &S->st;
-        uint32_t first_half = 0, epoch0 = 1;                  /* the status words were just zeroed: epoch 0 = not published */
-        int id_passes = 8, passes = MAX_PASSES;               /* every id byte; constant digits are skipped on the device */
-        int32_t thr_min = INT32_MAX;
-        void* args[] = {&H, &n, &first_half, &id_passes, &passes, &plan, &status, &ustatus, &epoch0, &st, &k_max, &thr_min};
-        e = launch_cooperative(tiles < resident ? tiles : resident, args, stream);
+        CompactBatch cb;
+        cb.n_lists = 1; cb.max_passes = MAX_PASSES; cb.k_max = k; cb.thr_min = INT32_MAX;
+        CompactList& M = cb.L[0];
+        for (int h = 0; h < 2; ++h) { M.H.id[h] = S->id[h]; M.H.ek[h] = S->ek[h]; }
+        M.n = n; M.first_half = 0;
+        M.id_passes = 8; M.passes = MAX_PASSES;               /* every id byte; constant digits are skipped on the device */
+        M.plan = &S->plan; M.status = S->status; M.ustatus = S->ustatus;
+        M.epoch0 = 1;                                         /* the status words were just zeroed: epoch 0 = not published */
+        M.st = &S->st;
+        e = launch_batch(cb, stream);
         if (e != cudaSuccess) return e;
     }
     const uint32_t eb = (k + 255u) / 256u;
