@@ -13,7 +13,8 @@
  * Top-k for any k <= k_max and the excursion set for any thr >= thr_min are then prefixes of the list.
  *
  * One compaction = ONE cooperative launch (k_compact: every CTA resident, grid-wide barriers between its phases), with
- * no host round trip in it:
+ * no host round trip in it -- for the lists of all scales of a handle that are due at once, each on its share of the grid
+ * (select_compact_batch, cs_select_batch.h):
  *   histogram      digit histograms of ALL passes in one sweep over the list
  *   plan           every CTA, from the global counts: which passes are needed (a digit that is the same in every entry
  *                  is skipped: the high bytes of the estimate key almost always are), exclusive digit bases, ping-pong plan
