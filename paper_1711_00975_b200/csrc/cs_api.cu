@@ -336,22 +336,23 @@ bool bad_p(double p) { return !(p > 0.0) || p > 1.0; }
 constexpr uint32_t BIN_MAX = 4096;                    /* bins per pass (words of `cursor`) */
 constexpr uint64_t BIN_MIN_N = 1ull << 22;            /* auto mode: below this the direct kernel is as fast */
 constexpr size_t BIN_SMEM = 216 * 1024;               /* shared memory of one scatter CTA (8 pairs per round at cfg 3: 211 KB) */
+constexpr uint32_t PAIRS_MIN = 5, PAIRS_MAX = 12;     /* pairs of particles per thread between two flush phases */
 
 struct BinPlan {
-    uint32_t log2w, log2S, SL, C, threads;
+    uint32_t log2w, log2S, SL, C, threads, pairs;
     int rows_per_pass, rows_direct;       /* rows of one pass, and how many of them take the direct route */
 };
 
 int ilog2(uint64_t v) { return bit_length(v) - 1; }
 
-uint32_t staging_capacity(uint32_t threads, uint32_t SL) {
-    const double lambda = 2.0 * SCATTER_PAIRS_PER_ROUND * threads / SL;    /* records per bin, round and CTA */
+uint32_t staging_capacity(uint32_t threads, uint32_t SL, uint32_t pairs) {
+    const double lambda = 2.0 * pairs * threads / SL;              /* records per bin, round and CTA */
     /* up to 31 records left from the round before + this round's arrivals (Poisson, mean lambda) + 3 sigma: the few
      * records beyond (measured 3e-8 of all at cfg 3) take the red.global route.  Sized at 6 sigma the same shared memory
-     * holds 6 pairs per round instead of 8, and the flush phases between rounds are what the extra pairs save. */
+     * holds 6 pairs per round instead of 8 at cfg 3, and the flush phases between rounds are what the extra pairs save. */
     uint32_t C = (uint32_t)(32.0 + lambda + 3.0 * std::sqrt(lambda) + 8.0);
     C = (C + 7u) & ~7u;
-    return C > 256 ? 256 : C;                          /* beyond: staging overflows go through red.global */
+    return C > 384 ? 384 : C;                          /* beyond: staging overflows go through red.global */
 }
 
 /* Rows of a pass of r rows that take the direct route.  Hybrid: the scatter kernel is bound by the integer pipes,
@@ -380,7 +381,7 @@ bool bin_plan(const cs_sketch* s, BinPlan* pl) {
     int rows = 0;
     for (int r = 1; r <= 8 && r <= s->d; ++r) {
         const uint32_t nb = (uint32_t)(r - direct_rows(s, r)) * SL;
-        if (nb <= BIN_MAX && scatter_smem_bytes(nb, staging_capacity(1024, SL)) <= BIN_SMEM) rows = r;
+        if (nb <= BIN_MAX && scatter_smem_bytes(nb, staging_capacity(1024, SL, PAIRS_MIN)) <= BIN_SMEM) rows = r;
     }
     if (!rows) return false;
     const int groups = (s->d + rows - 1) / rows;
@@ -390,8 +391,13 @@ bool bin_plan(const cs_sketch* s, BinPlan* pl) {
     pl->rows_direct = direct_rows(s, rows);
     /* two CTAs of 512 threads per SM when their staging buffers fit: one CTA's flush phase overlaps the other's hashing */
     const uint32_t nb = (uint32_t)(rows - pl->rows_direct) * SL;
-    pl->threads = scatter_smem_bytes(nb, staging_capacity(512, SL)) <= 110 * 1024 ? 512 : 1024;
-    pl->C = staging_capacity(pl->threads, SL);
+    pl->threads = scatter_smem_bytes(nb, staging_capacity(512, SL, PAIRS_MAX)) <= 110 * 1024 ? 512 : 1024;
+    /* as many pairs per round as the staging buffers have room for: the flush phases between rounds are overhead */
+    pl->pairs = PAIRS_MIN;
+    while (pl->pairs < PAIRS_MAX && scatter_smem_bytes(nb, staging_capacity(pl->threads, SL, pl->pairs + 1)) <=
+                                        (pl->threads == 512 ? 110 * 1024 : BIN_SMEM))
+        pl->pairs += 1;
+    pl->C = staging_capacity(pl->threads, SL, pl->pairs);
     return true;
 }
 
@@ -432,7 +438,7 @@ int update_binned(cs_sketch* s, const BinPlan& pl, const float* xyz, uint64_t n,
                 B.bins = s->bins; B.cursor = s->cursor; B.cap = (uint32_t)cap;
                 B.rows_direct = pl.rows_direct < nr ? pl.rows_direct : nr;
                 B.nb = (uint32_t)(nr - B.rows_direct) * pl.SL;
-                B.threads = pl.threads; B.C = pl.C; B.log2S = pl.log2S; B.log2w = pl.log2w;
+                B.threads = pl.threads; B.C = pl.C; B.pairs = pl.pairs; B.log2S = pl.log2S; B.log2w = pl.log2w;
                 B.stats = s->bin_stats;
                 if (B.nb) CS_CUDA(cudaMemsetAsync(s->cursor, 0, B.nb * sizeof(uint32_t), s->stream));
                 cudaError_t e = launch_update_binned(P, B, xyz + 3 * off, m, s->sm_count, s->stream, &s->tm);

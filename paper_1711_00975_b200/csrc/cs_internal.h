@@ -116,13 +116,13 @@ struct BinParams {
     uint32_t nb;          // bins of this pass = binned rows << (log2w - log2S)
     uint32_t threads;     // CTA size of the scatter kernel (512 or 1024)
     uint32_t C;           // records per shared-memory staging buffer, a multiple of 8
+    uint32_t pairs;       // pairs of particles per thread between two flush phases (the host sizes C with it)
     uint32_t log2S;       // <= 15
     uint32_t log2w;
     int32_t rows_direct;  // the first rows_direct rows of the pass use red.global instead of the bins
     unsigned long long* stats;  // 4 counters (may be NULL): records that left the binned route -- [0] staging buffer full,
                                 // [1] bin region full, [2] leftovers of partial buffers at kernel end; [3] records binned
 };
-constexpr int SCATTER_PAIRS_PER_ROUND = 8;      // pairs of particles per thread between two flush phases of k_bin_scatter
 size_t scatter_smem_bytes(uint32_t nb, uint32_t C);
 cudaError_t launch_update_binned(const PassParams& P, const BinParams& B, const float* xyz, uint64_t n, int sm_count,
                                  cudaStream_t st, PhaseTimer* tm);

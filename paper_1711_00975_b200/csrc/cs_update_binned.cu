@@ -27,8 +27,7 @@ namespace cs {
 
 constexpr int BIN_THREADS = 1024;
 constexpr uint32_t UNIT = 32;            // records per flush unit (64 bytes)
-// pairs of particles a thread bins between two flush phases: cs_internal.h SCATTER_PAIRS_PER_ROUND (the host sizes the
-// staging buffers with it)
+// pairs of particles a thread bins between two flush phases: BinParams::pairs (the host sizes the staging buffers with it)
 
 __device__ __forceinline__ float2 ld_stream8(const float2* p) {
     float2 v;
@@ -125,7 +124,7 @@ __device__ __forceinline__ void bin_particle(const PassParams& P, const InsertCt
 
 /* Particles [head, head + 2*pairs) are read as pairs (3 x 8 B per thread, 8-byte aligned); the <= 1 particle
  * before and the <= 1 after are applied directly by block 0.
- * One round = every thread bins SCATTER_PAIRS_PER_ROUND pairs; then every bin that holds >= 32 records is flushed.  (A
+ * One round = every thread bins B.pairs pairs; then every bin that holds >= 32 records is flushed.  (A
  * queue of the bins that are due, built in a phase of its own between two more barriers, cost 0.26 ms of 20.2 at cfg 3:
  * with ~130 records per bin and round nearly every bin is due.) */
 template <int R, bool BIG>
@@ -152,7 +151,7 @@ k_bin_scatter(const __grid_constant__ PassParams P, const __grid_constant__ BinP
 
     const float2* body = reinterpret_cast<const float2*>(xyz + 3 * (uint64_t)head);
     const uint64_t per_sub = (uint64_t)gridDim.x * NT;                 // pairs of one sub-round over the grid
-    const uint64_t per_round = per_sub * SCATTER_PAIRS_PER_ROUND;
+    const uint64_t per_round = per_sub * B.pairs;
     const uint64_t rounds = (pairs + per_round - 1) / per_round;
     const uint32_t lane = threadIdx.x & 31u, warp = threadIdx.x >> 5;
     const uint32_t grp = lane >> 2, l4 = lane & 3u;
@@ -160,7 +159,7 @@ k_bin_scatter(const __grid_constant__ PassParams P, const __grid_constant__ BinP
 
     for (uint64_t r = 0; r < rounds; ++r) {
 #pragma unroll 1
-        for (int u = 0; u < SCATTER_PAIRS_PER_ROUND; ++u) {
+        for (uint32_t u = 0; u < B.pairs; ++u) {
             const uint64_t g = r * per_round + u * per_sub + (uint64_t)blockIdx.x * NT + threadIdx.x;
             if (g < pairs) {
                 const float2 q0 = ld_stream8(body + 3 * g);
