@@ -231,7 +231,7 @@ def _roofline(wl, world, N, value, ms_per_step, phases, hbm_peak, hbm_src, A_red
                       "gather_peak_G_per_s": A_gather / 1e9,
                       "counter_updates_per_s_G": kept * wl.d * n_scales / (upd_ms * 1e-3) / 1e9 if upd_ms else None,
                       "note": "counter updates/s of the update phase can exceed the red.global peak: " + n_rows_direct_note},
-        "path": {"roof_particles_per_s": path_roof, "frac": (value / world) / path_roof,
+        "path": {"roof_particles_per_s": path_roof, "frac": (value / world) / path_roof, "hard_bound": False,
                  "formula": "min(HBM/12B, A_L2/(d*scales*p)) per GPU with A_L2 = the L2-resident red.global.add peak "
                             "measured in this run; the whole update+scan+select step against it (BASELINE.json north_star)",
                  "note": "the contract's denominator, not a hard bound of this design: the update sends 4 of 7 rows through "
