@@ -82,12 +82,37 @@ class ClockSampler:
          "clocks_event_reasons.hw_thermal_slowdown,clocks_event_reasons.sw_thermal_slowdown,"
          "clocks_event_reasons.sw_power_cap")
 
-    def __init__(self, index: int, interval_ms: int = 100):
-        self.index, self.rows, self.proc, self.interval_ms = index, [], None, interval_ms
+    def __init__(self, index: int, interval_ms: int = 100, source: str = "nvidia-smi"):
+        self.index, self.rows, self.proc, self.interval_ms, self.source = index, [], None, interval_ms, source
+        self.live = False
+
+    def _nvml_loop(self, nv, h, mx):
+        bits = [nv.nvmlClocksThrottleReasonHwSlowdown, nv.nvmlClocksThrottleReasonHwThermalSlowdown,
+                nv.nvmlClocksThrottleReasonSwThermalSlowdown, nv.nvmlClocksThrottleReasonSwPowerCap]
+        while self.live:
+            try:
+                sm = nv.nvmlDeviceGetClockInfo(h, nv.NVML_CLOCK_SM)
+                r = nv.nvmlDeviceGetCurrentClocksThrottleReasons(h)
+                self.rows.append((time.monotonic(), [str(sm), str(mx)] + ["Active" if r & b else "Not Active" for b in bits]))
+            except Exception:
+                pass
+            time.sleep(self.interval_ms / 1000.0)
 
     def start(self):
         if self.interval_ms <= 0:
             return
+        if self.source == "nvml":                       # the library nvidia-smi reads, in this process (no start-up, one
+            try:                                        # clock and one reasons query per sample)
+                import pynvml as nv
+                nv.nvmlInit()
+                h = nv.nvmlDeviceGetHandleByIndex(self.index)
+                mx = nv.nvmlDeviceGetMaxClockInfo(h, nv.NVML_CLOCK_SM)
+                self.live = True
+                self.proc = threading.Thread(target=self._nvml_loop, args=(nv, h, mx), daemon=True)
+                self.proc.start()
+                return
+            except Exception:
+                self.live, self.proc, self.source = False, None, "nvidia-smi"
         try:
             self.proc = subprocess.Popen(["nvidia-smi", "-i", str(self.index), f"--query-gpu={self.Q}",
                                           "--format=csv,noheader,nounits", "-lms", str(self.interval_ms)],
@@ -115,7 +140,10 @@ class ClockSampler:
         if self.proc is None:
             return {"sm_mhz": None, "sm_max_mhz": None, "reasons": ["nvidia-smi unavailable"]}
         time.sleep(0.05 + self.interval_ms / 1000.0)
-        self.proc.terminate()
+        if self.live:
+            self.live = False
+        else:
+            self.proc.terminate()
         sm, mx, reasons = [], [], set()
         names = ["hw_slowdown", "hw_thermal_slowdown", "sw_thermal_slowdown", "sw_power_cap"]
         for t, r in self.rows:
@@ -130,7 +158,7 @@ class ClockSampler:
                     reasons.add(nm)
         sm.sort()
         return {"sm_mhz": sm[len(sm) // 2] if sm else None, "sm_max_mhz": max(mx) if mx else None,
-                "reasons": sorted(reasons), "samples": len(sm)}
+                "reasons": sorted(reasons), "samples": len(sm), "source": self.source}
 
 
 def run_oracle_sample(wl, host_xyz, k):
@@ -329,7 +357,7 @@ def main_arm(args, wl):
     hbm_peak, hbm_src = _peaks()
     sm_count = torch.cuda.get_device_properties(local).multi_processor_count
 
-    clocks = ClockSampler(local, args.clock_interval_ms)
+    clocks = ClockSampler(local, args.clock_interval_ms, args.clock_source)
     if rank == 0:
         clocks.start()
     for _ in range(args.warmup):
@@ -495,7 +523,7 @@ def streamed_arm(args, wl):
         g.scan_children(parents, 0, 1)
         return [g.topk(k, 1, device="cpu")]
 
-    clocks = ClockSampler(0, args.clock_interval_ms)
+    clocks = ClockSampler(0, args.clock_interval_ms, args.clock_source)
     clocks.start()
     for _ in range(args.warmup):
         step()
@@ -616,6 +644,7 @@ def main():
     ap.add_argument("--clock-interval-ms", type=int, default=100,
                     help="nvidia-smi sampling period during the timed region (100: the timed region of cfg 5 lasts 100 ms); "
                          "0 = no sampling (debugging)")
+    ap.add_argument("--clock-source", default="nvidia-smi", choices=["nvidia-smi", "nvml"])
     ap.add_argument("--sweep", action="store_true", help="print the roofline-denominator sweep instead of a bench line")
     args = ap.parse_args()
     if args.sweep:
