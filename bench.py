@@ -333,6 +333,15 @@ def main_arm(args, wl):
         torch.cuda.synchronize()
 
     def timed(nsteps, host=None, upd_events=None):
+        import gc
+        gc.collect()          # keep interpreter collections out of the timed region (cfg 5: 100 ms in all)
+        gc.disable()
+        try:
+            return _timed(nsteps, host, upd_events)
+        finally:
+            gc.enable()
+
+    def _timed(nsteps, host=None, upd_events=None):
         barrier()
         e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
         e0.record()

@@ -41,9 +41,11 @@ namespace cs {
 
 constexpr int SORT_THREADS = 256;
 constexpr int SORT_WARPS = SORT_THREADS / 32;
-constexpr int SORT_ITEMS = 8;                              // items per lane
-constexpr int SORT_TILE = SORT_THREADS * SORT_ITEMS;       // 2048 entries per block
-constexpr int SORT_SEG = 32 * SORT_ITEMS;                  // consecutive entries owned by one warp
+constexpr int SORT_ITEMS = 8;                              // items per lane: long lists (tiles of 2048 entries)
+constexpr int SORT_ITEMS_SHORT = 4;                        // lists whose tiles of 1024 all run at once: shorter chains per
+                                                           // tile (cfg 3 select 1.00 -> 0.91 ms; long lists lose: cfg 5 1.33 -> 1.52)
+constexpr int SORT_TILE = SORT_THREADS * SORT_ITEMS;       // the long tile (sizes the static scratch)
+constexpr uint32_t SHORT_TILES_MAX = 148 * 8;              // upper bound of the tiles a short list has (CTA slots of the GPU)
 constexpr int LOOKBACK = 8;                                // predecessors a look-back step fetches together
 constexpr int MAX_PASSES = 12;                             // 8 id bytes (ids < 2^60 need 8) + 4 estimate-key bytes
 
@@ -144,6 +146,7 @@ __device__ __forceinline__ void make_plan(const SortPlan* plan, uint32_t n, int 
  * its digit counts and obtains its offsets from the tiles before it by decoupled look-back (status: tiles x 256 words).
  * Tiles are dealt to the (co-resident) CTAs round-robin and each CTA takes its tiles in increasing order, so a tile only
  * ever waits for tiles that are done or running. */
+template <int ITEMS>
 __device__ __forceinline__ void pass_tile(const HalfPtrs& H, uint32_t n, int pass, int id_passes, uint32_t tile,
                                           const LocalPlan& L, uint32_t (*wcnt)[256], uint64_t* __restrict__ status,
                                           uint32_t epoch) {
@@ -156,12 +159,12 @@ __device__ __forceinline__ void pass_tile(const HalfPtrs& H, uint32_t n, int pas
     uint64_t* __restrict__ did = H.id[src ^ 1u];
     uint32_t* __restrict__ dek = H.ek[src ^ 1u];
 
-    const uint32_t base = tile * SORT_TILE + wq * SORT_SEG;
-    uint64_t kid[SORT_ITEMS];
-    uint32_t kek[SORT_ITEMS], off[SORT_ITEMS];
+    const uint32_t base = tile * (SORT_THREADS * ITEMS) + wq * (32 * ITEMS);
+    uint64_t kid[ITEMS];
+    uint32_t kek[ITEMS], off[ITEMS];
     uint32_t* mine = wcnt[wq];
 #pragma unroll
-    for (int r = 0; r < SORT_ITEMS; ++r) {
+    for (int r = 0; r < ITEMS; ++r) {
         const uint32_t i = base + r * 32 + lane;
         const bool valid = i < n;
         kid[r] = valid ? __ldcg(sid + i) : 0;                   // written by other CTAs in the pass before: L2, not L1
@@ -219,7 +222,7 @@ __device__ __forceinline__ void pass_tile(const HalfPtrs& H, uint32_t n, int pas
     }
     __syncthreads();
 #pragma unroll
-    for (int r = 0; r < SORT_ITEMS; ++r) {
+    for (int r = 0; r < ITEMS; ++r) {
         const uint32_t i = base + r * 32 + lane;
         if (i < n) {
             const uint32_t dg = digit_of(kid[r], kek[r], pass, id_passes);
@@ -233,8 +236,9 @@ __device__ __forceinline__ void pass_tile(const HalfPtrs& H, uint32_t n, int pas
 
 /* ---- duplicate removal on the sorted list ------------------------------------------------------------------------ */
 
-/* One tile: each thread owns SORT_ITEMS consecutive entries; block scan of the per-thread counts of "first of its id"
+/* One tile: each thread owns ITEMS consecutive entries; block scan of the per-thread counts of "first of its id"
  * flags; the tile's offset comes from a look-back over the tile totals (ustatus: one word per tile). */
+template <int ITEMS>
 __device__ __forceinline__ void uniq_tile(const HalfPtrs& H, uint32_t n, uint32_t tile, uint32_t tiles, const LocalPlan& L,
                                           SortPlan* plan, uint32_t* wsum, uint32_t* s_excl, uint64_t* __restrict__ ustatus,
                                           uint32_t epoch) {
@@ -243,12 +247,12 @@ __device__ __forceinline__ void uniq_tile(const HalfPtrs& H, uint32_t n, uint32_
     const uint32_t* __restrict__ sek = H.ek[src];
     uint64_t* __restrict__ did = H.id[src ^ 1u];
     uint32_t* __restrict__ dek = H.ek[src ^ 1u];
-    const uint32_t first = tile * SORT_TILE + threadIdx.x * SORT_ITEMS;
-    uint64_t v[SORT_ITEMS];
+    const uint32_t first = tile * (SORT_THREADS * ITEMS) + threadIdx.x * ITEMS;
+    uint64_t v[ITEMS];
     uint64_t prev = (first > 0 && first <= n) ? __ldcg(sid + first - 1) : 0;
     uint32_t flags = 0, c = 0;
 #pragma unroll
-    for (int r = 0; r < SORT_ITEMS; ++r) {
+    for (int r = 0; r < ITEMS; ++r) {
         const uint32_t i = first + r;
         v[r] = i < n ? __ldcg(sid + i) : 0;
         if (i < n && (i == 0 || v[r] != prev)) { flags |= 1u << r; ++c; }
@@ -296,7 +300,7 @@ __device__ __forceinline__ void uniq_tile(const HalfPtrs& H, uint32_t n, uint32_
     __syncthreads();
     uint32_t dst = *s_excl + wbase + incl - c;
 #pragma unroll
-    for (int r = 0; r < SORT_ITEMS; ++r) {
+    for (int r = 0; r < ITEMS; ++r) {
         if (flags & (1u << r)) {
             did[dst] = v[r];
             dek[dst] = __ldcg(sek + first + r);
@@ -359,7 +363,7 @@ struct CompactBatch {
  *   digit histograms of all passes | plan | one sweep per needed digit | duplicate removal | cut | plan zeroed again
  * With one list a pass that no entry needs is skipped with its barrier; with several, every CTA takes the barriers of
  * max_passes passes (the lists need different ones). */
-template <bool MULTI>
+template <bool MULTI, int ITEMS>
 __global__ void __launch_bounds__(SORT_THREADS, 4)
 k_compact(const __grid_constant__ CompactBatch B) {
     __shared__ LocalPlan L;
@@ -372,7 +376,7 @@ k_compact(const __grid_constant__ CompactBatch B) {
         while (li + 1 < B.n_lists && blockIdx.x >= B.L[li].cta0 + B.L[li].ctas) ++li;
     const CompactList& M = B.L[li];                           // one list: a static index, operands straight from the constant bank
     const uint32_t bid = blockIdx.x - M.cta0, nct = M.ctas;
-    const uint32_t n = M.n, tiles = (n + SORT_TILE - 1) / SORT_TILE;
+    const uint32_t n = M.n, tiles = (n + SORT_THREADS * ITEMS - 1) / (SORT_THREADS * ITEMS);
 
     hist_sweep(M.H.id[M.first_half], M.H.ek[M.first_half], n, M.id_passes, M.passes, L, M.plan, bid, nct);
     grid.sync();
@@ -382,11 +386,11 @@ k_compact(const __grid_constant__ CompactBatch B) {
         if (!MULTI && !mine) continue;
         if (mine)
             for (uint32_t tile = bid; tile < tiles; tile += nct)
-                pass_tile(M.H, n, p, M.id_passes, tile, L, wcnt, M.status, (M.epoch0 + (uint32_t)p) & 0x3FFFFFFFu);
+                pass_tile<ITEMS>(M.H, n, p, M.id_passes, tile, L, wcnt, M.status, (M.epoch0 + (uint32_t)p) & 0x3FFFFFFFu);
         grid.sync();
     }
     for (uint32_t tile = bid; tile < tiles; tile += nct)
-        uniq_tile(M.H, n, tile, tiles, L, M.plan, wsum, &s_excl, M.ustatus, (M.epoch0 + (uint32_t)M.passes) & 0x3FFFFFFFu);
+        uniq_tile<ITEMS>(M.H, n, tile, tiles, L, M.plan, wsum, &s_excl, M.ustatus, (M.epoch0 + (uint32_t)M.passes) & 0x3FFFFFFFu);
     grid.sync();
     if (bid == 0) {
         if (threadIdx.x == 0) cut_list(M.H, L.sorted_half ^ 1u, __ldcg(&M.plan->uniq_total), M.st, B.k_max, B.thr_min);
@@ -419,12 +423,20 @@ __global__ void k_count_ge(const uint32_t* __restrict__ ek, uint32_t n, int32_t 
 
 /* ---- host orchestration ----------------------------------------------------------------------------------- */
 
-static uint32_t tiles_of(uint64_t n) { return (uint32_t)((n + SORT_TILE - 1) / SORT_TILE); }
+static uint32_t tiles_of(uint64_t n, int items = SORT_ITEMS) {
+    const uint64_t tile = (uint64_t)SORT_THREADS * items;
+    return (uint32_t)((n + tile - 1) / tile);
+}
 
-/* scratch layout (uint32 words): SortPlan | status[tiles][256] (u64) | ustatus[tiles] (u64) */
+/* scratch layout (uint32 words): SortPlan | status[rows][256] (u64) | ustatus[rows] (u64); rows: the long tiles of a full
+ * buffer, or the short tiles of the longest list that is sorted with short tiles */
 static uint64_t plan_words() { return (sizeof(SortPlan) + 15) / 16 * 4; }
+static uint64_t status_rows(uint64_t cap) {
+    const uint64_t t = tiles_of(cap);
+    return (t > SHORT_TILES_MAX ? t : SHORT_TILES_MAX) + 1;
+}
 uint64_t select_scratch_words(uint64_t n) {
-    const uint64_t t = tiles_of(n) + 1;
+    const uint64_t t = status_rows(n);
     return plan_words() + t * 256 * 2 + t * 2 + 16;
 }
 
@@ -436,13 +448,15 @@ static cudaError_t resident_ctas(uint32_t* out) {
     if (e != cudaSuccess) return e;
     uint32_t v = dev < 64 ? cached[dev].load(std::memory_order_relaxed) : 0u;
     if (!v) {
-        int per_sm = 0, sms = 0;
-        int per_sm_multi = 0;
-        e = cudaOccupancyMaxActiveBlocksPerMultiprocessor(&per_sm, k_compact<false>, SORT_THREADS, 0);
-        if (e != cudaSuccess) return e;
-        e = cudaOccupancyMaxActiveBlocksPerMultiprocessor(&per_sm_multi, k_compact<true>, SORT_THREADS, 0);
-        if (per_sm_multi < per_sm) per_sm = per_sm_multi;
-        if (e != cudaSuccess) return e;
+        int per_sm = 1 << 30, sms = 0;
+        const void* fns[4] = {(const void*)k_compact<false, SORT_ITEMS>, (const void*)k_compact<true, SORT_ITEMS>,
+                              (const void*)k_compact<false, SORT_ITEMS_SHORT>, (const void*)k_compact<true, SORT_ITEMS_SHORT>};
+        for (int f = 0; f < 4; ++f) {                        /* one bound for all forms of the kernel */
+            int x = 0;
+            e = cudaOccupancyMaxActiveBlocksPerMultiprocessor(&x, fns[f], SORT_THREADS, 0);
+            if (e != cudaSuccess) return e;
+            if (x < per_sm) per_sm = x;
+        }
         e = cudaDeviceGetAttribute(&sms, cudaDevAttrMultiProcessorCount, dev);
         if (e != cudaSuccess) return e;
         v = (uint32_t)(per_sm * sms);
@@ -457,16 +471,21 @@ static cudaError_t resident_ctas(uint32_t* out) {
  * all) and launches k_compact.  k_compact works with any share that is resident at once (tiles are dealt round-robin).
  * Where fewer CTAs fit than the occupancy calculation says (a context restricted to part of the SMs), the launch is
  * refused: halve the budget and retry. */
-static cudaError_t launch_batch(CompactBatch& cb, cudaStream_t stream) {
+static cudaError_t launch_batch(CompactBatch& cb, cudaStream_t stream, bool allow_short) {
     uint32_t budget = 0;
     cudaError_t e = resident_ctas(&budget);
     if (e != cudaSuccess) return e;
     for (;;) {
+        /* short tiles when every one of them gets a CTA of its own in this launch */
+        uint64_t total_short = 0;
+        for (int i = 0; i < cb.n_lists; ++i) total_short += tiles_of(cb.L[i].n, SORT_ITEMS_SHORT);
+        const bool use_short = allow_short && total_short <= budget && total_short <= SHORT_TILES_MAX;
+        const int items = use_short ? SORT_ITEMS_SHORT : SORT_ITEMS;
         uint64_t total = 0;
-        for (int i = 0; i < cb.n_lists; ++i) total += tiles_of(cb.L[i].n);
+        for (int i = 0; i < cb.n_lists; ++i) total += tiles_of(cb.L[i].n, items);
         uint32_t at = 0;
         for (int i = 0; i < cb.n_lists; ++i) {
-            const uint32_t t = tiles_of(cb.L[i].n);
+            const uint32_t t = tiles_of(cb.L[i].n, items);
             uint32_t c = total <= budget ? t : (uint32_t)((uint64_t)budget * t / total);
             if (c > t) c = t;
             if (c < 1) c = 1;
@@ -475,7 +494,9 @@ static cudaError_t launch_batch(CompactBatch& cb, cudaStream_t stream) {
             at += c;
         }
         void* args[] = {&cb};
-        const void* fn = cb.n_lists > 1 ? (const void*)k_compact<true> : (const void*)k_compact<false>;
+        const void* fn = cb.n_lists > 1
+            ? (use_short ? (const void*)k_compact<true, SORT_ITEMS_SHORT> : (const void*)k_compact<true, SORT_ITEMS>)
+            : (use_short ? (const void*)k_compact<false, SORT_ITEMS_SHORT> : (const void*)k_compact<false, SORT_ITEMS>);
         e = cudaLaunchCooperativeKernel(fn, dim3(at), dim3(SORT_THREADS), args, 0, stream);
         if (e != cudaErrorCooperativeLaunchTooLarge || budget <= (uint32_t)cb.n_lists) return e;
         cudaGetLastError();
@@ -512,7 +533,7 @@ cudaError_t select_compact_batch(const CompactRequest* req, int count, uint32_t 
         M.passes = M.id_passes + 4;
         M.plan = reinterpret_cast<SortPlan*>(q.B->scratch);
         M.status = reinterpret_cast<uint64_t*>(q.B->scratch + plan_words());
-        M.ustatus = M.status + (uint64_t)(tiles_of(cap) + 1) * 256;
+        M.ustatus = M.status + status_rows(cap) * 256;
         M.epoch0 = *q.epoch + 1;
         *q.epoch += (uint32_t)M.passes + 1;                  /* one epoch per look-back sweep: the passes, then uniq's */
         M.st = q.st_dev;
@@ -520,7 +541,7 @@ cudaError_t select_compact_batch(const CompactRequest* req, int count, uint32_t 
     }
     if (cb.n_lists == 0) return cudaSuccess;
     *launches += 1;
-    return launch_batch(cb, stream);
+    return launch_batch(cb, stream, true);
 }
 
 /* Enqueues one compaction of the first n entries of half `src` (one launch on `stream`, no synchronisation).  Afterwards
@@ -613,7 +634,7 @@ cudaError_t select_static(const uint64_t* ids, const int32_t* est, uint32_t n, u
         M.plan = &S->plan; M.status = S->status; M.ustatus = S->ustatus;
         M.epoch0 = 1;                                         /* the status words were just zeroed: epoch 0 = not published */
         M.st = &S->st;
-        e = launch_batch(cb, stream);
+        e = launch_batch(cb, stream, false);              /* the static status words cover long tiles only */
         if (e != cudaSuccess) return e;
     }
     const uint32_t eb = (k + 255u) / 256u;
