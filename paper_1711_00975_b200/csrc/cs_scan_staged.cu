@@ -530,12 +530,26 @@ cudaError_t launch_scan_staged_cb(const PassParams& P, const ScanTarget& tg, con
     Q2.out = B.list[1]; Q2.cnt_out = B.cnt[1];
     Q2.row0 = first;
     if (tm) tm->mark(PH_SCAN_NEXT, st);
-    launch_stage_r<true>(rest, false, blocks, P, Q2, tg, xyz, n, head, groups, gpb, st);
+    /* The rows left go in two stages: ONE row first, then the others.  Nearly every survivor of the bitmap stage arrives one
+     * fail short of rejection and leaves after the next row; with all rows in one kernel some lane of every warp needs the
+     * later rows, so every warp paid their instructions and their dependent gathers. */
+    const int r1 = (rest >= 2 && n >= (1ull << 22)) ? 1 : rest;      /* short chunks: the extra launch costs more */
+    launch_stage_r<true>(r1, false, blocks, P, Q2, tg, xyz, n, head, groups, gpb, st);
     StageParams F = Q2;
     F.in = B.list[1];
     F.cnt_in = B.cnt[1];
-    launch_final<true>(blocks, P, F, tg, st);
     *launches += 2;
+    if (rest > r1) {
+        StageParams Q3 = Q2;
+        Q3.in = B.list[1]; Q3.cnt_in = B.cnt[1];
+        Q3.out = B.list[0]; Q3.cnt_out = B.cnt[0];
+        Q3.row0 = first + r1;
+        launch_stage_r<true>(rest - r1, false, blocks, P, Q3, tg, xyz, n, head, groups, gpb, st);
+        F.in = B.list[0];
+        F.cnt_in = B.cnt[0];
+        *launches += 1;
+    }
+    launch_final<true>(blocks, P, F, tg, st);
     return cudaGetLastError();
 }
 
