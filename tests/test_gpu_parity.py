@@ -335,6 +335,25 @@ def test_small_candidate_capacity_forces_overflow_and_growth(cs):
     assert st["compactions"] >= 2
 
 
+def test_multiscale_overflow_with_an_empty_scale(cs):
+    """Four grids, excursion sets only (k = 0), a threshold that only the coarser grids reach, capacity 1024: the lists of
+    the coarse grids overflow, every scale is compacted in one launch (cs_select.cu, select_compact_batch) -- among them
+    lists that hold nothing -- chunks are re-run and the buffers grow.  The sets must equal the oracle's."""
+    wl, xyz = _gen("cfg5", 1 << 20)
+    host = xyz.cpu().numpy()
+    o = ora.OracleSketch(wl.d, wl.w, wl.G, wl.L, wl.seed)
+    o.update(host)
+    o.scan_begin()
+    o.scan(host)
+    top = [int(o.topk(1, s)[1][0]) for s in range(len(wl.G))]
+    o.close()
+    thr = min(top) + 1                                     # above every estimate of at least one grid (the finest)
+    if max(top) < thr + 2:
+        pytest.skip("the grids of this stream reach the same estimates")
+    _check_all(cs, wl, xyz, k=0, thresholds=(thr, thr + 2), cap=1024)
+    _check_all(cs, wl, xyz, k=50, thresholds=(thr,), cap=1024, split=[300001])
+
+
 def test_heavy_duplication_single_cell(cs):
     """All particles in one cell: every scanned particle is a duplicate candidate."""
     from paper_1711_00975_b200 import synth
