@@ -227,7 +227,9 @@ int cs_scan_children(cs_sketch* s, int parent_scale, int child_scale, const uint
 
 /* Top-k (made deterministic, R9): the first min(k, #candidates)
  * candidates in (estimate descending, cell id ascending) order.  ids_out / est_out: any pointer, room for k
- * entries; *n_out (host) = number written.  k <= k_max. */
+ * entries; *n_out (host) = number written.  k <= k_max.  The first result call (cs_topk / cs_excursion) after a scan puts
+ * the candidate lists of ALL scales that still wait into their final order, in one launch behind one synchronisation;
+ * later result calls on any scale only copy. */
 int cs_topk(cs_sketch* s, int scale, uint64_t k, uint64_t* ids_out, int32_t* est_out, uint64_t* n_out);
 
 /* Excursion set (R8): every candidate with estimate >= thr, same order.  Writes the
