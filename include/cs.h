@@ -113,7 +113,9 @@ int cs_set_table_budget(cs_sketch* s, uint64_t bytes);
 /* How the passes cut one call into launches (0 = keep the current value); the result never depends on it.
  *   stage_particles  particles per batch of the host-streamed calls = size of one slot of the device staging ring
  *                    (default 2^24: 3 slots x 192 MiB); changing it frees the ring, which is re-allocated on use
- *   update_chunk     particles per scatter/apply pair of the binned update (default 2^27; record scratch ~ 8 B each)
+ *   update_chunk     particles per scatter/apply pair of the binned update (default 2^30, halved down to 2^27 while the
+ *                    record scratch -- 2 B x binned rows per particle, 8.6 GB for 2^30 particles at d = 7 -- would take
+ *                    more than a quarter of the free device memory)
  *   scan_chunk       most particles one re-scan launch covers (default 2^27)
  *   compact_chunk    particles per sampling-compaction launch when sample_p < 0.5 (default 2^28)
  * Each a multiple of 4 in [64, 2^30].  Small values make short streams take the multi-batch paths (tests do). */
