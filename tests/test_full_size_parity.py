@@ -1,5 +1,5 @@
 """Full-size parity against the oracle (SURVEY section 4 tier T3, 8.d.4), in the launch configuration bench.py times:
-cfg 3 and cfg 5 at N = 2^30 device-resident (automatic update / scan modes, 8 binned chunks, ~12 scan chunks) and three
+cfg 3 and cfg 5 at N = 2^30 device-resident (automatic update / scan modes, one binned update chunk, ~12 scan chunks) and three
 2^28-particle batches of cfg 4 through the host-streamed calls with the default 2^24-particle staging ring (48 batches:
 every slot is reused 16 times).  The oracle side is tests/sharded_oracle.py: the plain oracle over P disjoint index
 ranges, tables summed, lists merged by its own rule (valid by PAPER.md:578; pinned in tests/test_oracle_pins.py).
